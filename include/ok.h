@@ -1,0 +1,140 @@
+/* ok.h -- C-ABI of libokdirac: the precalculated-W Oktay-Kronfeld Dirac apply, the W
+ * precalculation and BiCGStab, on one NVIDIA B200 (sm_100a).
+ *
+ * Reference: arXiv:1311.5029, Sec. 2.  Problem statement:
+ *   - Eq. (2.1): solve  sum_{y,beta,b} M^{alpha beta,ab}_{xy} psi^{beta b}_y = xi^{alpha a}_x ;
+ *   - Eq. (2.2): M psi is a 27-term stencil, each term a per-site 12x12 complex spin-colour
+ *     matrix W ("precalculation matrix") times the 12-spinor at x + offset;
+ *   - "The W matrices remain the same for all CG iterations. We precalculate and reuse them."
+ * Hence the three calls: ok_precalc_W (links -> W), ok_dirac_apply (W, psi -> M psi),
+ * ok_bicgstab (W, xi -> psi; "bi-stabilized CG").
+ *
+ * General rules
+ *   - Every data pointer is a DEVICE pointer (cudaMalloc'ed / torch CUDA tensor), 16-byte
+ *     aligned, unless the argument is documented as HOST.  `ok_params*`, `iters`, `resid`
+ *     are HOST pointers.
+ *   - The caller owns every buffer.  The library allocates no persistent device memory and
+ *     frees nothing; scratch comes from the buffer given to ok_set_workspace.
+ *   - All work is enqueued on the stream given to ok_set_stream (default: the legacy default
+ *     stream).  Calls are asynchronous except ok_bicgstab, ok_*_host and the first use of a W
+ *     buffer the library has not seen (one 1 KiB header read), which synchronise that stream.
+ *   - Return value: 0 (OK_SUCCESS) or a negative ok_status.  No exceptions, no aborts.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns OK_ECUDA.
+ *
+ * Canonical (external) layouts, complex numbers interleaved (re, im):
+ *   site index   n = x + Lx*(y + Ly*(z + Lz*t)),  dims = {Lx, Ly, Lz, T};  V = Lx*Ly*Lz*T
+ *   links        double  U[n][mu][a][b][2]   mu = 0,1,2 (x,y,z), 3 (t); U_mu(x) joins x to x+mu;
+ *                always fp64 (the precalculation computes in fp64 and rounds W once)
+ *   spinor       real    psi[n][3*alpha+a][2]            (alpha = spin 0..3, a = colour 0..2)
+ *   multi-RHS    real    psi[n][3*alpha+a][rhs][2]       (nrhs = 12)
+ *   W            real    W[n][term][3*alpha+a][3*beta+b][2]   term order below
+ *   `real` is float for OK_FP32 and double for OK_FP64.
+ *
+ * Stencil term order (Eq. 2.2), offsets in lattice units (dx,dy,dz,dt):
+ *   0: 0 | 1,2: +x,-x | 3,4: +y,-y | 5,6: +z,-z | 7,8: +t,-t | 9,10: +2x,-2x | 11,12: +2y,-2y |
+ *   13,14: +2z,-2z | then for (i,j) = (x,y),(x,z),(y,z): +i+j, -i-j, +i-j, -i+j  (15..26).
+ *   out(x) = sum_term W_term(x) psi(x + offset_term), coordinates modulo dims.  Boundary
+ *   conditions (bc) are folded into W by ok_precalc_W; ok_dirac_apply is purely periodic.
+ *
+ * Internal (device) layouts -- what psi/out/src/x/W of the three main calls hold.  Sites are
+ * grouped in blocks of 32 consecutive site indices (the last block zero-padded):
+ *   spinor  [block][c][site_in_block][16 bytes]   fp32: c = 0..5, (re,im) of components 2c, 2c+1
+ *                                                 fp64: c = 0..11, (re,im) of component c
+ *   W       1024-byte header, then [block][term][row 0..11][c][site_in_block][16 bytes]
+ *           with c pairing the COLUMNS of W exactly as the spinor pairs components.
+ *   nrhs=12 spinor: [block][component 0..11][site_in_block][rhs 0..11][re,im] (fp32 only).
+ *   Use ok_pack_ and ok_unpack_ to convert; the sizes are given by ok_vec_bytes and ok_W_bytes.
+ */
+#ifndef OK_H_
+#define OK_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OK_FP32 0
+#define OK_FP64 1
+
+#define OK_NTERMS 27
+#define OK_SITE_BLOCK 32
+#define OK_W_HEADER_BYTES 1024
+
+typedef enum ok_status {
+  OK_SUCCESS = 0,
+  OK_EINVAL = -1,      /* bad dims / precision / nrhs / null or misaligned pointer / unknown W   */
+  OK_ECUDA = -2,       /* CUDA runtime or launch error; text via ok_strerror(OK_ECUDA)           */
+  OK_EBREAKDOWN = -3,  /* BiCGStab breakdown: |rho|, |<rhat,v>|, <t,t> or |omega| < 1e-300 / NaN */
+  OK_EMAXIT = -4,      /* BiCGStab did not converge in maxit iterations (x, iters, resid valid)   */
+  OK_EWORKSPACE = -5   /* workspace missing or smaller than ok_work_bytes                        */
+} ok_status;
+
+typedef struct ok_params {
+  int32_t dims[4];    /* Lx, Ly, Lz, T; each >= 2                                              */
+  int32_t precision;  /* OK_FP32 / OK_FP64: storage and arithmetic of W and spinors            */
+  int32_t bc[4];      /* +1 periodic, -1 antiperiodic (fermion field); paper: {+1,+1,+1,-1}    */
+  int32_t nrhs;       /* 1, or 12 for the multi-right-hand-side mode (fp32 only)               */
+  double kappa, u0;   /* hopping parameter, tadpole factor (Eq. 2.6)                           */
+  double zeta, rs;    /* Eqs. (2.6)-(2.8)                                                      */
+  double cB, cE, cEE, c1, c2, c3, c4, c5;
+} ok_params;
+
+/* ---- sizes (pure host arithmetic; 0 on invalid params) ---------------------------------- */
+size_t ok_W_bytes(const ok_params* p);    /* device bytes of W incl. header and block padding   */
+size_t ok_vec_bytes(const ok_params* p);  /* device bytes of one spinor field, internal layout  */
+size_t ok_work_bytes(const ok_params* p); /* workspace needed by ok_precalc_W, ok_bicgstab, ok_*_host */
+
+/* ---- execution context ------------------------------------------------------------------ */
+int ok_set_stream(void* cuda_stream);             /* cudaStream_t as void*; NULL = default stream */
+int ok_set_workspace(void* dev, size_t bytes);    /* DEVICE scratch, caller-owned, 256-B aligned  */
+
+/* ---- layout conversion (device -> device, asynchronous) --------------------------------- */
+int ok_pack_spinor(const ok_params* p, const void* canon, void* packed);
+int ok_unpack_spinor(const ok_params* p, const void* packed, void* canon);
+/* canonical W [n][27][12][12] (precision of p) <-> internal W; ok_pack_W also writes the header.
+ * Lets a caller inject precalculation matrices computed elsewhere, or inspect them. */
+int ok_pack_W(const ok_params* p, const void* canon_W, void* W);
+int ok_unpack_W(const void* W, void* canon_W);
+
+/* ---- the hot path ------------------------------------------------------------------------ */
+
+/* Precalculation, PAPER.md:59, 89-107 (Eqs. 2.6-2.12, 2.3, 2.10): builds the 27 matrices per
+ * site from SU(3) links (canonical layout, fp64) and writes them, with the header, into W
+ * (ok_W_bytes).  Arithmetic in fp64; W rounded once to p->precision.  Needs the workspace. */
+int ok_precalc_W(const void* links, const ok_params* params, void* W);
+
+/* Dirac apply, PAPER.md:53-55 (Eq. 2.2): out = M psi.  psi, out: internal spinor layout,
+ * out must not alias psi.  Dimensions/precision are taken from W's header. */
+int ok_dirac_apply(const void* W, const void* psi, void* out);
+
+/* BiCGStab: solves M x = src (x0 = 0; x on entry ignored), unpreconditioned,
+ * reductions and scalars in fp64 with a fixed summation order (bit-reproducible).  Stops when
+ * the recursive residual satisfies ||r|| <= tol ||src|| AND the recomputed true residual does
+ * too (otherwise restarts from the true residual).  *iters = BiCGStab iterations (2 applies
+ * each); *resid = true relative residual ||src - M x|| / ||src|| at exit.  nrhs = 12: every
+ * column has its own scalars; converged columns are frozen; *iters = max over columns and
+ * *resid = max over columns.  iters/resid: HOST pointers.  Needs the workspace. */
+int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, int* iters, double* resid);
+
+/* Same apply with HOST spinors in the canonical layout (precision of W): copies psi to the
+ * device, packs, applies, unpacks and copies back, synchronising the stream.  W stays
+ * device-resident across calls (the paper keeps the precalculation matrices on the GPU and
+ * copies the fermion field every call).  Needs the workspace. */
+int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host);
+
+/* ---- diagnostics -------------------------------------------------------------------------- */
+/* Read the parameters stored in W's header back into *p (HOST). */
+int ok_W_params(const void* W, ok_params* p);
+/* Number of kernels the library has launched since load (for launch accounting in benches). */
+uint64_t ok_launch_count(void);
+/* Select the apply kernel variant (0 = default).  Tuning knob; results are identical. */
+int ok_set_apply_variant(int variant);
+const char* ok_strerror(int status);
+const char* ok_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OK_H_ */

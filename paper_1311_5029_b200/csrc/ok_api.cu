@@ -1,0 +1,234 @@
+// C-ABI entry points of libokdirac (include/ok.h): argument checks, sizes, handle table.
+// Every step of the hot path runs in the CUDA kernels of the other translation units.
+#include <mutex>
+#include <string.h>
+#include <unordered_map>
+
+#include "ok_internal.cuh"
+
+namespace okd {
+
+const int8_t kOffsets[kTerms][4] = {
+    {0, 0, 0, 0},
+    {1, 0, 0, 0},  {-1, 0, 0, 0}, {0, 1, 0, 0},  {0, -1, 0, 0}, {0, 0, 1, 0},  {0, 0, -1, 0},
+    {0, 0, 0, 1},  {0, 0, 0, -1},
+    {2, 0, 0, 0},  {-2, 0, 0, 0}, {0, 2, 0, 0},  {0, -2, 0, 0}, {0, 0, 2, 0},  {0, 0, -2, 0},
+    {1, 1, 0, 0},  {-1, -1, 0, 0}, {1, -1, 0, 0}, {-1, 1, 0, 0},
+    {1, 0, 1, 0},  {-1, 0, -1, 0}, {1, 0, -1, 0}, {-1, 0, 1, 0},
+    {0, 1, 1, 0},  {0, -1, -1, 0}, {0, 1, -1, 0}, {0, -1, 1, 0}};
+
+Ctx& ctx() {
+  static Ctx c;
+  return c;
+}
+
+int fail_cuda(cudaError_t e, const char* where) {
+  snprintf(ctx().err, sizeof(ctx().err), "CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), where);
+  return OK_ECUDA;
+}
+
+bool valid_params(const ok_params* p) {
+  if (!p) return false;
+  long long V = 1;
+  for (int d = 0; d < 4; ++d) {
+    if (p->dims[d] < 2 || p->dims[d] > 4096) return false;
+    if (p->bc[d] != 1 && p->bc[d] != -1) return false;
+    V *= p->dims[d];
+  }
+  if (V > (1LL << 30)) return false;
+  if (p->precision != OK_FP32 && p->precision != OK_FP64) return false;
+  if (p->nrhs != 1 && p->nrhs != 12) return false;
+  if (p->nrhs == 12 && p->precision != OK_FP32) return false;
+  if (!(p->kappa > 0.0) || !(p->u0 > 0.0)) return false;
+  return true;
+}
+
+Geom make_geom(const ok_params* p) {
+  Geom g;
+  g.V = 1;
+  for (int d = 0; d < 4; ++d) {
+    g.L[d] = p->dims[d];
+    g.V *= p->dims[d];
+  }
+  g.nblk = (g.V + kBlock - 1) / kBlock;
+  return g;
+}
+
+static std::mutex g_mu;
+static std::unordered_map<const void*, ok_params> g_table;
+
+int remember_W(const void* W, const ok_params* p) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  g_table[W] = *p;
+  return OK_SUCCESS;
+}
+
+int lookup_W(const void* W, ok_params* p) {
+  if (!aligned16(W)) return OK_EINVAL;
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_table.find(W);
+    if (it != g_table.end()) {
+      *p = it->second;
+      return OK_SUCCESS;
+    }
+  }
+  WHeader h;
+  OK_CUDA(cudaMemcpyAsync(&h, W, sizeof(h), cudaMemcpyDeviceToHost, ctx().stream));
+  OK_CUDA(cudaStreamSynchronize(ctx().stream));
+  if (h.magic != kMagic || h.layout != kLayoutDense || !valid_params(&h.p)) return OK_EINVAL;
+  remember_W(W, &h.p);
+  *p = h.p;
+  return OK_SUCCESS;
+}
+
+static int write_header(void* W, const ok_params* p) {
+  // Staged through a static pinned-free host copy: cudaMemcpyAsync from pageable memory copies
+  // the source before returning, so a stack object is safe here.
+  char buf[OK_W_HEADER_BYTES];
+  memset(buf, 0, sizeof(buf));
+  WHeader h;
+  h.magic = kMagic;
+  h.layout = kLayoutDense;
+  h.p = *p;
+  memcpy(buf, &h, sizeof(h));
+  OK_CUDA(cudaMemcpyAsync(W, buf, sizeof(buf), cudaMemcpyHostToDevice, ctx().stream));
+  return remember_W(W, p);
+}
+
+}  // namespace okd
+
+using namespace okd;
+
+extern "C" {
+
+size_t ok_vec_bytes(const ok_params* p) {
+  if (!valid_params(p)) return 0;
+  Geom g = make_geom(p);
+  return (size_t)g.nblk * kBlock * 12 * 2 * real_bytes(p) * (size_t)p->nrhs;
+}
+
+size_t ok_W_bytes(const ok_params* p) {
+  if (!valid_params(p)) return 0;
+  Geom g = make_geom(p);
+  return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * kTerms * 144 * 2 * real_bytes(p);
+}
+
+size_t ok_work_bytes(const ok_params* p) {
+  if (!valid_params(p)) return 0;
+  size_t a = precalc_work_bytes(p), b = bicgstab_work_bytes(p);
+  size_t host_io = 2 * ok_vec_bytes(p) + 2 * ok_vec_bytes(p);   // ok_dirac_apply_host staging
+  size_t m = a > b ? a : b;
+  return (m > host_io ? m : host_io) + 4096;
+}
+
+int ok_set_stream(void* s) {
+  ctx().stream = static_cast<cudaStream_t>(s);
+  return OK_SUCCESS;
+}
+
+int ok_set_workspace(void* dev, size_t bytes) {
+  if (dev && (reinterpret_cast<uintptr_t>(dev) & 255)) return OK_EINVAL;
+  ctx().work = dev;
+  ctx().work_bytes = dev ? bytes : 0;
+  return OK_SUCCESS;
+}
+
+int ok_set_apply_variant(int v) {
+  if (v < 0 || v > 63) return OK_EINVAL;
+  ctx().apply_variant = v;
+  return OK_SUCCESS;
+}
+
+uint64_t ok_launch_count(void) { return ctx().launches; }
+
+int ok_pack_spinor(const ok_params* p, const void* canon, void* packed) {
+  if (!valid_params(p) || !aligned16(canon) || !aligned16(packed)) return OK_EINVAL;
+  return launch_pack_spinor(p, canon, packed, false);
+}
+
+int ok_unpack_spinor(const ok_params* p, const void* packed, void* canon) {
+  if (!valid_params(p) || !aligned16(canon) || !aligned16(packed)) return OK_EINVAL;
+  return launch_pack_spinor(p, canon, const_cast<void*>(packed), true);
+}
+
+int ok_pack_W(const ok_params* p, const void* canon, void* W) {
+  if (!valid_params(p) || !aligned16(canon) || !aligned16(W)) return OK_EINVAL;
+  int st = write_header(W, p);
+  if (st) return st;
+  return launch_pack_W(p, canon, W_payload(W), false);
+}
+
+int ok_unpack_W(const void* W, void* canon) {
+  ok_params p;
+  if (!aligned16(canon)) return OK_EINVAL;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  return launch_pack_W(&p, canon, const_cast<char*>(W_payload(W)), true);
+}
+
+int ok_W_params(const void* W, ok_params* p) {
+  if (!p) return OK_EINVAL;
+  return lookup_W(W, p);
+}
+
+int ok_precalc_W(const void* links, const ok_params* p, void* W) {
+  if (!valid_params(p) || !aligned16(links) || !aligned16(W)) return OK_EINVAL;
+  if (!ctx().work || ctx().work_bytes < precalc_work_bytes(p)) return OK_EWORKSPACE;
+  int st = write_header(W, p);
+  if (st) return st;
+  return launch_precalc(p, links, W_payload(W), ctx().work);
+}
+
+int ok_dirac_apply(const void* W, const void* psi, void* out) {
+  if (!aligned16(psi) || !aligned16(out) || psi == out) return OK_EINVAL;
+  ok_params p;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  return launch_apply(&p, W_payload(W), psi, out, nullptr, nullptr, nullptr);
+}
+
+int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host) {
+  if (!psi_host || !out_host) return OK_EINVAL;
+  ok_params p;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  size_t vb = ok_vec_bytes(&p);
+  Geom g = make_geom(&p);
+  size_t cb = (size_t)g.V * 12 * 2 * real_bytes(&p) * p.nrhs;   // canonical bytes (no padding)
+  if (!ctx().work || ctx().work_bytes < 4 * vb) return OK_EWORKSPACE;
+  char* w = static_cast<char*>(ctx().work);
+  char *canon_in = w, *packed_in = w + vb, *packed_out = w + 2 * vb, *canon_out = w + 3 * vb;
+  OK_CUDA(cudaMemcpyAsync(canon_in, psi_host, cb, cudaMemcpyHostToDevice, ctx().stream));
+  if ((st = launch_pack_spinor(&p, canon_in, packed_in, false))) return st;
+  if ((st = launch_apply(&p, W_payload(W), packed_in, packed_out, nullptr, nullptr, nullptr))) return st;
+  if ((st = launch_pack_spinor(&p, canon_out, packed_out, true))) return st;
+  OK_CUDA(cudaMemcpyAsync(out_host, canon_out, cb, cudaMemcpyDeviceToHost, ctx().stream));
+  OK_CUDA(cudaStreamSynchronize(ctx().stream));
+  return OK_SUCCESS;
+}
+
+int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, int* iters, double* resid) {
+  if (!aligned16(src) || !aligned16(x) || src == x || !iters || !resid || !(tol > 0.0) || maxit < 1) return OK_EINVAL;
+  ok_params p;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  if (!ctx().work || ctx().work_bytes < bicgstab_work_bytes(&p)) return OK_EWORKSPACE;
+  return run_bicgstab(&p, W_payload(W), src, x, tol, maxit, iters, resid);
+}
+
+const char* ok_strerror(int status) {
+  switch (status) {
+    case OK_SUCCESS: return "success";
+    case OK_EINVAL: return "invalid argument (dims, precision, nrhs, null/misaligned pointer, or unknown W buffer)";
+    case OK_ECUDA: return ctx().err;
+    case OK_EBREAKDOWN: return "BiCGStab breakdown";
+    case OK_EMAXIT: return "BiCGStab: maximum iterations reached without convergence";
+    case OK_EWORKSPACE: return "workspace missing or too small (see ok_work_bytes / ok_set_workspace)";
+    default: return "unknown status";
+  }
+}
+
+const char* ok_version(void) { return "okdirac 0.1 (sm_100a)"; }
+
+}  // extern "C"

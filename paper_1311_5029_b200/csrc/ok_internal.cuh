@@ -1,0 +1,81 @@
+// Internal declarations shared by the translation units of libokdirac (not part of the ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "ok.h"
+
+namespace okd {
+
+constexpr int kBlock = OK_SITE_BLOCK;   // sites per block (= warp width: lane <-> site)
+constexpr int kTerms = OK_NTERMS;
+constexpr uint32_t kMagic = 0x4F4B5731u;   // "OKW1"
+constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
+
+struct Geom {
+  int L[4];
+  int V;      // sites
+  int nblk;   // ceil(V / 32)
+};
+
+struct WHeader {         // first OK_W_HEADER_BYTES of a W buffer (device) and its host mirror
+  uint32_t magic;
+  uint32_t layout;
+  ok_params p;
+};
+static_assert(sizeof(WHeader) <= OK_W_HEADER_BYTES, "header too large");
+
+struct Ctx {
+  cudaStream_t stream = nullptr;
+  void* work = nullptr;
+  size_t work_bytes = 0;
+  int apply_variant = 0;
+  uint64_t launches = 0;
+  char err[512] = "no error";
+};
+Ctx& ctx();
+
+int fail_cuda(cudaError_t e, const char* where);
+
+#define OK_CUDA(call)                                         \
+  do {                                                        \
+    cudaError_t e__ = (call);                                 \
+    if (e__ != cudaSuccess) return okd::fail_cuda(e__, #call); \
+  } while (0)
+
+#define OK_LAUNCHED(name)                                         \
+  do {                                                            \
+    okd::ctx().launches++;                                        \
+    cudaError_t e__ = cudaGetLastError();                         \
+    if (e__ != cudaSuccess) return okd::fail_cuda(e__, name);     \
+  } while (0)
+
+bool valid_params(const ok_params* p);
+Geom make_geom(const ok_params* p);
+inline size_t real_bytes(const ok_params* p) { return p->precision == OK_FP64 ? 8 : 4; }
+inline bool aligned16(const void* q) { return q && (reinterpret_cast<uintptr_t>(q) & 15) == 0; }
+
+// W handle table: header mirror keyed by device pointer (filled by pack/precalc, or by one
+// synchronous header read the first time an unknown pointer is seen).
+int remember_W(const void* W, const ok_params* p);
+int lookup_W(const void* W, ok_params* p);
+inline const char* W_payload(const void* W) { return static_cast<const char*>(W) + OK_W_HEADER_BYTES; }
+inline char* W_payload(void* W) { return static_cast<char*>(W) + OK_W_HEADER_BYTES; }
+
+// Stencil offsets in the term order of ok.h (host copy; device copies live in each TU).
+extern const int8_t kOffsets[kTerms][4];
+
+// ---- launchers (each enqueues on ctx().stream and returns an ok_status) -------------------
+int launch_pack_spinor(const ok_params* p, const void* canon, void* packed, bool unpack);
+int launch_pack_W(const ok_params* p, const void* canon, void* Wpayload, bool unpack);
+int launch_apply(const ok_params* p, const void* Wpayload, const void* psi, void* out,
+                 double* dot_partials /* nullable */, const void* dot_a, const void* dot_b);
+int launch_precalc(const ok_params* p, const void* links, void* Wpayload, void* work);
+size_t precalc_work_bytes(const ok_params* p);
+int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
+                 int* iters, double* resid);
+size_t bicgstab_work_bytes(const ok_params* p);
+
+}  // namespace okd

@@ -1,0 +1,409 @@
+// W precalculation: the 27 "precalculation matrices" of Eq. (2.2) from
+// SU(3) links, Eqs. (2.6)-(2.9), (2.11), (2.12) for the 14 positive matrices and the conjugation
+// relations (2.3), (2.10) for the 13 negative ones.  One-time cost, bound by the W write.
+//
+// Arithmetic is fp64 throughout; W is rounded once to the storage precision.
+//
+// Representation: every 6x6 block of the paper is a Pauli combination  sum_{k=0..3} sigma_k (x) C_k
+// (sigma_0 = 1) of four 3x3 colour matrices C_k.  The kernel computes the C_k ("P4") of the
+// diagonal block A and of the off-diagonal block B of a term, from which the 12x12 entries follow:
+//   (a,a')=(0,0): C0+C3   (1,1): C0-C3   (0,1): C1 - i C2   (1,0): C1 + i C2 .
+// With B_k, E_k the clover fields (DESIGN.md R-F), U = U_i(x), cyclic (i,k,l), Eq. (2.8) reduces to
+//   S^+_i: C0 = i cs (U B_i(x+i) + B_i(x) U), C_i = (zeta-2c1-12c2)/2 U,
+//          C_k = cs (U B_l(x+i) - B_l(x) U),  C_l = -cs (U B_k(x+i) - B_k(x) U),   cs = c3/(2 u0^4)
+//   D^+_i: C0 = -(rs zeta+8c4)/2 U, C_i = 0,
+//          C_k =  i cg G_l + i c5/u0^4 (U B_k(x+i) + B_k(x) U),
+//          C_l = -i cg G_k + i c5/u0^4 (U B_l(x+i) + B_l(x) U),   cg = (c5/4)(u0^-2 - u0^-4),
+//   G_m = U_m(x)U_i(x+m)U_m(x+i)^dag - U_m(x-m)^dag U_i(x-m) U_m(x-m+i)   (staples).
+// Negative matrices are NOT read from another site's W: the positive blocks are recomputed at
+// the shifted site and conjugated, so the kernel has no inter-site dependency.
+// Boundary conditions: U_mu(x) is multiplied by bc[mu] on the last slice of axis mu at load
+// time (DESIGN.md R-BC); closed loops are unaffected, every hop across the boundary gets one sign.
+#include "ok_internal.cuh"
+
+namespace okd {
+
+struct cm3 {
+  double2 e[9];
+};
+
+struct PrecalcArgs {
+  Geom g;
+  int bc[4];
+  int Vpad;
+  double mass;                 // u0 / (2 kappa)
+  double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
+  double s4;                   // c_EE / (2 u0^4)      (Eq. 2.7)
+  double a1, cs, d1, cg, c5u;  // Eq. (2.8)
+  double dii, sii;             // c4/u0, (c1+2c2)/(2u0) (Eq. 2.9)
+  double sij;                  // c2/(2u0)             (Eqs. 2.11, 2.12)
+};
+
+__constant__ int8_t c_poff[kTerms][4];
+static bool g_poff_uploaded = false;
+
+// ------------------------------------------------------------------------- complex 3x3 algebra
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cmulc(double2 a, double2 b) { return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }   // a * conj(b)
+__device__ __forceinline__ double2 cconjmul(double2 a, double2 b) { return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }  // conj(a) * b
+
+__device__ __forceinline__ cm3 zero3() {
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) r.e[i] = make_double2(0.0, 0.0);
+  return r;
+}
+__device__ cm3 mul(const cm3& A, const cm3& B) {   // A B
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double2 s = cmul(A.e[3 * i], B.e[j]);
+#pragma unroll
+      for (int k = 1; k < 3; ++k) { double2 q = cmul(A.e[3 * i + k], B.e[3 * k + j]); s.x += q.x; s.y += q.y; }
+      r.e[3 * i + j] = s;
+    }
+  return r;
+}
+__device__ cm3 mul_nd(const cm3& A, const cm3& B) {   // A B^dag
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double2 s = cmulc(A.e[3 * i], B.e[3 * j]);
+#pragma unroll
+      for (int k = 1; k < 3; ++k) { double2 q = cmulc(A.e[3 * i + k], B.e[3 * j + k]); s.x += q.x; s.y += q.y; }
+      r.e[3 * i + j] = s;
+    }
+  return r;
+}
+__device__ cm3 mul_dn(const cm3& A, const cm3& B) {   // A^dag B
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      double2 s = cconjmul(A.e[i], B.e[j]);
+#pragma unroll
+      for (int k = 1; k < 3; ++k) { double2 q = cconjmul(A.e[3 * k + i], B.e[3 * k + j]); s.x += q.x; s.y += q.y; }
+      r.e[3 * i + j] = s;
+    }
+  return r;
+}
+__device__ __forceinline__ cm3 adj(const cm3& A) {
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) r.e[3 * i + j] = make_double2(A.e[3 * j + i].x, -A.e[3 * j + i].y);
+  return r;
+}
+// r += (cr + i ci) * A
+__device__ __forceinline__ void axpy(cm3& r, double cr, double ci, const cm3& A) {
+#pragma unroll
+  for (int i = 0; i < 9; ++i) {
+    r.e[i].x += cr * A.e[i].x - ci * A.e[i].y;
+    r.e[i].y += cr * A.e[i].y + ci * A.e[i].x;
+  }
+}
+
+// ------------------------------------------------------------------------- geometry
+struct Site {
+  int c[4];
+};
+__device__ __forceinline__ Site site_of(int n, const Geom& g) {
+  Site s;
+  s.c[0] = n % g.L[0]; n /= g.L[0];
+  s.c[1] = n % g.L[1]; n /= g.L[1];
+  s.c[2] = n % g.L[2];
+  s.c[3] = n / g.L[2];
+  return s;
+}
+__device__ __forceinline__ int index_of(const Site& s, const Geom& g) {
+  return s.c[0] + g.L[0] * (s.c[1] + g.L[1] * (s.c[2] + g.L[2] * s.c[3]));
+}
+__device__ __forceinline__ Site shift(Site s, int mu, int d, const Geom& g) {   // |d| <= L
+  int v = s.c[mu] + d;
+  v += (v < 0) ? g.L[mu] : 0;
+  v -= (v >= g.L[mu]) ? g.L[mu] : 0;
+  s.c[mu] = v;
+  return s;
+}
+
+// U_mu(x) with the boundary-condition sign folded in.
+__device__ __forceinline__ cm3 ldU(const double2* __restrict__ links, const Site& s, int mu, const PrecalcArgs& a) {
+  const double2* p = links + ((size_t)index_of(s, a.g) * 4 + mu) * 9;
+  const double sg = (a.bc[mu] < 0 && s.c[mu] == a.g.L[mu] - 1) ? -1.0 : 1.0;
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) {
+    double2 v = __ldg(p + i);
+    r.e[i] = make_double2(sg * v.x, sg * v.y);
+  }
+  return r;
+}
+__device__ __forceinline__ cm3 ldF(const cm3* __restrict__ FS, int k, const Site& s, const PrecalcArgs& a) {
+  const double2* p = reinterpret_cast<const double2*>(FS + (size_t)k * a.Vpad + index_of(s, a.g));
+  cm3 r;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) r.e[i] = __ldg(p + i);
+  return r;
+}
+
+// ------------------------------------------------------------------------- step a1: clover F
+// FS[k][n]: k = 0..2 -> B_1,B_2,B_3 = F_23, F_31, F_12 ; k = 3..5 -> E_i = F_4i   (anti-Hermitian,
+// F = (Q - Q^dag)/8, Q = sum of the four leaves starting and ending at x, no trace subtraction).
+__global__ void __launch_bounds__(128) field_strength_kernel(const double2* __restrict__ links, cm3* __restrict__ FS, PrecalcArgs a) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  const int k = blockIdx.y;
+  if (n >= a.g.V) return;
+  int mu, nu;
+  if (k < 3) { mu = (k + 1) % 3; nu = (k + 2) % 3; } else { mu = 3; nu = k - 3; }
+  const Site x = site_of(n, a.g);
+  const Site xpm = shift(x, mu, 1, a.g), xpn = shift(x, nu, 1, a.g);
+  const Site xmm = shift(x, mu, -1, a.g), xmn = shift(x, nu, -1, a.g);
+  const Site xmmpn = shift(xmm, nu, 1, a.g), xmmmn = shift(xmm, nu, -1, a.g), xpmmn = shift(xpm, nu, -1, a.g);
+  cm3 Q, T;
+  // U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+  T = mul(ldU(links, x, mu, a), ldU(links, xpm, nu, a));
+  T = mul_nd(T, ldU(links, xpn, mu, a));
+  Q = mul_nd(T, ldU(links, x, nu, a));
+  // U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+  T = mul_nd(ldU(links, x, nu, a), ldU(links, xmmpn, mu, a));
+  T = mul_nd(T, ldU(links, xmm, nu, a));
+  T = mul(T, ldU(links, xmm, mu, a));
+  axpy(Q, 1.0, 0.0, T);
+  // U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+  T = mul_dn(ldU(links, xmm, mu, a), adj(ldU(links, xmmmn, nu, a)));
+  T = mul(T, ldU(links, xmmmn, mu, a));
+  T = mul(T, ldU(links, xmn, nu, a));
+  axpy(Q, 1.0, 0.0, T);
+  // U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+  T = mul_dn(ldU(links, xmn, nu, a), ldU(links, xmn, mu, a));
+  T = mul(T, ldU(links, xpmmn, nu, a));
+  T = mul_nd(T, ldU(links, x, mu, a));
+  axpy(Q, 1.0, 0.0, T);
+  cm3 F;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      F.e[3 * i + j].x = (Q.e[3 * i + j].x - Q.e[3 * j + i].x) * 0.125;
+      F.e[3 * i + j].y = (Q.e[3 * i + j].y + Q.e[3 * j + i].y) * 0.125;
+    }
+  FS[(size_t)k * a.Vpad + n] = F;
+}
+
+// ------------------------------------------------------------------------- step a2: W assembly
+struct P4 {
+  cm3 c[4];
+};
+
+// Positive blocks of the term family at site x.  A = diagonal block, B = off-diagonal block.
+//   fam 0: W^0 (Eq. 2.6)   fam 1: W^+_4 (2.7)   fam 2: W^+_i (2.8)   fam 3: W^++_ii (2.9)
+//   fam 4: W^++_ij (2.11)  fam 5: W^+-_ij (2.12)
+__device__ void positive_blocks(int fam, int i, int j, const Site& x, const double2* __restrict__ links,
+                                const cm3* __restrict__ FS, const PrecalcArgs& a, P4& A, P4& B) {
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { A.c[k] = zero3(); B.c[k] = zero3(); }
+  if (fam == 0) {
+    for (int m = 0; m < 3; ++m) {
+      axpy(A.c[m + 1], 0.0, a.d0, ldF(FS, m, x, a));       // D^0 = d0 * i sum sigma_m B_m
+      axpy(B.c[m + 1], a.s0, 0.0, ldF(FS, 3 + m, x, a));   // S^0 = s0 * sum sigma_m E_m
+    }
+  } else if (fam == 1) {
+    const cm3 U = ldU(links, x, 3, a);
+    const Site xp = shift(x, 3, 1, a.g);
+    for (int m = 0; m < 3; ++m) {
+      axpy(B.c[m + 1], a.s4, 0.0, mul(U, ldF(FS, 3 + m, xp, a)));
+      axpy(B.c[m + 1], -a.s4, 0.0, mul(ldF(FS, 3 + m, x, a), U));
+    }
+    axpy(A.c[0], -1.0, 0.0, U);
+  } else if (fam == 2) {
+    const int k = (i + 1) % 3, l = (i + 2) % 3;
+    const cm3 U = ldU(links, x, i, a);
+    const Site xp = shift(x, i, 1, a.g);
+    axpy(B.c[i + 1], a.a1, 0.0, U);
+    axpy(A.c[0], a.d1, 0.0, U);
+    {   // m = i : only the sum enters (S, C0)
+      cm3 P = mul(U, ldF(FS, i, xp, a));
+      axpy(P, 1.0, 0.0, mul(ldF(FS, i, x, a), U));
+      axpy(B.c[0], 0.0, a.cs, P);
+    }
+    {   // m = k : Dif_k -> S.C_l (minus), Sum_k -> D.C_k
+      const cm3 P = mul(U, ldF(FS, k, xp, a)), Q = mul(ldF(FS, k, x, a), U);
+      axpy(B.c[l + 1], -a.cs, 0.0, P); axpy(B.c[l + 1], a.cs, 0.0, Q);
+      axpy(A.c[k + 1], 0.0, a.c5u, P); axpy(A.c[k + 1], 0.0, a.c5u, Q);
+    }
+    {   // m = l : Dif_l -> S.C_k (plus), Sum_l -> D.C_l
+      const cm3 P = mul(U, ldF(FS, l, xp, a)), Q = mul(ldF(FS, l, x, a), U);
+      axpy(B.c[k + 1], a.cs, 0.0, P); axpy(B.c[k + 1], -a.cs, 0.0, Q);
+      axpy(A.c[l + 1], 0.0, a.c5u, P); axpy(A.c[l + 1], 0.0, a.c5u, Q);
+    }
+    if (a.cg != 0.0) {
+      for (int q = 0; q < 2; ++q) {
+        const int m = q ? l : k;           // staple direction
+        const int tgt = q ? k : l;         // sigma index receiving G_m:  +i cg G_l -> C_k ; -i cg G_k -> C_l
+        const double sgn = q ? 1.0 : -1.0;
+        // up: U_m(x) U_i(x+m) U_m(x+i)^dag
+        cm3 G = mul(ldU(links, x, m, a), ldU(links, shift(x, m, 1, a.g), i, a));
+        G = mul_nd(G, ldU(links, xp, m, a));
+        axpy(A.c[tgt + 1], 0.0, sgn * a.cg, G);
+        // down: U_m(x-m)^dag U_i(x-m) U_m(x-m+i)
+        const Site xm = shift(x, m, -1, a.g);
+        G = mul_dn(ldU(links, xm, m, a), ldU(links, xm, i, a));
+        G = mul(G, ldU(links, shift(xm, i, 1, a.g), m, a));
+        axpy(A.c[tgt + 1], 0.0, -sgn * a.cg, G);
+      }
+    }
+  } else if (fam == 3) {
+    const cm3 P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), i, a));
+    axpy(A.c[0], a.dii, 0.0, P);
+    axpy(B.c[i + 1], a.sii, 0.0, P);
+  } else if (fam == 4) {
+    cm3 P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), j, a));
+    axpy(P, 1.0, 0.0, mul(ldU(links, x, j, a), ldU(links, shift(x, j, 1, a.g), i, a)));
+    axpy(B.c[i + 1], a.sij, 0.0, P);
+    axpy(B.c[j + 1], a.sij, 0.0, P);
+  } else {
+    const Site xmj = shift(x, j, -1, a.g);
+    cm3 P = mul_nd(ldU(links, x, i, a), ldU(links, shift(xmj, i, 1, a.g), j, a));
+    axpy(P, 1.0, 0.0, mul_dn(ldU(links, xmj, j, a), ldU(links, xmj, i, a)));
+    axpy(B.c[i + 1], a.sij, 0.0, P);
+    axpy(B.c[j + 1], -a.sij, 0.0, P);
+  }
+}
+
+// entry (alpha', a ; beta', b) of sum_k sigma_k (x) C_k
+__device__ __forceinline__ double2 pauli_entry(const P4& P, int al, int be, int ab) {
+  const double2 c0 = P.c[0].e[ab], c1 = P.c[1].e[ab], c2 = P.c[2].e[ab], c3 = P.c[3].e[ab];
+  if (al == be) return al == 0 ? make_double2(c0.x + c3.x, c0.y + c3.y) : make_double2(c0.x - c3.x, c0.y - c3.y);
+  // (0,1): c1 - i c2 ; (1,0): c1 + i c2
+  return al == 0 ? make_double2(c1.x + c2.y, c1.y - c2.x) : make_double2(c1.x - c2.y, c1.y + c2.x);
+}
+
+template <typename real> struct WUnit;
+template <> struct WUnit<float> { using type = float4; static constexpr int NC = 6; };
+template <> struct WUnit<double> { using type = double2; static constexpr int NC = 12; };
+
+template <typename real>
+__global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                                            typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
+  using unit_t = typename WUnit<real>::type;
+  constexpr int NC = WUnit<real>::NC;
+  const int lane = threadIdx.x;
+  const int term = blockIdx.y * 9 + threadIdx.y;
+  const int blk = blockIdx.x;
+  const int n = blk * kBlock + lane;
+  unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
+  if (n >= a.g.V) {   // padded site: zeros
+    unit_t z = {};
+    for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
+    return;
+  }
+  // term -> family, directions, sign of the hop
+  int fam, i = 0, j = 0;
+  bool neg = false;
+  if (term == 0) fam = 0;
+  else if (term <= 6) { fam = 2; i = (term - 1) >> 1; neg = ((term - 1) & 1); }
+  else if (term <= 8) { fam = 1; neg = (term == 8); }
+  else if (term <= 14) { fam = 3; i = (term - 9) >> 1; neg = ((term - 9) & 1); }
+  else {
+    const int q = (term - 15) >> 2, w = (term - 15) & 3;   // pair index, (++, --, +-, -+)
+    i = q == 2 ? 1 : 0;
+    j = q == 0 ? 1 : 2;
+    fam = (w < 2) ? 4 : 5;
+    neg = (w & 1);
+  }
+  Site x = site_of(n, a.g);
+  if (neg) {   // positive blocks at x - offset(term_positive) = x + offset(term)
+    for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
+  }
+  P4 A, B;
+  positive_blocks(fam, i, j, x, links, FS, a, A, B);
+  if (neg) {   // Eqs. (2.3), (2.10): A -> A^dag, B -> -B^dag
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      A.c[k] = adj(A.c[k]);
+      cm3 t = adj(B.c[k]);
+#pragma unroll
+      for (int q = 0; q < 9; ++q) B.c[k].e[q] = make_double2(-t.e[q].x, -t.e[q].y);
+    }
+  }
+  // block pattern: UL, LR use A (or 0); UR uses B; LL uses +-B
+  const bool ulA = !(fam == 4 || fam == 5) && !(fam == 1 && !neg);
+  const bool lrA = !(fam == 4 || fam == 5) && !(fam == 1 && neg);
+  const double llsgn = (fam == 0) ? -1.0 : 1.0;
+  const double mass = (fam == 0) ? a.mass : 0.0;
+
+  for (int r = 0; r < 12; ++r) {
+    const int alpha = r / 3, ca = r % 3, bi = alpha >> 1, al = alpha & 1;
+    double2 row[12];
+#pragma unroll
+    for (int col = 0; col < 12; ++col) {
+      const int beta = col / 3, cb = col % 3, bj = beta >> 1, be = beta & 1;
+      double2 v = make_double2(0.0, 0.0);
+      if (bi == bj) {
+        if (bi == 0 ? ulA : lrA) v = pauli_entry(A, al, be, 3 * ca + cb);
+        if (r == col) v.x += mass;
+      } else {
+        v = pauli_entry(B, al, be, 3 * ca + cb);
+        if (bi == 1) { v.x *= llsgn; v.y *= llsgn; }
+      }
+      row[col] = v;
+    }
+    unit_t* dst = Wt + (size_t)r * NC * kBlock;
+    if constexpr (sizeof(real) == 4) {
+#pragma unroll
+      for (int c = 0; c < 6; ++c)
+        dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
+    } else {
+#pragma unroll
+      for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
+    }
+  }
+}
+
+size_t precalc_work_bytes(const ok_params* p) {
+  Geom g = make_geom(p);
+  return (size_t)6 * g.nblk * kBlock * sizeof(cm3);
+}
+
+int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) {
+  if (!g_poff_uploaded) {
+    OK_CUDA(cudaMemcpyToSymbol(c_poff, kOffsets, sizeof(kOffsets)));
+    g_poff_uploaded = true;
+  }
+  PrecalcArgs a;
+  a.g = make_geom(p);
+  for (int d = 0; d < 4; ++d) a.bc[d] = p->bc[d];
+  a.Vpad = a.g.nblk * kBlock;
+  const double u0 = p->u0, u2 = u0 * u0, u3 = u2 * u0, u4 = u2 * u2;
+  a.mass = u0 / (2.0 * p->kappa);
+  a.d0 = -(p->cB * p->zeta + 16.0 * p->c5) / (2.0 * u3);
+  a.s0 = -(p->cE * p->zeta) / (2.0 * u3);
+  a.s4 = p->cEE / (2.0 * u4);
+  a.a1 = 0.5 * (p->zeta - 2.0 * p->c1 - 12.0 * p->c2);
+  a.cs = p->c3 / (2.0 * u4);
+  a.d1 = -0.5 * (p->rs * p->zeta + 8.0 * p->c4);
+  a.cg = 0.25 * p->c5 * (1.0 / u2 - 1.0 / u4);
+  a.c5u = p->c5 / u4;
+  a.dii = p->c4 / u0;
+  a.sii = (p->c1 + 2.0 * p->c2) / (2.0 * u0);
+  a.sij = p->c2 / (2.0 * u0);
+  cm3* FS = static_cast<cm3*>(work);
+  cudaStream_t st = ctx().stream;
+  field_strength_kernel<<<dim3((a.g.V + 127) / 128, 6), 128, 0, st>>>(static_cast<const double2*>(links), FS, a);
+  OK_LAUNCHED("field_strength_kernel");
+  dim3 grid(a.g.nblk, 3), block(32, 9);
+  if (p->precision == OK_FP64)
+    assemble_W_kernel<double><<<grid, block, 0, st>>>(static_cast<const double2*>(links), FS, static_cast<double2*>(Wp), a);
+  else
+    assemble_W_kernel<float><<<grid, block, 0, st>>>(static_cast<const double2*>(links), FS, static_cast<float4*>(Wp), a);
+  OK_LAUNCHED("assemble_W_kernel");
+  return OK_SUCCESS;
+}
+
+}  // namespace okd
