@@ -171,6 +171,21 @@ def run_reference(args, wl):
 
 
 # ------------------------------------------------------------------------------ our arm
+def max_over_ranks(values, dist, device):
+    """Replicas-only aggregation (DESIGN.md 8): every rank times the same workload on its own GPU;
+    the job's time is the slowest rank's.  `dist` is torch.distributed (initialised) or None."""
+    import torch
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_value(world, alg_bytes, apply_ms):
+    """Whole-job GB/s of `world` replicas that each moved alg_bytes in apply_ms (max over ranks)."""
+    return world * alg_bytes / (apply_ms * 1e-3) / 1e9
+
+
 def run_ours(args, wl):
     import torch
     from paper_1311_5029_b200 import binding as B
@@ -269,12 +284,9 @@ def run_ours(args, wl):
 
     # ---- max over ranks
     a_ms = float(np.mean(apply_ms))
-    vals = torch.tensor([total_ms, a_ms, e2e_ms, float(np.mean(solve_s))], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
-    total_ms, a_ms, e2e_ms, s_s = [float(v) for v in vals.cpu()]
+    total_ms, a_ms, e2e_ms, s_s = max_over_ranks([total_ms, a_ms, e2e_ms, float(np.mean(solve_s))], dist, dev)
     alg = V * BYTES_PER_SITE[sbytes]
-    value = world * alg / (a_ms * 1e-3) / 1e9
+    value = aggregate_value(world, alg, a_ms)
     peaks = measured_peaks()
 
     if rank == 0:
