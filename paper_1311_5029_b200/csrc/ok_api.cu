@@ -76,7 +76,8 @@ int lookup_W(const void* W, ok_params* p) {
   WHeader h;
   OK_CUDA(cudaMemcpyAsync(&h, W, sizeof(h), cudaMemcpyDeviceToHost, ctx().stream));
   OK_CUDA(cudaStreamSynchronize(ctx().stream));
-  if (h.magic != kMagic || h.layout != kLayoutDense || !valid_params(&h.p)) return OK_EINVAL;
+  if (h.magic != kMagic || !valid_params(&h.p)) return OK_EINVAL;
+  if (h.layout != (h.p.nrhs == 12 ? kLayoutMrhs : kLayoutDense)) return OK_EINVAL;
   remember_W(W, &h.p);
   *p = h.p;
   return OK_SUCCESS;
@@ -89,7 +90,7 @@ static int write_header(void* W, const ok_params* p) {
   memset(buf, 0, sizeof(buf));
   WHeader h;
   h.magic = kMagic;
-  h.layout = kLayoutDense;
+  h.layout = p->nrhs == 12 ? kLayoutMrhs : kLayoutDense;
   h.p = *p;
   memcpy(buf, &h, sizeof(h));
   OK_CUDA(cudaMemcpyAsync(W, buf, sizeof(buf), cudaMemcpyHostToDevice, ctx().stream));
@@ -111,12 +112,13 @@ size_t ok_vec_bytes(const ok_params* p) {
 size_t ok_W_bytes(const ok_params* p) {
   if (!valid_params(p)) return 0;
   Geom g = make_geom(p);
+  if (p->nrhs == 12) return OK_W_HEADER_BYTES + (size_t)g.V * kMrhsWSiteFloats * sizeof(float);
   return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * kTerms * 144 * 2 * real_bytes(p);
 }
 
 size_t ok_work_bytes(const ok_params* p) {
   if (!valid_params(p)) return 0;
-  size_t a = precalc_work_bytes(p), b = bicgstab_work_bytes(p);
+  size_t a = precalc_work_bytes(p), b = p->nrhs == 12 ? bicgstab_mrhs_work_bytes(p) : bicgstab_work_bytes(p);
   size_t host_io = 2 * ok_vec_bytes(p) + 2 * ok_vec_bytes(p);   // ok_dirac_apply_host staging
   size_t m = a > b ? a : b;
   return (m > host_io ? m : host_io) + 4096;
@@ -185,6 +187,7 @@ int ok_dirac_apply(const void* W, const void* psi, void* out) {
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
+  if (p.nrhs == 12) return launch_apply_mrhs(&p, W_payload(W), psi, out);
   return launch_apply(&p, W_payload(W), psi, out, nullptr, nullptr, nullptr);
 }
 
@@ -201,7 +204,9 @@ int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host) {
   char *canon_in = w, *packed_in = w + vb, *packed_out = w + 2 * vb, *canon_out = w + 3 * vb;
   OK_CUDA(cudaMemcpyAsync(canon_in, psi_host, cb, cudaMemcpyHostToDevice, ctx().stream));
   if ((st = launch_pack_spinor(&p, canon_in, packed_in, false))) return st;
-  if ((st = launch_apply(&p, W_payload(W), packed_in, packed_out, nullptr, nullptr, nullptr))) return st;
+  st = p.nrhs == 12 ? launch_apply_mrhs(&p, W_payload(W), packed_in, packed_out)
+                    : launch_apply(&p, W_payload(W), packed_in, packed_out, nullptr, nullptr, nullptr);
+  if (st) return st;
   if ((st = launch_pack_spinor(&p, canon_out, packed_out, true))) return st;
   OK_CUDA(cudaMemcpyAsync(out_host, canon_out, cb, cudaMemcpyDeviceToHost, ctx().stream));
   OK_CUDA(cudaStreamSynchronize(ctx().stream));
@@ -213,6 +218,10 @@ int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, 
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
+  if (p.nrhs == 12) {
+    if (!ctx().work || ctx().work_bytes < bicgstab_mrhs_work_bytes(&p)) return OK_EWORKSPACE;
+    return run_bicgstab_mrhs(&p, W_payload(W), src, x, tol, maxit, iters, resid);
+  }
   if (!ctx().work || ctx().work_bytes < bicgstab_work_bytes(&p)) return OK_EWORKSPACE;
   return run_bicgstab(&p, W_payload(W), src, x, tol, maxit, iters, resid);
 }

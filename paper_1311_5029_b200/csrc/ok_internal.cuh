@@ -13,6 +13,25 @@ constexpr int kBlock = OK_SITE_BLOCK;   // sites per block (= warp width: lane <
 constexpr int kTerms = OK_NTERMS;
 constexpr uint32_t kMagic = 0x4F4B5731u;   // "OKW1"
 constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
+constexpr uint32_t kLayoutMrhs = 2;        // nrhs = 12: per-site tcgen05 A-operand tiles (ok_apply_mrhs.cu)
+
+// ---- nrhs = 12 (tensor-core) layouts, fp32 only -------------------------------------------------
+// W: per site the real-split A operand [W_r ; W_i] (24 x 324, padded to K = 328) in the UMMA K-major
+// no-swizzle canonical order: [row group m/8 = 0..2][k chunk k/4 = 0..81][m%8][k%4], m = 12*part + row,
+// k = 12*term + col; chunk 81 is a zero pad.  31 488 B per site.
+constexpr int kMrhsChunks = 82;
+constexpr int kMrhsWSiteFloats = 3 * kMrhsChunks * 32;
+// spinor: per site the B operand [Psi_r , Psi_i] (24 x 12) as 9 core matrices:
+// [n group n/8 = 0..2][k chunk c/4 = 0..2][n%8][c%4], n = 2*rhs + part, c = component.  1152 B per site.
+constexpr int kMrhsVecSiteFloats = 288;
+__host__ __device__ inline int mrhs_W_index(int term, int row, int col, int part) {
+  const int m = 12 * part + row, k = 12 * term + col;
+  return ((m >> 3) * kMrhsChunks + (k >> 2)) * 32 + (m & 7) * 4 + (k & 3);
+}
+__host__ __device__ inline int mrhs_vec_index(int comp, int rhs, int part) {
+  const int n = 2 * rhs + part;
+  return ((n >> 3) * 3 + (comp >> 2)) * 32 + (n & 7) * 4 + (comp & 3);
+}
 
 struct Geom {
   int L[4];
@@ -77,5 +96,10 @@ size_t precalc_work_bytes(const ok_params* p);
 int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
                  int* iters, double* resid);
 size_t bicgstab_work_bytes(const ok_params* p);
+// nrhs = 12
+int launch_apply_mrhs(const ok_params* p, const void* Wpayload, const void* psi, void* out);
+int run_bicgstab_mrhs(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
+                      int* iters, double* resid);
+size_t bicgstab_mrhs_work_bytes(const ok_params* p);
 
 }  // namespace okd

@@ -24,23 +24,47 @@ __global__ void pack_spinor_kernel(const vec_t* __restrict__ canon, vec_t* __res
   }
 }
 
-// nrhs = 12, fp32: canonical [n][comp][rhs] complex -> internal [block][comp][site][rhs] complex.
-// Unit = float4 = two consecutive rhs; per (site, comp) there are 6 units.
-__global__ void pack_spinor_mrhs_kernel(const float4* __restrict__ canon, float4* __restrict__ packed, int V,
-                                        int nblk, bool unpack) {
+// nrhs = 12, fp32: canonical [n][comp][rhs][re,im] <-> per-site B-operand records (ok_internal.cuh,
+// mrhs_vec_index).  One thread per complex number.
+__global__ void pack_spinor_mrhs_kernel(const float2* __restrict__ canon, float* __restrict__ packed, int V, bool unpack) {
   long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  long long total = (long long)nblk * 12 * kBlock * 6;
-  if (u >= total) return;
-  int q = (int)(u % 6);
-  int s = (int)((u / 6) % kBlock);
-  int comp = (int)((u / (6 * kBlock)) % 12);
-  int b = (int)(u / (6LL * kBlock * 12));
-  int n = b * kBlock + s;
-  long long cu = ((long long)n * 12 + comp) * 6 + q;
+  if (u >= (long long)V * 144) return;
+  const int rhs = (int)(u % 12), comp = (int)((u / 12) % 12);
+  const long long n = u / 144;
+  float* rec = packed + n * kMrhsVecSiteFloats;
+  const int ir = mrhs_vec_index(comp, rhs, 0), ii = mrhs_vec_index(comp, rhs, 1);
   if (unpack) {
-    if (n < V) const_cast<float4*>(canon)[cu] = packed[u];
+    const_cast<float2*>(canon)[u] = make_float2(rec[ir], rec[ii]);
   } else {
-    packed[u] = (n < V) ? canon[cu] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float2 v = canon[u];
+    rec[ir] = v.x;
+    rec[ii] = v.y;
+  }
+}
+
+// nrhs = 12 W: canonical [n][27][12][12][re,im] <-> per-site A-operand tiles (mrhs_W_index); the
+// zero pad chunk (k = 324..327) is written when packing.
+__global__ void pack_W_mrhs_kernel(const float2* __restrict__ canon, float* __restrict__ packed, int V, bool unpack) {
+  constexpr int kPer = kTerms * 144 + 96;
+  long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (u >= (long long)V * kPer) return;
+  const int e = (int)(u % kPer);
+  const long long n = u / kPer;
+  float* tile = packed + n * kMrhsWSiteFloats;
+  if (e >= kTerms * 144) {   // pad chunk: 3 row groups x 32 floats
+    const int q = e - kTerms * 144;
+    if (!unpack) tile[((q >> 5) * kMrhsChunks + (kMrhsChunks - 1)) * 32 + (q & 31)] = 0.f;
+    return;
+  }
+  const int col = e % 12, row = (e / 12) % 12, term = e / 144;
+  const int ir = mrhs_W_index(term, row, col, 0), ii = mrhs_W_index(term, row, col, 1);
+  const long long cu = n * (kTerms * 144) + e;
+  if (unpack) {
+    const_cast<float2*>(canon)[cu] = make_float2(tile[ir], tile[ii]);
+  } else {
+    const float2 v = canon[cu];
+    tile[ir] = v.x;
+    tile[ii] = v.y;
   }
 }
 
@@ -48,9 +72,9 @@ int launch_pack_spinor(const ok_params* p, const void* canon, void* packed, bool
   Geom g = make_geom(p);
   const int T = 256;
   if (p->nrhs == 12) {
-    long long total = (long long)g.nblk * 12 * kBlock * 6;
+    long long total = (long long)g.V * 144;
     pack_spinor_mrhs_kernel<<<(unsigned)((total + T - 1) / T), T, 0, ctx().stream>>>(
-        static_cast<const float4*>(canon), static_cast<float4*>(packed), g.V, g.nblk, unpack);
+        static_cast<const float2*>(canon), static_cast<float*>(packed), g.V, unpack);
     OK_LAUNCHED("pack_spinor_mrhs_kernel");
     return OK_SUCCESS;
   }
@@ -93,6 +117,13 @@ __global__ void pack_W_kernel(const vec_t* __restrict__ canon, vec_t* __restrict
 
 int launch_pack_W(const ok_params* p, const void* canon, void* Wp, bool unpack) {
   Geom g = make_geom(p);
+  if (p->nrhs == 12) {
+    long long tot = (long long)g.V * (kTerms * 144 + 96);
+    pack_W_mrhs_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx().stream>>>(static_cast<const float2*>(canon),
+                                                                                static_cast<float*>(Wp), g.V, unpack);
+    OK_LAUNCHED("pack_W_mrhs_kernel");
+    return OK_SUCCESS;
+  }
   int NC = p->precision == OK_FP64 ? 12 : 6;
   long long total = (long long)g.nblk * kTerms * 12 * NC * kBlock;
   const int T = 256;

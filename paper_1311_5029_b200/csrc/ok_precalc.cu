@@ -31,6 +31,7 @@ struct PrecalcArgs {
   Geom g;
   int bc[4];
   int Vpad;
+  int mrhs;                    // 1: write the nrhs = 12 tensor-core tile layout (ok_internal.cuh)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
   double s4;                   // c_EE / (2 u0^4)      (Eq. 2.7)
@@ -298,6 +299,7 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
   const int blk = blockIdx.x;
   const int n = blk * kBlock + lane;
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
+  if (a.mrhs && n >= a.g.V) return;   // the tile layout has no padded sites
   if (n >= a.g.V) {   // padded site: zeros
     unit_t z = {};
     for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
@@ -356,6 +358,20 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
     }
     unit_t* dst = Wt + (size_t)r * NC * kBlock;
     if constexpr (sizeof(real) == 4) {
+      if (a.mrhs) {   // A-operand tile of ok_apply_mrhs.cu: rows (part, r), k = 12 term + col
+        float* tile = reinterpret_cast<float*>(W) + (size_t)n * kMrhsWSiteFloats;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+          *reinterpret_cast<float4*>(tile + mrhs_W_index(term, r, 4 * q, 0)) =
+              make_float4((float)row[4 * q].x, (float)row[4 * q + 1].x, (float)row[4 * q + 2].x, (float)row[4 * q + 3].x);
+          *reinterpret_cast<float4*>(tile + mrhs_W_index(term, r, 4 * q, 1)) =
+              make_float4((float)row[4 * q].y, (float)row[4 * q + 1].y, (float)row[4 * q + 2].y, (float)row[4 * q + 3].y);
+        }
+        if (term == 0 && r < 3)   // zero pad chunk k = 324..327 of row group r
+          for (int q = 0; q < 8; ++q)
+            *reinterpret_cast<float4*>(tile + (r * kMrhsChunks + kMrhsChunks - 1) * 32 + 4 * q) = make_float4(0.f, 0.f, 0.f, 0.f);
+        continue;
+      }
 #pragma unroll
       for (int c = 0; c < 6; ++c)
         dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
@@ -380,6 +396,7 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   a.g = make_geom(p);
   for (int d = 0; d < 4; ++d) a.bc[d] = p->bc[d];
   a.Vpad = a.g.nblk * kBlock;
+  a.mrhs = p->nrhs == 12;
   const double u0 = p->u0, u2 = u0 * u0, u3 = u2 * u0, u4 = u2 * u2;
   a.mass = u0 / (2.0 * p->kappa);
   a.d0 = -(p->cB * p->zeta + 16.0 * p->c5) / (2.0 * u3);
