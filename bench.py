@@ -40,16 +40,31 @@ sys.path.insert(0, ROOT)
 from paper_1311_5029_b200 import inputs as I  # noqa: E402
 
 METRIC = "OK Dirac apply HBM GB/s (% of B200 peak) + BiCGStab solve s at 20^3x64 fp32"
-BYTES_PER_SITE = {4: 27 * 144 * 2 * 4 + 2 * 24 * 4, 8: 27 * 144 * 2 * 8 + 2 * 24 * 8}   # 31 296 / 62 592
+KERNEL_NAME = {(4, 1): "okd::apply_direct_kernel<float,...>", (8, 1): "okd::apply_direct_kernel<double,...>",
+               (4, 12): "okd::apply_mrhs_kernel (tcgen05 kind::tf32)"}
 FLOP_PER_SITE = 27 * 144 * 8                                                             # 31 104
 NAPPLY = 20
 
 WORKLOADS = {
-    # name: (dims, precision bytes, eps, link seed, source seed, kappa, tol)
+    # name: (dims, precision bytes, eps (None = Haar links), link seed, source seed, kappa, tol)
     "20x20x20x64-fp32": ((20, 20, 20, 64), 4, 0.25, 5, 6, 0.10, 1e-6),      # BASELINE configs[2] (the metric's config)
     "8x8x8x16-fp64": ((8, 8, 8, 16), 8, 0.30, 3, 2, 0.10, 1e-12),           # configs[1] shape, for quick runs
     "4x4x4x8-fp64": ((4, 4, 4, 8), 8, 0.30, 1, 2, 0.10, 1e-10),             # configs[0]
+    "20x20x20x64-fp64": ((20, 20, 20, 64), 8, 0.25, 5, 6, 0.10, 1e-10),     # configs[2] lattice in fp64 (31.9 GB of W)
+    "20x20x20x64-fp32-rhs12": ((20, 20, 20, 64), 4, 0.25, 7, None, 0.10, 1e-6),   # configs[3]: 12 point sources at the origin
+    "32x32x32x64-fp32": ((32, 32, 32, 64), 4, None, 8, 9, 0.08, 1e-6),      # configs[4]: Haar links, 65 GB of W
+    "4x4x4x8-fp32-rhs12": ((4, 4, 4, 8), 4, 0.25, 7, None, 0.10, 1e-6),     # quick check of the 12-RHS mode
 }
+NRHS = {"20x20x20x64-fp32-rhs12": 12, "4x4x4x8-fp32-rhs12": 12}
+
+
+def make_links(dims, eps, lseed):
+    return I.haar_links(dims, lseed) if eps is None else I.near_identity_links(dims, eps, lseed)
+
+
+def alg_bytes_per_site(sbytes, nrhs):
+    """W once + the spinor block read once + written once."""
+    return 27 * 144 * 2 * sbytes + 2 * 24 * sbytes * nrhs
 
 
 def fallback_peaks():
@@ -112,15 +127,16 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------ oracle arm
-def oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=12.0, nsample=4096, U=None):
+def oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=12.0, nsample=4096, U=None, nrhs=1):
     """Times the oracle's stored-W apply (Eq. 2.2) on a bounded sample of the workload's sites.
     Returns dict(value GB/s-equivalent of the fp32 contract bytes, cores, sample, ...)."""
     from oracle.ok_oracle import Oracle   # test infrastructure; allowed here for the CPU baseline only
     if U is None:
-        U = I.near_identity_links(dims, eps, lseed)
+        U = make_links(dims, eps, lseed)
     u0 = I.tadpole_u0(I.mean_plaquette(dims, U))
     o = Oracle(U, I.make_params(dims, kappa, u0))
-    psi = I.gaussian_spinor(dims, sseed)
+    # the apply's cost is data-independent: Gaussian columns stand in for the point sources of the 12-RHS config
+    cols = [I.gaussian_spinor(dims, (sseed if sseed is not None else 6) + j) for j in range(nrhs)]
     V = o.V
     nsample = min(nsample, V)
     idx = (np.arange(nsample) * (V // nsample)).astype(np.int64)      # evenly spread sites
@@ -130,17 +146,19 @@ def oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=12.0, nsample=4096, U
     c0, w0 = time.process_time(), time.perf_counter()
     reps = 0
     while True:
-        o.apply_W(psi, idx=idx, W=W)
+        for psi in cols:
+            o.apply_W(psi, idx=idx, W=W)
         reps += 1
         if time.perf_counter() - w0 > budget_s:
             break
     wall = time.perf_counter() - w0
     cpu = time.process_time() - c0
     sites_per_s = reps * nsample / wall
-    return {"value": sites_per_s * BYTES_PER_SITE[4] / 1e9, "unit": "GB/s", "cores": max(1, int(round(cpu / wall))),
+    return {"value": sites_per_s * alg_bytes_per_site(4, nrhs) / 1e9, "unit": "GB/s", "cores": max(1, int(round(cpu / wall))),
             "kind": "oracle", "host_cores": os.cpu_count(),
             "sample": f"{nsample} evenly spaced sites of the {'x'.join(map(str, dims))} lattice, stored fp64 W, "
-                      f"{reps} applies in {wall:.1f} s (numpy einsum); oracle precalc of the sample took {t_pre:.1f} s",
+                      f"{reps} applies{' of %d columns' % nrhs if nrhs > 1 else ''} in {wall:.1f} s (numpy einsum); "
+                      f"oracle precalc of the sample took {t_pre:.1f} s",
             "sites_per_s": sites_per_s, "applies_per_s_equiv": sites_per_s / V,
             "precalc_sites_per_s": nsample / t_pre}
 
@@ -150,13 +168,14 @@ def run_reference(args, wl):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    U = I.near_identity_links(dims, eps, lseed)
+    U = make_links(dims, eps, lseed)
+    nrhs = NRHS.get(wl, 1)
     per = []
     for _ in range(args.warmup):
-        oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=1.0, nsample=1024, U=U)
+        oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=1.0, nsample=1024, U=U, nrhs=nrhs)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        per.append(oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=4.0, nsample=2048, U=U))
+        per.append(oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=4.0, nsample=2048, U=U, nrhs=nrhs))
     wall = time.perf_counter() - t0
     val = float(np.mean([p["value"] for p in per]))
     cb = dict(per[-1])
@@ -206,13 +225,17 @@ def run_ours(args, wl):
     B.lib()
 
     # ---- inputs (seeded, synthetic; generated on the host, resident in HBM before timing)
-    U = I.near_identity_links(dims, eps, lseed)
+    nrhs = NRHS.get(wl, 1)
+    U = make_links(dims, eps, lseed)
     plaq = I.mean_plaquette(dims, U)
     pd = I.make_params(dims, kappa, I.tadpole_u0(plaq))
-    p = B.make_params(pd, prec)
+    p = B.make_params(pd, prec, nrhs=nrhs)
     V = int(np.prod(dims))
     cdt = torch.complex64 if sbytes == 4 else torch.complex128
-    psi_np = I.gaussian_spinor(dims, sseed)
+    if nrhs == 1:
+        psi_np = I.gaussian_spinor(dims, sseed)
+    else:      # configs[3]: all 12 spin-colour point sources at the origin, canonical [site][comp][rhs]
+        psi_np = np.stack([I.point_source(dims, site=0, comp=j) for j in range(nrhs)], axis=2)
     links = torch.from_numpy(U).to(dev)
     canon = torch.from_numpy(psi_np).to(cdt).to(dev)
     W = B.alloc_W(p, dev)
@@ -280,12 +303,12 @@ def run_ours(args, wl):
         B.ok_dirac_apply_host(W, host_in, host_out)      # synchronises the stream itself
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - e0) / n_e2e
-    io_bytes = V * 12 * 2 * sbytes
+    io_bytes = V * 12 * 2 * sbytes * nrhs
 
     # ---- max over ranks
     a_ms = float(np.mean(apply_ms))
     total_ms, a_ms, e2e_ms, s_s = max_over_ranks([total_ms, a_ms, e2e_ms, float(np.mean(solve_s))], dist, dev)
-    alg = V * BYTES_PER_SITE[sbytes]
+    alg = V * alg_bytes_per_site(sbytes, nrhs)
     value = aggregate_value(world, alg, a_ms)
     peaks = measured_peaks()
 
@@ -298,20 +321,21 @@ def run_ours(args, wl):
                     traffic = int(row["dram_bytes_per_launch"])
         except Exception:
             pass
-        cpu = oracle_sample(dims, eps, lseed, sseed, kappa, U=U) if world == 1 and not args.no_cpu_baseline else None
+        cpu = (oracle_sample(dims, eps, lseed, sseed, kappa, U=U, nrhs=nrhs, nsample=4096 if nrhs == 1 else 1024)
+               if world == 1 and not args.no_cpu_baseline else None)
         line = {
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if sbytes == 4 else "f64", "data": "synthetic",
-            "config": {"workload": wl, "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
+            "config": {"workload": wl, "nrhs": nrhs, "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
                        "sites": V, "l2_flush": "not needed: W (%.1f GB) >> L2 (126 MB)" % (B.ok_W_bytes(p) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "plaquette": plaq, "u0": pd["u0"]},
             "pct_of_peak": {"measured_copy": 100 * value / world / peaks["hbm_gbs"], "nominal_8000": 100 * value / world / 8000.0},
             "apply_ms": a_ms, "applies_per_s": world * 1e3 / a_ms, "sites_per_s": world * V * 1e3 / a_ms,
-            "gflops": world * V * FLOP_PER_SITE / (a_ms * 1e-3) / 1e9,
+            "gflops": world * V * FLOP_PER_SITE * nrhs / (a_ms * 1e-3) / 1e9,
             "bicgstab_solve_s": s_s, "bicgstab_iters": int(np.max(iters_l)), "bicgstab_true_resid": float(np.max(resid_l)),
             "precalc_ms": float(np.mean(pre_ms)),
-            "roofline": {"bound": "hbm", "kernel": "okd::apply_direct_kernel<float,...>", "achieved": alg / (a_ms * 1e-3) / 1e9,
+            "roofline": {"bound": "hbm", "kernel": KERNEL_NAME[(sbytes, nrhs)], "achieved": alg / (a_ms * 1e-3) / 1e9,
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": alg / (a_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                          "peak_source": peaks["_source"], "algorithmic_bytes_per_launch": alg, "traffic": traffic},
             "e2e": {"value": world * alg / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_apply": e2e_ms,
