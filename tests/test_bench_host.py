@@ -58,7 +58,7 @@ def test_traffic_table_parses():
     rows = list(csv.DictReader(open(os.path.join(ROOT, "profiles", "apply_ncu_traffic.csv"))))
     assert rows and all(set(r) >= {"workload", "kernel", "dram_bytes_per_launch"} for r in rows)
     for r in rows:
-        alg = 512000 * bench.BYTES_PER_SITE[4]
+        alg = 512000 * bench.alg_bytes_per_site(4, 1)
         if r["workload"] == "20x20x20x64-fp32":
             assert 0.95 * alg < int(r["dram_bytes_per_launch"]) < 1.2 * alg
 
