@@ -127,6 +127,11 @@ int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host);
 /* ---- diagnostics -------------------------------------------------------------------------- */
 /* Read the parameters stored in W's header back into *p (HOST). */
 int ok_W_params(const void* W, ok_params* p);
+/* Drop the library's host-side record of W (the header mirror that lets the three main calls run
+ * without a params argument and without reading the device).  Call it before freeing the buffer or
+ * reusing its memory for anything else; a later W written there by ok_precalc_W / ok_pack_W is
+ * recorded again.  Unknown pointers are ignored.  Returns OK_SUCCESS. */
+int ok_forget_W(const void* W);
 /* Number of kernels the library has launched since load (for launch accounting in benches). */
 uint64_t ok_launch_count(void);
 /* Select the apply kernel variant (0 = default).  Tuning knob; results are identical. */

@@ -47,6 +47,7 @@ EXPORTS = {
                               C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_dirac_apply_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "ok_W_params": (C.c_int, [C.c_void_p, C.POINTER(ok_params)]),
+    "ok_forget_W": (C.c_int, [C.c_void_p]),
     "ok_launch_count": (C.c_uint64, []),
     "ok_set_apply_variant": (C.c_int, [C.c_int]),
     "ok_strerror": (C.c_char_p, [C.c_int]),
@@ -174,6 +175,10 @@ def ok_W_params(W):
     return q
 
 
+def ok_forget_W(W):
+    _check(lib().ok_forget_W(_ptr(W)), "ok_forget_W")
+
+
 def ok_launch_count():
     return int(lib().ok_launch_count())
 
@@ -190,7 +195,12 @@ def alloc_bytes(nbytes, device="cuda:0"):
 
 
 def alloc_W(p, device="cuda:0"):
-    return alloc_bytes(ok_W_bytes(p), device)
+    """W buffer; the library's record of it is dropped when the tensor is freed (the caching
+    allocator hands the same address out again, ok.h: ok_forget_W)."""
+    import weakref
+    t = alloc_bytes(ok_W_bytes(p), device)
+    weakref.finalize(t, lib().ok_forget_W, t.data_ptr())
+    return t
 
 
 def alloc_vec(p, device="cuda:0"):

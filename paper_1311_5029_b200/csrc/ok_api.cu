@@ -169,6 +169,12 @@ int ok_unpack_W(const void* W, void* canon) {
   return launch_pack_W(&p, canon, const_cast<char*>(W_payload(W)), true);
 }
 
+int ok_forget_W(const void* W) {
+  std::lock_guard<std::mutex> lk(g_mu);
+  g_table.erase(W);
+  return OK_SUCCESS;
+}
+
 int ok_W_params(const void* W, ok_params* p) {
   if (!p) return OK_EINVAL;
   return lookup_W(W, p);
