@@ -8,18 +8,25 @@
 // above the 2e-5 tolerance, so each operand is split a = hi + lo with hi = trunc_tf32(a) (what the
 // tensor core sees when fed the raw fp32 word) and lo = a - hi (exact in fp32).  hi and lo are STACKED in
 // the M and N dimensions of one accumulator:  [A_hi ; A_lo] (48 x K) times [B_hi , B_lo] (K x 48)
-// gives all four products from ONE series of 41 MMAs (M = 64, N = 48, K = 8) instead of three series;
-// the epilogue adds the four quadrants.  Error: lo operands truncated again, ~2^-20 relative.
+// gives all four products from ONE series of 41 MMAs (M = 64, N = 48, K = 8); the epilogue adds the
+// four quadrants.  Error: lo operands truncated again, ~2^-21 relative.
 //
-// CTA = 128 threads, a run of consecutive sites, several CTAs per SM.  Per site, 7 pipeline stages of
-// 4 stencil terms (K = 48; the last has 3 terms + a zero pad chunk, K = 40), double-buffered in smem:
-//   fill:  all threads stream the W tile chunks (global, evict-first) and gather the neighbour
-//          spinor records (L2), split hi/lo in registers, store both into the UMMA canonical
-//          K-major no-swizzle layout (core matrix = 8 rows x 16 B; LBO = 128 B, SBO = 1536 B);
-//   mma:   one thread issues 6 (5) tcgen05.mma into the 64-lane x 48-column fp32 accumulator in TMEM
-//          and commits to the stage's mbarrier (which frees the buffer);
-//   epilogue (per site): warps 0-2 read their 16 accumulator lanes with tcgen05.ld, fold hi/lo
-//          columns, exchange through smem, combine re/im and write the output record.
+// One persistent CTA per SM, 20 specialised warps, sites dealt round-robin (site = blockIdx.x + k gridDim.x,
+// so the CTAs sweep the lattice together and the gathered spinor records stay in L2).  The K dimension of a
+// site is cut into 7 chunks of 4 stencil terms (48 k; the last chunk 36 + 4 zero k), pipelined through an
+// 8-stage ring that spans site boundaries:
+//   A operand (W)   lives in TENSOR MEMORY: 8 warps (two per TMEM lane quarter) stream the W chunk from HBM
+//                   (evict-first 16-B loads, 3 chunks of prefetch in registers), form lo = w - trunc(w) and
+//                   write hi and lo rows with tcgen05.st.16x256b (a thread's 4 registers are rows g, g+8 =
+//                   hi, lo of one W row-part).  W never touches shared memory.
+//   B operand (Psi) lives in shared memory: 6 warps gather the 4 neighbour records of the chunk from L2,
+//                   split hi/lo and store both halves in the UMMA canonical K-major no-swizzle layout
+//                   (core matrix = 8 rows x 16 B; LBO = 128 B, SBO = 1536 B).
+//   MMA             one thread issues 6 (5) tcgen05.mma (A from TMEM, B from smem) per chunk into one of two
+//                   64-lane x 48-column fp32 accumulators and commits to the stage's mbarrier.
+//   epilogue        4 warps (one per lane quarter) read the accumulator with tcgen05.ld.16x256b, fold the
+//                   hi/lo rows and columns, combine re/im and write the 1152-B output record through smem.
+//   index           1 warp computes the 27 neighbour site indices of upcoming sites into a small smem ring.
 // Layouts of W and of the spinor records: ok_internal.cuh (kLayoutMrhs).
 #include "ok_internal.cuh"
 
@@ -30,17 +37,29 @@ static bool g_moff_uploaded = false;
 
 namespace {
 
-constexpr int kStageChunks = 12;                    // k-chunks (4 k each) per stage = 4 terms
-constexpr int kSBO = kStageChunks * 128;            // 1536 B between 8-row groups
-constexpr int kLBO = 128;                           // between the two k-chunks of one MMA
-constexpr int kAStage = 6 * kSBO;                   // rows 0..47 (hi 24 + lo 24); rows 48..63 read garbage from B
-constexpr int kBStage = 6 * kSBO;                   // n 0..47
-constexpr int kStage = kAStage + kBStage;           // 18 432 B
-constexpr int kStagesPerSite = 7;
-constexpr int kSmemT = 48 * 24 * 4;                 // epilogue exchange
-constexpr int kSmemBytes = 2 * kStage + kSmemT;     // 41 472 B
-constexpr int kTmemCols = 64;
+constexpr int kStages = 8;                          // chunk ring (A slot in TMEM + B tile in smem)
+constexpr int kSBO = 12 * 128;                      // 1536 B between 8-row groups of the B tile
+constexpr int kLBO = 128;                           // between the two k-chunks (4 k each) of one MMA
+constexpr int kBStage = 6 * kSBO;                   // n = 0..47 (hi 24 + lo 24): 9216 B
+constexpr int kACols = kMrhsChunkK;                 // 48 TMEM columns per A slot
+constexpr int kDCol0 = kStages * kACols;            // 384: accumulator 0; accumulator 1 at +64
+constexpr int kTmemCols = 512;
+constexpr int kNbrRing = 4;
+constexpr int kAPrefetch = 3;                       // W chunks in flight per A warp (registers)
+
+constexpr int kWarpMma = 0, kWarpB0 = 1, kWarpA = 4, kWarpEpi = 12, kWarpB1 = 16, kWarpIdx = 19;
+constexpr int kWarps = 20, kThreads = kWarps * 32;
+
+constexpr int kSmemB = kStages * kBStage;           // 73 728
+constexpr int kSmemOut = 2 * kMrhsVecSiteFloats * 4;
+constexpr int kSmemNbr = kNbrRing * 32 * 4;
+constexpr int kSmemBytes = kSmemB + kSmemOut + kSmemNbr;
+
 constexpr uint32_t kIdesc = (1u << 4) /*D f32*/ | (2u << 7) /*A tf32*/ | (2u << 10) /*B tf32*/ | ((48u >> 3) << 17) | ((64u >> 4) << 24);
+
+struct Bars {
+  uint64_t full[kStages], empty[kStages], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
+};
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -48,24 +67,38 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {   // K-major, no
   return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)(kLBO >> 4) << 16) | ((uint64_t)(kSBO >> 4) << 32) | ((uint64_t)1 << 46);
 }
 
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t a = smem_u32(bar);
   uint32_t done = 0;
   while (!done) {
     asm volatile(
         "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
         : "=r"(done)
-        : "r"(bar), "r"(parity)
+        : "r"(a), "r"(parity)
         : "memory");
   }
 }
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-__device__ __forceinline__ float4 tf32_lo(const float4& v) {   // v - trunc_tf32(v), exact
-  float4 r;
-  r.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u);
-  r.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u);
-  r.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u);
-  r.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u);
-  return r;
+__device__ __forceinline__ float tf32_lo(float v) { return v - __uint_as_float(__float_as_uint(v) & 0xFFFFE000u); }   // exact
+__device__ __forceinline__ float4 tf32_lo(const float4& v) { return make_float4(tf32_lo(v.x), tf32_lo(v.y), tf32_lo(v.z), tf32_lo(v.w)); }
+
+// 16 lanes x 8 columns: registers (r0, r1) -> lane t/4, columns 2(t%4), 2(t%4)+1 ; (r2, r3) -> lane t/4 + 8 (measured).
+__device__ __forceinline__ void tmem_st_16x256(uint32_t taddr, float r0, float r1, float r2, float r3) {
+  asm volatile("tcgen05.st.sync.aligned.16x256b.x1.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "f"(r0), "f"(r1), "f"(r2), "f"(r3) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_16x256(uint32_t taddr, float& r0, float& r1, float& r2, float& r3) {
+  asm volatile("tcgen05.ld.sync.aligned.16x256b.x1.b32 {%0, %1, %2, %3}, [%4];" : "=f"(r0), "=f"(r1), "=f"(r2), "=f"(r3) : "r"(taddr));
 }
 
 __device__ __forceinline__ int wrapc(int x, int L) {
@@ -74,156 +107,265 @@ __device__ __forceinline__ int wrapc(int x, int L) {
   return x;
 }
 
+struct AChunk {   // one thread's share of a W chunk: one row-part, 12 k values
+  float4 v[3];
+};
+
 }  // namespace
 
-__global__ void __launch_bounds__(128, 5)
-apply_mrhs_kernel(const float4* __restrict__ W, const float4* __restrict__ psi, float4* __restrict__ out, Geom g,
-                  int sites_per_cta) {
+__global__ void __launch_bounds__(kThreads, 1)
+apply_mrhs_kernel(const float* __restrict__ W, const float4* __restrict__ psi, float4* __restrict__ out, Geom g) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ uint32_t s_tmem;
-  __shared__ __align__(8) uint64_t s_bar[3];   // [0],[1]: stage buffer free ; [2]: site accumulator complete
+  __shared__ __align__(8) Bars bars;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  float* sT = reinterpret_cast<float*>(smem + 2 * kStage);
+  uint8_t* sB = smem;
+  float* sOut = reinterpret_cast<float*>(smem + kSmemB);
+  int* sNbr = reinterpret_cast<int*>(smem + kSmemB + kSmemOut);
 
   if (tid == 0) {
-    for (int i = 0; i < 3; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s_bar[i])));
+    for (int i = 0; i < kStages; ++i) { mbar_init(&bars.full[i], 7); mbar_init(&bars.empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&bars.dfull[i], 1); mbar_init(&bars.dempty[i], 4); }
+    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], 6); }
     asm volatile("fence.mbarrier_init.release.cluster;");
   }
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  asm volatile("tcgen05.fence::before_thread_sync;");
+  tc_fence_before();
   __syncthreads();
-  asm volatile("tcgen05.fence::after_thread_sync;");
+  tc_fence_after();
   const uint32_t tmem = s_tmem;
-  const uint32_t bar_free[2] = {smem_u32(&s_bar[0]), smem_u32(&s_bar[1])};
-  const uint32_t bar_done = smem_u32(&s_bar[2]);
 
-  const int site0 = blockIdx.x * sites_per_cta;
-  const int nsite = min(sites_per_cta, g.V - site0);
-  uint32_t it = 0;
-  for (int ls = 0; ls < nsite; ++ls) {
-    const int n = site0 + ls;
-    const int x = n % g.L[0];
-    int q = n / g.L[0];
-    const int y = q % g.L[1];
-    q /= g.L[1];
-    const int z = q % g.L[2];
-    const int t = q / g.L[2];
-    const float4* Wsite = W + (size_t)n * (kMrhsWSiteFloats / 4);
+  const int nsite = ((int)blockIdx.x < g.V) ? (g.V - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  const int total = nsite * kMrhsChunks;   // chunk iterations of this CTA
 
-    for (int s = 0; s < kStagesPerSite; ++s, ++it) {
-      const uint32_t buf = it & 1u;
-      mbar_wait(bar_free[buf], ((it >> 1) & 1u) ^ 1u);   // MMAs that read this buffer two stages ago are done
-      uint8_t* sA = smem + buf * kStage;
-      uint8_t* sB = sA + kAStage;
-      const int nch = (s < 6) ? kStageChunks : 10;       // last stage: 9 chunks + the zero pad chunk
-      // ---- A: 3 row groups x nch chunks x 8 rows, 16-B units; global order == smem order
-      for (int u = tid; u < 3 * nch * 8; u += 128) {
-        const int rg = u / (nch * 8), w = u - rg * (nch * 8);
-        const float4 v = __ldcs(Wsite + (rg * kMrhsChunks + s * kStageChunks) * 8 + w);
-        *reinterpret_cast<float4*>(sA + rg * kSBO + w * 16) = v;
-        *reinterpret_cast<float4*>(sA + (3 + rg) * kSBO + w * 16) = tf32_lo(v);
+  if (warp == kWarpMma) {
+    // ------------------------------------------------------------------ MMA issuer
+    if (lane == 0) {
+      for (int k = 0, it = 0; k < nsite; ++k) {
+        const int d = k & 1;
+        mbar_wait(&bars.dempty[d], (((uint32_t)k >> 1) & 1u) ^ 1u);   // epilogue drained this accumulator
+        tc_fence_after();
+        const uint32_t dcol = tmem + kDCol0 + 64 * d;
+        for (int c = 0; c < kMrhsChunks; ++c, ++it) {
+          const int st = it & (kStages - 1);
+          mbar_wait(&bars.full[st], ((uint32_t)it / kStages) & 1u);
+          tc_fence_after();
+          const uint32_t a0 = tmem + st * kACols, b0 = smem_u32(sB + st * kBStage);
+          const int nmma = (c < 6) ? 6 : 5;
+          for (int j = 0; j < nmma; ++j) {
+            const uint64_t db = umma_desc(b0 + j * 256);
+            const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u, zero = 0u;
+            asm volatile(
+                "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n\t}\n" ::"r"(dcol),
+                "r"(a0 + 8 * j), "l"(db), "r"(kIdesc), "r"(acc), "r"(zero)
+                : "memory");
+          }
+          umma_commit(&bars.empty[st]);                 // frees the A slot and the B tile
+          if (c == kMrhsChunks - 1) umma_commit(&bars.dfull[d]);
+        }
       }
-      // ---- B: 4 (3) neighbour records of 72 units: [n group 3][chunk 3][row 8]
-      const int nterm = (s < 6) ? 4 : 3;
-      for (int u = tid; u < nterm * 72; u += 128) {
-        const int tl = u / 72, r = u - tl * 72;
-        const int ng = r / 24, w = r - ng * 24;
-        const int o = 4 * s + tl;
-        const int xx = wrapc(x + c_moff[o][0], g.L[0]);
-        const int yy = wrapc(y + c_moff[o][1], g.L[1]);
-        const int zz = wrapc(z + c_moff[o][2], g.L[2]);
-        const int tt = wrapc(t + c_moff[o][3], g.L[3]);
-        const int nn = xx + g.L[0] * (yy + g.L[1] * (zz + g.L[2] * tt));
-        const float4 v = __ldg(psi + (size_t)nn * (kMrhsVecSiteFloats / 4) + r);
-        uint8_t* dst = sB + ng * kSBO + (tl * 24 + w) * 16;
-        *reinterpret_cast<float4*>(dst) = v;
-        *reinterpret_cast<float4*>(dst + 3 * kSBO) = tf32_lo(v);
+    }
+    __syncwarp();
+  } else if (warp >= kWarpA && warp < kWarpA + 8) {
+    // ------------------------------------------------------------------ A producers: W (HBM) -> TMEM
+    const int q = warp & 3, half = (warp - kWarpA) >> 2;
+    const int gq = lane >> 2, cp = lane & 3;
+    const bool active = gq < 6;                         // 6 row-parts per quarter; lanes 6,7 (+8) are pad rows
+    const int rp = q * 6 + gq;
+    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
+
+    auto load = [&](int it, AChunk& a) {
+      const int k = it / kMrhsChunks, c = it - k * kMrhsChunks;
+      const size_t n = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+      const float* tile = W + n * kMrhsWSiteFloats;
+      if (!active) { a.v[0] = a.v[1] = a.v[2] = make_float4(0.f, 0.f, 0.f, 0.f); return; }
+      if (c < 6) {
+        const float4* p = reinterpret_cast<const float4*>(tile + c * kMrhsChunkFloats + rp * kMrhsChunkK) + cp;
+        a.v[0] = __ldcs(p); a.v[1] = __ldcs(p + 4); a.v[2] = __ldcs(p + 8);
+      } else {
+        const float* row = tile + 6 * kMrhsChunkFloats + rp * kMrhsLastK;
+        const float4* p = reinterpret_cast<const float4*>(row) + cp;
+        a.v[0] = __ldcs(p); a.v[1] = __ldcs(p + 4);
+        const float2 t2 = __ldcs(reinterpret_cast<const float2*>(row + 32) + cp);
+        a.v[2] = make_float4(t2.x, t2.y, 0.f, 0.f);
       }
-      if (s == 6 && tid < 48) {   // zero pad chunk (stage chunk 9) of the 6 n groups
-        const int ng6 = tid >> 3, row = tid & 7;
-        *reinterpret_cast<float4*>(sB + ng6 * kSBO + (9 * 8 + row) * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+    };
+    auto store = [&](int it, const AChunk& a) {
+      const int st = it & (kStages - 1);
+      mbar_wait(&bars.empty[st], (((uint32_t)it / kStages) & 1u) ^ 1u);
+      tc_fence_after();
+      const uint32_t t0 = tmem + lane_base + st * kACols;
+#pragma unroll
+      for (int J = 0; J < 3; ++J) {
+        const float4 hi = a.v[J], lo = tf32_lo(hi);
+        tmem_st_16x256(t0 + 16 * J, hi.x, hi.y, lo.x, lo.y);
+        tmem_st_16x256(t0 + 16 * J + 8, hi.z, hi.w, lo.z, lo.w);   // last chunk: columns 40..47 are never read
+      }
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.full[st]);
+    };
+
+    AChunk ring[kAPrefetch];
+#pragma unroll
+    for (int i = 0; i < kAPrefetch; ++i)
+      if (half + 2 * i < total) load(half + 2 * i, ring[i]);
+    for (int it = half; it < total; it += 2 * kAPrefetch) {
+#pragma unroll
+      for (int i = 0; i < kAPrefetch; ++i) {
+        const int cur = it + 2 * i;
+        if (cur < total) {
+          store(cur, ring[i]);
+          if (cur + 2 * kAPrefetch < total) load(cur + 2 * kAPrefetch, ring[i]);
+        }
+      }
+    }
+  } else if ((warp >= kWarpB0 && warp < kWarpB0 + 3) || (warp >= kWarpB1 && warp < kWarpB1 + 3)) {
+    // ------------------------------------------------------------------ B producers: Psi (L2) -> smem
+    const int grp = warp >= kWarpB1 ? 1 : 0;
+    const int v = (warp - (grp ? kWarpB1 : kWarpB0)) * 32 + lane;   // 0..95; 72 units per record
+    const bool active = v < 72;
+    const int ng = v / 24, w = v - ng * 24;
+    const uint32_t dst0 = (uint32_t)(ng * kSBO + w * 16);
+
+    auto load = [&](int it, float4 (&r)[4]) {
+      const int k = it / kMrhsChunks, c = it - k * kMrhsChunks;
+      const int slot = k & (kNbrRing - 1);
+      if (c < 2) mbar_wait(&bars.nfull[slot], ((uint32_t)k / kNbrRing) & 1u);   // first chunk of site k for this group
+#pragma unroll
+      for (int rec = 0; rec < 4; ++rec) {
+        const int term = 4 * c + rec;
+        r[rec] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (active && term < kTerms) {
+          const int nn = sNbr[slot * 32 + term];
+          r[rec] = __ldg(psi + (size_t)nn * (kMrhsVecSiteFloats / 4) + v);
+        }
+      }
+      if (c >= 5) {   // last chunk of site k for this group: the index slot may be refilled
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars.nempty[slot]);
+      }
+    };
+    auto store = [&](int it, const float4 (&r)[4]) {
+      const int st = it & (kStages - 1);
+      mbar_wait(&bars.empty[st], (((uint32_t)it / kStages) & 1u) ^ 1u);
+      if (active) {
+        uint8_t* base = sB + st * kBStage + dst0;
+#pragma unroll
+        for (int rec = 0; rec < 4; ++rec) {
+          *reinterpret_cast<float4*>(base + rec * 384) = r[rec];
+          *reinterpret_cast<float4*>(base + rec * 384 + 3 * kSBO) = tf32_lo(r[rec]);
+        }
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core
-      __syncthreads();
-      if (tid == 0) {
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t a0 = smem_u32(sA), b0 = smem_u32(sB);
-        const int nmma = nch >> 1;
-        for (int j = 0; j < nmma; ++j) {
-          const uint64_t da = umma_desc(a0 + j * 256), db = umma_desc(b0 + j * 256);
-          const uint32_t acc = (s > 0 || j > 0) ? 1u : 0u, zero = 0u;
-          asm volatile(
-              "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-              "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}\n" ::"r"(tmem),
-              "l"(da), "l"(db), "r"(kIdesc), "r"(acc), "r"(zero)
-              : "memory");
-        }
-        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar_free[buf]) : "memory");
-        if (s == kStagesPerSite - 1)
-          asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar_done) : "memory");
-      }
-    }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.full[st]);
+    };
 
-    // ---- epilogue of this site
-    mbar_wait(bar_done, (uint32_t)ls & 1u);
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    if (warp < 3) {   // accumulator row i lives in lane (i % 16) + 32 (i / 16): warp w holds rows 16w .. 16w+15
-      uint32_t d[48];
-      const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16);
-#pragma unroll
-      for (int c = 0; c < 48; c += 16)
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-            : "=r"(d[c + 0]), "=r"(d[c + 1]), "=r"(d[c + 2]), "=r"(d[c + 3]), "=r"(d[c + 4]), "=r"(d[c + 5]), "=r"(d[c + 6]),
-              "=r"(d[c + 7]), "=r"(d[c + 8]), "=r"(d[c + 9]), "=r"(d[c + 10]), "=r"(d[c + 11]), "=r"(d[c + 12]), "=r"(d[c + 13]),
-              "=r"(d[c + 14]), "=r"(d[c + 15])
-            : "r"(taddr + c));
-      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      if (lane < 16) {
-        float* dstT = sT + (warp * 16 + lane) * 24;
-#pragma unroll
-        for (int c = 0; c < 24; ++c) dstT[c] = __uint_as_float(d[c]) + __uint_as_float(d[24 + c]);   // B_hi + B_lo columns
+    float4 ra[4], rb[4];
+    if (grp < total) load(grp, ra);
+    for (int it = grp; it < total; it += 4) {
+      if (it + 2 < total) load(it + 2, rb);
+      store(it, ra);
+      if (it + 2 < total) {
+        if (it + 4 < total) load(it + 4, ra);
+        store(it + 2, rb);
       }
     }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (tid < 72) {   // one 16-B output unit: (n group, chunk c4, rhs-in-group p, part), components 4 c4 .. 4 c4 + 3
-      const int row8 = tid & 7, c4 = (tid >> 3) % 3, ng = tid / 24;
-      const int p = row8 >> 1, part = row8 & 1;
-      const int col_same = 8 * ng + 2 * p + part, col_other = 8 * ng + 2 * p + (1 - part);
-      float o[4];
+  } else if (warp >= kWarpEpi && warp < kWarpEpi + 4) {
+    // ------------------------------------------------------------------ epilogue: TMEM -> out
+    const int q = warp & 3;
+    const int gq = lane >> 2, cp = lane & 3;
+    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
+    const int et = tid - kWarpEpi * 32;   // 0..127
+    for (int k = 0; k < nsite; ++k) {
+      const int d = k & 1;
+      mbar_wait(&bars.dfull[d], ((uint32_t)k >> 1) & 1u);
+      tc_fence_after();
+      const uint32_t t0 = tmem + lane_base + kDCol0 + 64 * d;
+      float r[6][4];
 #pragma unroll
-      for (int ci = 0; ci < 4; ++ci) {
-        const int r = 4 * c4 + ci;
-        // S[m][n] = T[m][n] + T[24 + m][n]  (A_hi + A_lo rows); rows m < 12: W_r, m >= 12: W_i
-        const float s_r_same = sT[r * 24 + col_same] + sT[(24 + r) * 24 + col_same];
-        const float s_i_other = sT[(12 + r) * 24 + col_other] + sT[(36 + r) * 24 + col_other];
-        // re: W_r Psi_r - W_i Psi_i ; im: W_r Psi_i + W_i Psi_r
-        o[ci] = part == 0 ? s_r_same - s_i_other : s_r_same + s_i_other;
+      for (int j = 0; j < 6; ++j) tmem_ld_16x256(t0 + 8 * j, r[j][0], r[j][1], r[j][2], r[j][3]);
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.dempty[d]);
+      // rows g (hi) + g+8 (lo), columns c (B hi) + c+24 (B lo):  S[j][e], n = 8 j + 2 cp + e = 2 rhs + part_psi
+      float S[3][2], O[3][2];
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) S[j][e] = (r[j][e] + r[j][2 + e]) + (r[j + 3][e] + r[j + 3][2 + e]);
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) O[j][e] = __shfl_xor_sync(0xffffffffu, S[j][e], 4);   // partner row-part (Re <-> Im of W)
+      // row-part gq = 2 cr + part_w.  part_w = 0 lanes write Out_r = Sr[0] - Si[1]; part_w = 1 lanes write Out_i = Sr[1] + Si[0]
+      if (gq < 6) {
+        const int part = gq & 1, comp = 3 * q + (gq >> 1);
+        float* so = sOut + d * kMrhsVecSiteFloats;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          const float val = part == 0 ? S[j][0] - O[j][1] : O[j][1] + S[j][0];
+          // out record: n = 2 rhs + part = 8 j + 2 cp + part
+          so[(j * 3 + (comp >> 2)) * 32 + (2 * cp + part) * 4 + (comp & 3)] = val;
+        }
       }
-      out[(size_t)n * (kMrhsVecSiteFloats / 4) + tid] = make_float4(o[0], o[1], o[2], o[3]);
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      if (et < kMrhsVecSiteFloats / 4) {
+        const size_t n = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+        out[n * (kMrhsVecSiteFloats / 4) + et] = reinterpret_cast<const float4*>(sOut + d * kMrhsVecSiteFloats)[et];
+      }
+    }
+  } else if (warp == kWarpIdx) {
+    // ------------------------------------------------------------------ neighbour indices
+    for (int k = 0; k < nsite; ++k) {
+      const int slot = k & (kNbrRing - 1);
+      mbar_wait(&bars.nempty[slot], (((uint32_t)k / kNbrRing) & 1u) ^ 1u);
+      const int n = (int)blockIdx.x + k * (int)gridDim.x;
+      const int x = n % g.L[0];
+      int qq = n / g.L[0];
+      const int y = qq % g.L[1];
+      qq /= g.L[1];
+      const int z = qq % g.L[2];
+      const int t = qq / g.L[2];
+      if (lane < kTerms) {
+        const int xx = wrapc(x + c_moff[lane][0], g.L[0]);
+        const int yy = wrapc(y + c_moff[lane][1], g.L[1]);
+        const int zz = wrapc(z + c_moff[lane][2], g.L[2]);
+        const int tt = wrapc(t + c_moff[lane][3], g.L[3]);
+        sNbr[slot * 32 + lane] = xx + g.L[0] * (yy + g.L[1] * (zz + g.L[2] * tt));
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.nfull[slot]);
     }
   }
 
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  tc_fence_before();
   __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols));
 }
 
 int launch_apply_mrhs(const ok_params* p, const void* W, const void* psi, void* out) {
   if (p->nrhs != 12 || p->precision != OK_FP32) return OK_EINVAL;
+  static int sm_count = 0;
   if (!g_moff_uploaded) {
     OK_CUDA(cudaMemcpyToSymbol(c_moff, kOffsets, sizeof(kOffsets)));
+    int dev = 0;
+    OK_CUDA(cudaGetDevice(&dev));
+    OK_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+    OK_CUDA(cudaFuncSetAttribute(apply_mrhs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     g_moff_uploaded = true;
   }
   Geom g = make_geom(p);
-  const int spc = 16;
-  const int grid = (g.V + spc - 1) / spc;
-  apply_mrhs_kernel<<<grid, 128, kSmemBytes, ctx().stream>>>(static_cast<const float4*>(W), static_cast<const float4*>(psi),
-                                                           static_cast<float4*>(out), g, spc);
+  const int grid = g.V < sm_count ? g.V : sm_count;   // one persistent CTA per SM (it owns all 512 TMEM columns)
+  apply_mrhs_kernel<<<grid, kThreads, kSmemBytes, ctx().stream>>>(static_cast<const float*>(W), static_cast<const float4*>(psi),
+                                                                 static_cast<float4*>(out), g);
   OK_LAUNCHED("apply_mrhs_kernel");
   return OK_SUCCESS;
 }

@@ -16,18 +16,34 @@ constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
 constexpr uint32_t kLayoutMrhs = 2;        // nrhs = 12: per-site tcgen05 A-operand tiles (ok_apply_mrhs.cu)
 
 // ---- nrhs = 12 (tensor-core) layouts, fp32 only -------------------------------------------------
-// W: per site the real-split A operand [W_r ; W_i] (24 x 324, padded to K = 328) in the UMMA K-major
-// no-swizzle canonical order: [row group m/8 = 0..2][k chunk k/4 = 0..81][m%8][k%4], m = 12*part + row,
-// k = 12*term + col; chunk 81 is a zero pad.  31 488 B per site.
-constexpr int kMrhsChunks = 82;
-constexpr int kMrhsWSiteFloats = 3 * kMrhsChunks * 32;
+// W: per site the real-split A operand [W_r ; W_i] (24 row-parts x K = 324), cut along K into 7 chunks of
+// 4 stencil terms (48 k; the last chunk holds 3 terms + 4 zero pad k = 40).  Inside a chunk the 24
+// row-parts are ordered for the four TMEM lane quarters of ok_apply_mrhs.cu: rp = 6*(row/3) + 2*(row%3)
+// + part (part 0 = Re, 1 = Im), each a contiguous run of 48 (40) floats.  Inside a run the k order is
+// permuted so that the 16 B a thread loads are exactly the 4 values it stores with tcgen05.st.16x256b:
+// float m = 16 J + 4 cp + 2 h + e  <->  TMEM column (= k in chunk) c = 16 J + 8 h + 2 cp + e
+// (columns 32..39 of the last chunk are stored in natural order).  31 488 B per site.
+constexpr int kMrhsChunkTerms = 4;
+constexpr int kMrhsChunks = 7;
+constexpr int kMrhsChunkK = 48;
+constexpr int kMrhsLastK = 40;
+constexpr int kMrhsChunkFloats = 24 * kMrhsChunkK;                          // 1152
+constexpr int kMrhsWSiteFloats = 6 * kMrhsChunkFloats + 24 * kMrhsLastK;    // 7872
+__host__ __device__ inline int mrhs_W_perm(int c) {   // column in chunk -> float position in the run
+  return (c & ~15) | (((c >> 1) & 3) << 2) | (((c >> 3) & 1) << 1) | (c & 1);
+}
+__host__ __device__ inline int mrhs_W_rowpart(int row, int part) { return 6 * (row / 3) + 2 * (row % 3) + part; }
+__host__ __device__ inline int mrhs_W_index(int term, int row, int col, int part) {
+  const int chunk = term >> 2, c = (term & 3) * 12 + col, rp = mrhs_W_rowpart(row, part);
+  if (chunk < 6) return chunk * kMrhsChunkFloats + rp * kMrhsChunkK + mrhs_W_perm(c);
+  return 6 * kMrhsChunkFloats + rp * kMrhsLastK + (c < 32 ? mrhs_W_perm(c) : c);
+}
+__host__ __device__ inline int mrhs_W_pad_index(int q) {   // q = 0..95: the zero pad floats (k = 36..39 of the last chunk)
+  return 6 * kMrhsChunkFloats + (q >> 2) * kMrhsLastK + 36 + (q & 3);
+}
 // spinor: per site the B operand [Psi_r , Psi_i] (24 x 12) as 9 core matrices:
 // [n group n/8 = 0..2][k chunk c/4 = 0..2][n%8][c%4], n = 2*rhs + part, c = component.  1152 B per site.
 constexpr int kMrhsVecSiteFloats = 288;
-__host__ __device__ inline int mrhs_W_index(int term, int row, int col, int part) {
-  const int m = 12 * part + row, k = 12 * term + col;
-  return ((m >> 3) * kMrhsChunks + (k >> 2)) * 32 + (m & 7) * 4 + (k & 3);
-}
 __host__ __device__ inline int mrhs_vec_index(int comp, int rhs, int part) {
   const int n = 2 * rhs + part;
   return ((n >> 3) * 3 + (comp >> 2)) * 32 + (n & 7) * 4 + (comp & 3);

@@ -43,7 +43,7 @@ __global__ void pack_spinor_mrhs_kernel(const float2* __restrict__ canon, float*
 }
 
 // nrhs = 12 W: canonical [n][27][12][12][re,im] <-> per-site A-operand tiles (mrhs_W_index); the
-// zero pad chunk (k = 324..327) is written when packing.
+// zero pad (k = 324..327 of every row-part) is written when packing.
 __global__ void pack_W_mrhs_kernel(const float2* __restrict__ canon, float* __restrict__ packed, int V, bool unpack) {
   constexpr int kPer = kTerms * 144 + 96;
   long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -51,9 +51,8 @@ __global__ void pack_W_mrhs_kernel(const float2* __restrict__ canon, float* __re
   const int e = (int)(u % kPer);
   const long long n = u / kPer;
   float* tile = packed + n * kMrhsWSiteFloats;
-  if (e >= kTerms * 144) {   // pad chunk: 3 row groups x 32 floats
-    const int q = e - kTerms * 144;
-    if (!unpack) tile[((q >> 5) * kMrhsChunks + (kMrhsChunks - 1)) * 32 + (q & 31)] = 0.f;
+  if (e >= kTerms * 144) {   // the 96 zero pad floats of the last chunk
+    if (!unpack) tile[mrhs_W_pad_index(e - kTerms * 144)] = 0.f;
     return;
   }
   const int col = e % 12, row = (e / 12) % 12, term = e / 144;

@@ -358,18 +358,15 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
     }
     unit_t* dst = Wt + (size_t)r * NC * kBlock;
     if constexpr (sizeof(real) == 4) {
-      if (a.mrhs) {   // A-operand tile of ok_apply_mrhs.cu: rows (part, r), k = 12 term + col
+      if (a.mrhs) {   // A-operand tile of ok_apply_mrhs.cu (ok_internal.cuh: mrhs_W_index)
         float* tile = reinterpret_cast<float*>(W) + (size_t)n * kMrhsWSiteFloats;
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {
-          *reinterpret_cast<float4*>(tile + mrhs_W_index(term, r, 4 * q, 0)) =
-              make_float4((float)row[4 * q].x, (float)row[4 * q + 1].x, (float)row[4 * q + 2].x, (float)row[4 * q + 3].x);
-          *reinterpret_cast<float4*>(tile + mrhs_W_index(term, r, 4 * q, 1)) =
-              make_float4((float)row[4 * q].y, (float)row[4 * q + 1].y, (float)row[4 * q + 2].y, (float)row[4 * q + 3].y);
+        for (int col = 0; col < 12; ++col) {
+          tile[mrhs_W_index(term, r, col, 0)] = (float)row[col].x;
+          tile[mrhs_W_index(term, r, col, 1)] = (float)row[col].y;
         }
-        if (term == 0 && r < 3)   // zero pad chunk k = 324..327 of row group r
-          for (int q = 0; q < 8; ++q)
-            *reinterpret_cast<float4*>(tile + (r * kMrhsChunks + kMrhsChunks - 1) * 32 + 4 * q) = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (term == 0)   // zero pad k = 324..327 of the two row-parts of row r
+          for (int q = 0; q < 8; ++q) tile[mrhs_W_pad_index(4 * mrhs_W_rowpart(r, q >> 2) + (q & 3))] = 0.f;
         continue;
       }
 #pragma unroll
