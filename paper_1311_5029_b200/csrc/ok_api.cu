@@ -112,7 +112,7 @@ size_t ok_vec_bytes(const ok_params* p) {
 size_t ok_W_bytes(const ok_params* p) {
   if (!valid_params(p)) return 0;
   Geom g = make_geom(p);
-  if (p->nrhs == 12) return OK_W_HEADER_BYTES + (size_t)g.V * kMrhsWSiteFloats * sizeof(float);
+  if (p->nrhs == 12) return OK_W_HEADER_BYTES + (size_t)g.V * kMrhsWSiteBytes;
   return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * kTerms * 144 * 2 * real_bytes(p);
 }
 

@@ -1,64 +1,62 @@
 // 12-right-hand-side Oktay-Kronfeld Dirac apply on the 5th-generation tensor cores:
 //   Out(x)[12 x 12] = sum_{term} W_term(x)[12 x 12] Psi(x + offset_term)[12 x 12]        PAPER.md:53-55, Eq. (2.2)
-// i.e. per site a complex 12 x 324 by 324 x 12 contraction, a different W at every site.
+// i.e. per site a complex 12 x 324 by 324 x 12 contraction, with a different W at every site.
 //
-// Real split: A = [W_r ; W_i] (24 x 324), B = [Psi_r , Psi_i] (324 x 24)  ->  P = A B (24 x 24),
-//   Out_r = P_rr - P_ii,  Out_i = P_ri + P_ir   (epilogue).
-// Precision: tcgen05 kind::tf32 truncates fp32 operands to 10 mantissa bits (measured on B200), far
-// above the 2e-5 tolerance, so each operand is split a = hi + lo with hi = trunc_tf32(a) (what the
-// tensor core sees when fed the raw fp32 word) and lo = a - hi (exact in fp32).  hi and lo are STACKED in
-// the M and N dimensions of one accumulator:  [A_hi ; A_lo] (48 x K) times [B_hi , B_lo] (K x 48)
-// gives all four products from ONE series of 41 MMAs (M = 64, N = 48, K = 8); the epilogue adds the
-// four quadrants.  Error: lo operands truncated again, ~2^-21 relative.
+// Real split, spinor on the M side:  D[n][w] = sum_k A[n][k] B[w][k],
+//   A = Psi^T (n = 2 rhs + part, 24 rows),  B = [W_r ; W_i] (w = (row, part), 24 rows),  K = 324 (+12 pad),
+//   Out_r = D(psi_r, W_r) - D(psi_i, W_i),  Out_i = D(psi_i, W_r) + D(psi_r, W_i)             (epilogue).
+// Precision: every fp32 operand is carried as two fp16 pieces x = hi + lo / 2048 (22 significant bits; the
+// spinor is first scaled per right-hand side by a power of two so that |x| < 2^15).  hi and lo are STACKED
+// as rows on both sides, A = [Psi_hi ; Psi_lo] (48 rows of M = 128), B = [W_hi ; W_lo] (N = 48), so one series
+// of 21 tcgen05.mma.kind::f16 (K = 16) per site yields all four products; the epilogue folds them with the
+// weights 1, 2^-11, 2^-11, 2^-22 in fp32.  W is stored pre-split in HBM (4 bytes per real, like fp32), so it
+// goes HBM -> shared memory -> tensor core with no thread touching it.
 //
-// One persistent CTA per SM, 20 specialised warps, sites dealt round-robin (site = blockIdx.x + k gridDim.x,
-// so the CTAs sweep the lattice together and the gathered spinor records stay in L2).  The K dimension of a
-// site is cut into 7 chunks of 4 stencil terms (48 k; the last chunk 36 + 4 zero k), pipelined through an
-// 8-stage ring that spans site boundaries:
-//   A operand (W)   lives in TENSOR MEMORY: 8 warps (two per TMEM lane quarter) stream the W chunk from HBM
-//                   (evict-first 16-B loads, 3 chunks of prefetch in registers), form lo = w - trunc(w) and
-//                   write hi and lo rows with tcgen05.st.16x256b (a thread's 4 registers are rows g, g+8 =
-//                   hi, lo of one W row-part).  W never touches shared memory.
-//   B operand (Psi) lives in shared memory: 6 warps gather the 4 neighbour records of the chunk from L2,
-//                   split hi/lo and store both halves in the UMMA canonical K-major no-swizzle layout
-//                   (core matrix = 8 rows x 16 B; LBO = 128 B, SBO = 1536 B).
-//   MMA             one thread issues 6 (5) tcgen05.mma (A from TMEM, B from smem) per chunk into one of two
-//                   64-lane x 48-column fp32 accumulators and commits to the stage's mbarrier.
-//   epilogue        4 warps (one per lane quarter) read the accumulator with tcgen05.ld.16x256b, fold the
-//                   hi/lo rows and columns, combine re/im and write the 1152-B output record through smem.
-//   index           1 warp computes the 27 neighbour site indices of upcoming sites into a small smem ring.
-// Layouts of W and of the spinor records: ok_internal.cuh (kLayoutMrhs).
+// One persistent CTA per SM, 16 specialised warps; sites are dealt in runs of consecutive x (L1 reuse of the
+// gathered spinor records), runs round-robin over the CTAs (so all CTAs sweep the lattice together and the
+// records stay in L2).  Per site 7 K-stages of 4 stencil terms (48 k = 24 TMEM columns):
+//   W loader   1 thread: one 31 488-B bulk copy (cp.async.bulk, L2 evict-first) per site into a 4-slot smem ring.
+//   A producers 9 warps (3 per TMEM lane quarter, quarter q = rows n = 8q..8q+7): gather the 4 neighbour records
+//              of a stage (three 16-B loads per thread, L1/L2), scale, split into fp16 hi/lo and write rows g
+//              (hi) and g + 8 (lo) with tcgen05.st.16x256b into a 16-slot ring of 24 TMEM columns.
+//   MMA        1 thread: 3 tcgen05.mma (A from tensor memory, B from smem) per stage into one of two
+//              128-lane x 48-column fp32 accumulators; tcgen05.commit frees the stage / the W slot.
+//   epilogue   3 warps (one per lane quarter): tcgen05.ld.16x256b, fold pieces, combine Re/Im, coalesced stores.
+//   index      1 warp: the 27 neighbour site indices of upcoming sites into a small smem ring.
+// A first small kernel finds max |psi| per right-hand side (the power-of-two scales).
+// Layouts of W and of the spinor records: ok_internal.cuh.
 #include "ok_internal.cuh"
 
 namespace okd {
 
 __constant__ int8_t c_moff[kTerms][4];
-static bool g_moff_uploaded = false;
+__device__ unsigned g_colmax[12];   // bit patterns of max |psi| per right-hand side (atomicMax on non-negative floats)
+static bool g_mrhs_ready = false;
 
 namespace {
 
-constexpr int kStages = 8;                          // chunk ring (A slot in TMEM + B tile in smem)
-constexpr int kSBO = 12 * 128;                      // 1536 B between 8-row groups of the B tile
-constexpr int kLBO = 128;                           // between the two k-chunks (4 k each) of one MMA
-constexpr int kBStage = 6 * kSBO;                   // n = 0..47 (hi 24 + lo 24): 9216 B
-constexpr int kACols = kMrhsChunkK;                 // 48 TMEM columns per A slot
-constexpr int kDCol0 = kStages * kACols;            // 384: accumulator 0; accumulator 1 at +64
+constexpr int kG = 3;                               // producer warps per lane quarter
+constexpr int kARing = 16;                          // A ring slots
+constexpr int kACols = 24;                          // TMEM columns per slot (48 fp16 k)
+constexpr int kWSlots = 4;                          // W ring (sites)
+constexpr int kWSlotBytes = kMrhsStages * kMrhsStageHalves * 2;   // 32 256 (the last 768 B stay zero)
+constexpr int kDCol0 = kARing * kACols;             // 384: accumulator 0; accumulator 1 at +64
 constexpr int kTmemCols = 512;
-constexpr int kNbrRing = 4;
-constexpr int kAPrefetch = 3;                       // W chunks in flight per A warp (registers)
+constexpr int kNbrRing = 8;
+constexpr int kSBO = 128, kLBO = 768;
 
-constexpr int kWarpMma = 0, kWarpB0 = 1, kWarpA = 4, kWarpEpi = 12, kWarpB1 = 16, kWarpIdx = 19;
-constexpr int kWarps = 20, kThreads = kWarps * 32;
+constexpr int kWarpMma = 3, kWarpTma = 7, kWarpIdx = 11, kWarpEpi = 12;
+constexpr int kWarps = 16, kThreads = kWarps * 32;
 
-constexpr int kSmemB = kStages * kBStage;           // 73 728
-constexpr int kSmemOut = 2 * kMrhsVecSiteFloats * 4;
+constexpr int kSmemW = kWSlots * kWSlotBytes;       // 129 024
 constexpr int kSmemNbr = kNbrRing * 32 * 4;
-constexpr int kSmemBytes = kSmemB + kSmemOut + kSmemNbr;
+constexpr int kSmemBytes = kSmemW + kSmemNbr;
 
-constexpr uint32_t kIdesc = (1u << 4) /*D f32*/ | (2u << 7) /*A tf32*/ | (2u << 10) /*B tf32*/ | ((48u >> 3) << 17) | ((64u >> 4) << 24);
+// D f32, A f16, B f16, both K-major, N = 48, M = 128
+constexpr uint32_t kIdesc = (1u << 4) | (0u << 7) | (0u << 10) | ((48u >> 3) << 17) | ((128u >> 4) << 24);
 
 struct Bars {
-  uint64_t full[kStages], empty[kStages], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
+  uint64_t afull[kARing], aempty[kARing], wfull[kWSlots], wempty[kWSlots], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -72,6 +70,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   const uint32_t a = smem_u32(bar);
@@ -90,45 +91,79 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-__device__ __forceinline__ float tf32_lo(float v) { return v - __uint_as_float(__float_as_uint(v) & 0xFFFFE000u); }   // exact
-__device__ __forceinline__ float4 tf32_lo(const float4& v) { return make_float4(tf32_lo(v.x), tf32_lo(v.y), tf32_lo(v.z), tf32_lo(v.w)); }
-
-// 16 lanes x 8 columns: registers (r0, r1) -> lane t/4, columns 2(t%4), 2(t%4)+1 ; (r2, r3) -> lane t/4 + 8 (measured).
-__device__ __forceinline__ void tmem_st_16x256(uint32_t taddr, float r0, float r1, float r2, float r3) {
-  asm volatile("tcgen05.st.sync.aligned.16x256b.x1.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "f"(r0), "f"(r1), "f"(r2), "f"(r3) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_16x256(uint32_t taddr, float& r0, float& r1, float& r2, float& r3) {
-  asm volatile("tcgen05.ld.sync.aligned.16x256b.x1.b32 {%0, %1, %2, %3}, [%4];" : "=f"(r0), "=f"(r1), "=f"(r2), "=f"(r3) : "r"(taddr));
-}
-
 __device__ __forceinline__ int wrapc(int x, int L) {
   x += (x < 0) ? L : 0;
   x -= (x >= L) ? L : 0;
   return x;
 }
 
-struct AChunk {   // one thread's share of a W chunk: one row-part, 12 k values
-  float4 v[3];
+__device__ __forceinline__ uint32_t pack_h2(float lo_elem, float hi_elem) {   // low 16 bits = first argument
+  const __half2 h = __floats2half2_rn(lo_elem, hi_elem);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+
+// power-of-two scale for one right-hand side from the bit pattern of max |psi|: max * S in [2^14, 2^15)
+__device__ __forceinline__ void rhs_scale(unsigned maxbits, float* S, float* invS) {
+  int e = (int)(maxbits >> 23);        // biased exponent, max in [2^(e-127), 2^(e-126))
+  int f = 268 - e;                     // biased exponent of S = 2^(141 - e)
+  f = f > 227 ? 227 : f;
+  if (maxbits == 0u) f = 127;
+  *S = __uint_as_float((uint32_t)f << 23);
+  *invS = __uint_as_float((uint32_t)(254 - f) << 23);
+}
+
+// work distribution: runs of `run` consecutive sites, run u -> CTA u % gridDim.x; k = position in this CTA's sequence
+struct Sched {
+  int run, nsite;
+  __device__ __forceinline__ int site(int k) const {
+    const int ui = k / run, r = k - ui * run;
+    return ((int)blockIdx.x + ui * (int)gridDim.x) * run + r;
+  }
 };
 
 }  // namespace
 
+// max |psi| per right-hand side: block = 4 sites x 72 float4 units; unit u of a record holds row n = u % 24
+__global__ void __launch_bounds__(288) colmax_kernel(const float4* __restrict__ psi, int V, unsigned* __restrict__ colmax) {
+  __shared__ unsigned smax[12];
+  if (threadIdx.x < 12) smax[threadIdx.x] = 0u;
+  __syncthreads();
+  const int unit = threadIdx.x % 72, slot = threadIdx.x / 72;
+  const int rhs = (unit % 24) >> 1;
+  unsigned m = 0u;
+  for (long long s = (long long)blockIdx.x * 4 + slot; s < V; s += (long long)gridDim.x * 4) {
+    const float4 v = __ldg(psi + s * 72 + unit);
+    m = max(m, __float_as_uint(v.x) & 0x7fffffffu);
+    m = max(m, __float_as_uint(v.y) & 0x7fffffffu);
+    m = max(m, __float_as_uint(v.z) & 0x7fffffffu);
+    m = max(m, __float_as_uint(v.w) & 0x7fffffffu);
+  }
+  atomicMax(&smax[rhs], m);
+  __syncthreads();
+  if (threadIdx.x < 12 && smax[threadIdx.x]) atomicMax(&colmax[threadIdx.x], smax[threadIdx.x]);
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
-apply_mrhs_kernel(const float* __restrict__ W, const float4* __restrict__ psi, float4* __restrict__ out, Geom g) {
+apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi, float* __restrict__ out, Geom g, int run,
+                  const unsigned* __restrict__ colmax) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ uint32_t s_tmem;
   __shared__ __align__(8) Bars bars;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  uint8_t* sB = smem;
-  float* sOut = reinterpret_cast<float*>(smem + kSmemB);
-  int* sNbr = reinterpret_cast<int*>(smem + kSmemB + kSmemOut);
+  uint8_t* sW = smem;
+  int* sNbr = reinterpret_cast<int*>(smem + kSmemW);
 
   if (tid == 0) {
-    for (int i = 0; i < kStages; ++i) { mbar_init(&bars.full[i], 7); mbar_init(&bars.empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&bars.dfull[i], 1); mbar_init(&bars.dempty[i], 4); }
-    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], 6); }
+    for (int i = 0; i < kARing; ++i) { mbar_init(&bars.afull[i], 3); mbar_init(&bars.aempty[i], 1); }
+    for (int i = 0; i < kWSlots; ++i) { mbar_init(&bars.wfull[i], 1); mbar_init(&bars.wempty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&bars.dfull[i], 1); mbar_init(&bars.dempty[i], 3); }
+    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], 3 * kG); }
     asm volatile("fence.mbarrier_init.release.cluster;");
   }
+  // the never-copied tail of every W slot (k chunk 5 of the last stage) must read as zero
+  for (int i = tid; i < kWSlots * 48; i += kThreads)
+    *reinterpret_cast<float4*>(sW + (i / 48) * kWSlotBytes + kMrhsWSiteBytes + (i % 48) * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(kTmemCols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -138,196 +173,74 @@ apply_mrhs_kernel(const float* __restrict__ W, const float4* __restrict__ psi, f
   tc_fence_after();
   const uint32_t tmem = s_tmem;
 
-  const int nsite = ((int)blockIdx.x < g.V) ? (g.V - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-  const int total = nsite * kMrhsChunks;   // chunk iterations of this CTA
+  Sched sch;
+  sch.run = run;
+  {
+    const int nruns = (g.V + run - 1) / run, b = (int)blockIdx.x, G = (int)gridDim.x;
+    const int mine = b < nruns ? (nruns - 1 - b) / G + 1 : 0;
+    int ns = mine * run;
+    if (mine > 0 && (nruns - 1) % G == b) ns -= nruns * run - g.V;   // this CTA owns the (possibly short) last run
+    sch.nsite = ns;
+  }
+  const int nsite = sch.nsite;
+  const int total = nsite * kMrhsStages;   // stage iterations of this CTA
 
   if (warp == kWarpMma) {
     // ------------------------------------------------------------------ MMA issuer
     if (lane == 0) {
       for (int k = 0, it = 0; k < nsite; ++k) {
-        const int d = k & 1;
+        const int d = k & 1, ws = k % kWSlots;
         mbar_wait(&bars.dempty[d], (((uint32_t)k >> 1) & 1u) ^ 1u);   // epilogue drained this accumulator
+        mbar_wait(&bars.wfull[ws], ((uint32_t)k / kWSlots) & 1u);     // W tile landed
         tc_fence_after();
         const uint32_t dcol = tmem + kDCol0 + 64 * d;
-        for (int c = 0; c < kMrhsChunks; ++c, ++it) {
-          const int st = it & (kStages - 1);
-          mbar_wait(&bars.full[st], ((uint32_t)it / kStages) & 1u);
+        const uint32_t w0 = smem_u32(sW + ws * kWSlotBytes);
+        for (int c = 0; c < kMrhsStages; ++c, ++it) {
+          const int st = it % kARing;
+          mbar_wait(&bars.afull[st], ((uint32_t)it / kARing) & 1u);
           tc_fence_after();
-          const uint32_t a0 = tmem + st * kACols, b0 = smem_u32(sB + st * kBStage);
-          const int nmma = (c < 6) ? 6 : 5;
-          for (int j = 0; j < nmma; ++j) {
-            const uint64_t db = umma_desc(b0 + j * 256);
+          const uint32_t a0 = tmem + st * kACols;
+#pragma unroll
+          for (int j = 0; j < 3; ++j) {
+            const uint64_t db = umma_desc(w0 + c * (kMrhsStageHalves * 2) + j * (2 * kLBO));
             const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u, zero = 0u;
             asm volatile(
                 "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n\t}\n" ::"r"(dcol),
+                "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n\t}\n" ::"r"(dcol),
                 "r"(a0 + 8 * j), "l"(db), "r"(kIdesc), "r"(acc), "r"(zero)
                 : "memory");
           }
-          umma_commit(&bars.empty[st]);                 // frees the A slot and the B tile
-          if (c == kMrhsChunks - 1) umma_commit(&bars.dfull[d]);
+          umma_commit(&bars.aempty[st]);
         }
+        umma_commit(&bars.wempty[ws]);
+        umma_commit(&bars.dfull[d]);
       }
     }
     __syncwarp();
-  } else if (warp >= kWarpA && warp < kWarpA + 8) {
-    // ------------------------------------------------------------------ A producers: W (HBM) -> TMEM
-    const int q = warp & 3, half = (warp - kWarpA) >> 2;
-    const int gq = lane >> 2, cp = lane & 3;
-    const bool active = gq < 6;                         // 6 row-parts per quarter; lanes 6,7 (+8) are pad rows
-    const int rp = q * 6 + gq;
-    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
-
-    auto load = [&](int it, AChunk& a) {
-      const int k = it / kMrhsChunks, c = it - k * kMrhsChunks;
-      const size_t n = (size_t)blockIdx.x + (size_t)k * gridDim.x;
-      const float* tile = W + n * kMrhsWSiteFloats;
-      if (!active) { a.v[0] = a.v[1] = a.v[2] = make_float4(0.f, 0.f, 0.f, 0.f); return; }
-      if (c < 6) {
-        const float4* p = reinterpret_cast<const float4*>(tile + c * kMrhsChunkFloats + rp * kMrhsChunkK) + cp;
-        a.v[0] = __ldcs(p); a.v[1] = __ldcs(p + 4); a.v[2] = __ldcs(p + 8);
-      } else {
-        const float* row = tile + 6 * kMrhsChunkFloats + rp * kMrhsLastK;
-        const float4* p = reinterpret_cast<const float4*>(row) + cp;
-        a.v[0] = __ldcs(p); a.v[1] = __ldcs(p + 4);
-        const float2 t2 = __ldcs(reinterpret_cast<const float2*>(row + 32) + cp);
-        a.v[2] = make_float4(t2.x, t2.y, 0.f, 0.f);
-      }
-    };
-    auto store = [&](int it, const AChunk& a) {
-      const int st = it & (kStages - 1);
-      mbar_wait(&bars.empty[st], (((uint32_t)it / kStages) & 1u) ^ 1u);
-      tc_fence_after();
-      const uint32_t t0 = tmem + lane_base + st * kACols;
-#pragma unroll
-      for (int J = 0; J < 3; ++J) {
-        const float4 hi = a.v[J], lo = tf32_lo(hi);
-        tmem_st_16x256(t0 + 16 * J, hi.x, hi.y, lo.x, lo.y);
-        tmem_st_16x256(t0 + 16 * J + 8, hi.z, hi.w, lo.z, lo.w);   // last chunk: columns 40..47 are never read
-      }
-      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bars.full[st]);
-    };
-
-    AChunk ring[kAPrefetch];
-#pragma unroll
-    for (int i = 0; i < kAPrefetch; ++i)
-      if (half + 2 * i < total) load(half + 2 * i, ring[i]);
-    for (int it = half; it < total; it += 2 * kAPrefetch) {
-#pragma unroll
-      for (int i = 0; i < kAPrefetch; ++i) {
-        const int cur = it + 2 * i;
-        if (cur < total) {
-          store(cur, ring[i]);
-          if (cur + 2 * kAPrefetch < total) load(cur + 2 * kAPrefetch, ring[i]);
-        }
+  } else if (warp == kWarpTma) {
+    // ------------------------------------------------------------------ W loader: HBM -> smem ring, one bulk copy per site
+    if (lane == 0) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      for (int k = 0; k < nsite; ++k) {
+        const int ws = k % kWSlots;
+        mbar_wait(&bars.wempty[ws], (((uint32_t)k / kWSlots) & 1u) ^ 1u);
+        mbar_expect_tx(&bars.wfull[ws], kMrhsWSiteBytes);
+        const uint8_t* src = W + (size_t)sch.site(k) * kMrhsWSiteBytes;
+        asm volatile(
+            "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                smem_u32(sW + ws * kWSlotBytes)),
+            "l"(src), "r"(kMrhsWSiteBytes), "r"(smem_u32(&bars.wfull[ws])), "l"(policy)
+            : "memory");
       }
     }
-  } else if ((warp >= kWarpB0 && warp < kWarpB0 + 3) || (warp >= kWarpB1 && warp < kWarpB1 + 3)) {
-    // ------------------------------------------------------------------ B producers: Psi (L2) -> smem
-    const int grp = warp >= kWarpB1 ? 1 : 0;
-    const int v = (warp - (grp ? kWarpB1 : kWarpB0)) * 32 + lane;   // 0..95; 72 units per record
-    const bool active = v < 72;
-    const int ng = v / 24, w = v - ng * 24;
-    const uint32_t dst0 = (uint32_t)(ng * kSBO + w * 16);
-
-    auto load = [&](int it, float4 (&r)[4]) {
-      const int k = it / kMrhsChunks, c = it - k * kMrhsChunks;
-      const int slot = k & (kNbrRing - 1);
-      if (c < 2) mbar_wait(&bars.nfull[slot], ((uint32_t)k / kNbrRing) & 1u);   // first chunk of site k for this group
-#pragma unroll
-      for (int rec = 0; rec < 4; ++rec) {
-        const int term = 4 * c + rec;
-        r[rec] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (active && term < kTerms) {
-          const int nn = sNbr[slot * 32 + term];
-          r[rec] = __ldg(psi + (size_t)nn * (kMrhsVecSiteFloats / 4) + v);
-        }
-      }
-      if (c >= 5) {   // last chunk of site k for this group: the index slot may be refilled
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bars.nempty[slot]);
-      }
-    };
-    auto store = [&](int it, const float4 (&r)[4]) {
-      const int st = it & (kStages - 1);
-      mbar_wait(&bars.empty[st], (((uint32_t)it / kStages) & 1u) ^ 1u);
-      if (active) {
-        uint8_t* base = sB + st * kBStage + dst0;
-#pragma unroll
-        for (int rec = 0; rec < 4; ++rec) {
-          *reinterpret_cast<float4*>(base + rec * 384) = r[rec];
-          *reinterpret_cast<float4*>(base + rec * 384 + 3 * kSBO) = tf32_lo(r[rec]);
-        }
-      }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bars.full[st]);
-    };
-
-    float4 ra[4], rb[4];
-    if (grp < total) load(grp, ra);
-    for (int it = grp; it < total; it += 4) {
-      if (it + 2 < total) load(it + 2, rb);
-      store(it, ra);
-      if (it + 2 < total) {
-        if (it + 4 < total) load(it + 4, ra);
-        store(it + 2, rb);
-      }
-    }
-  } else if (warp >= kWarpEpi && warp < kWarpEpi + 4) {
-    // ------------------------------------------------------------------ epilogue: TMEM -> out
-    const int q = warp & 3;
-    const int gq = lane >> 2, cp = lane & 3;
-    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
-    const int et = tid - kWarpEpi * 32;   // 0..127
-    for (int k = 0; k < nsite; ++k) {
-      const int d = k & 1;
-      mbar_wait(&bars.dfull[d], ((uint32_t)k >> 1) & 1u);
-      tc_fence_after();
-      const uint32_t t0 = tmem + lane_base + kDCol0 + 64 * d;
-      float r[6][4];
-#pragma unroll
-      for (int j = 0; j < 6; ++j) tmem_ld_16x256(t0 + 8 * j, r[j][0], r[j][1], r[j][2], r[j][3]);
-      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bars.dempty[d]);
-      // rows g (hi) + g+8 (lo), columns c (B hi) + c+24 (B lo):  S[j][e], n = 8 j + 2 cp + e = 2 rhs + part_psi
-      float S[3][2], O[3][2];
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-#pragma unroll
-        for (int e = 0; e < 2; ++e) S[j][e] = (r[j][e] + r[j][2 + e]) + (r[j + 3][e] + r[j + 3][2 + e]);
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-#pragma unroll
-        for (int e = 0; e < 2; ++e) O[j][e] = __shfl_xor_sync(0xffffffffu, S[j][e], 4);   // partner row-part (Re <-> Im of W)
-      // row-part gq = 2 cr + part_w.  part_w = 0 lanes write Out_r = Sr[0] - Si[1]; part_w = 1 lanes write Out_i = Sr[1] + Si[0]
-      if (gq < 6) {
-        const int part = gq & 1, comp = 3 * q + (gq >> 1);
-        float* so = sOut + d * kMrhsVecSiteFloats;
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const float val = part == 0 ? S[j][0] - O[j][1] : O[j][1] + S[j][0];
-          // out record: n = 2 rhs + part = 8 j + 2 cp + part
-          so[(j * 3 + (comp >> 2)) * 32 + (2 * cp + part) * 4 + (comp & 3)] = val;
-        }
-      }
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      if (et < kMrhsVecSiteFloats / 4) {
-        const size_t n = (size_t)blockIdx.x + (size_t)k * gridDim.x;
-        out[n * (kMrhsVecSiteFloats / 4) + et] = reinterpret_cast<const float4*>(sOut + d * kMrhsVecSiteFloats)[et];
-      }
-    }
+    __syncwarp();
   } else if (warp == kWarpIdx) {
     // ------------------------------------------------------------------ neighbour indices
     for (int k = 0; k < nsite; ++k) {
-      const int slot = k & (kNbrRing - 1);
+      const int slot = k % kNbrRing;
       mbar_wait(&bars.nempty[slot], (((uint32_t)k / kNbrRing) & 1u) ^ 1u);
-      const int n = (int)blockIdx.x + k * (int)gridDim.x;
+      const int n = sch.site(k);
       const int x = n % g.L[0];
       int qq = n / g.L[0];
       const int y = qq % g.L[1];
@@ -344,6 +257,117 @@ apply_mrhs_kernel(const float* __restrict__ W, const float4* __restrict__ psi, f
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars.nfull[slot]);
     }
+  } else if (warp >= kWarpEpi && warp < kWarpEpi + 3) {
+    // ------------------------------------------------------------------ epilogue: TMEM -> out
+    const int q = warp & 3;
+    const int gq = lane >> 2, cp = lane & 3;
+    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
+    const int nrow = 8 * q + gq;                 // n = 2 rhs + part
+    float S, invS;
+    rhs_scale(colmax[nrow >> 1], &S, &invS);
+    const float kLo = 1.f / kMrhsLoScale;
+    for (int k = 0; k < nsite; ++k) {
+      const int d = k & 1;
+      mbar_wait(&bars.dfull[d], ((uint32_t)k >> 1) & 1u);
+      tc_fence_after();
+      const uint32_t t0 = tmem + lane_base + kDCol0 + 64 * d;
+      float r[24];   // r[4J + e] = D[row g (psi hi)][col 8J + 2cp + e], r[4J + 2 + e] = D[row g + 8 (psi lo)][same col]
+      asm volatile("tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                   : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]), "=f"(r[8]),
+                     "=f"(r[9]), "=f"(r[10]), "=f"(r[11]), "=f"(r[12]), "=f"(r[13]), "=f"(r[14]), "=f"(r[15])
+                   : "r"(t0));
+      asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                   : "=f"(r[16]), "=f"(r[17]), "=f"(r[18]), "=f"(r[19]), "=f"(r[20]), "=f"(r[21]), "=f"(r[22]), "=f"(r[23])
+                   : "r"(t0 + 32));
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.dempty[d]);
+      // fold psi lo (rows g + 8) and W lo (columns 24..47 = J 3..5):  S[j][e] for W row w = 8 j + 2 cp + e = (c = 4 j + cp, part e)
+      float Sv[3][2], O[3];
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const float hi = fmaf(r[4 * j + 2 + e], kLo, r[4 * j + e]);
+          const float lo = fmaf(r[4 * (j + 3) + 2 + e], kLo, r[4 * (j + 3) + e]);
+          Sv[j][e] = fmaf(lo, kLo, hi) * invS;
+        }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) O[j] = __shfl_xor_sync(0xffffffffu, Sv[j][1], 4);   // partner row: Re <-> Im of psi
+      // even g (psi_r): Out_r = W_r psi_r - W_i psi_i ; odd g (psi_i): Out_i = W_r psi_i + W_i psi_r
+      float* rec = out + (size_t)sch.site(k) * kMrhsVecSiteFloats + nrow * 4 + cp;
+#pragma unroll
+      for (int j = 0; j < 3; ++j) rec[j * 96] = (gq & 1) ? Sv[j][0] + O[j] : Sv[j][0] - O[j];
+    }
+  } else if ((warp & 3) < 3 && warp < 4 * kG) {
+    // ------------------------------------------------------------------ A producers: Psi (L1/L2) -> fp16 hi/lo -> TMEM
+    const int q = warp & 3, gi = warp >> 2;
+    const int gq = lane >> 2, cp = lane & 3;
+    const int nrow = 8 * q + gq;
+    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
+    float S, invS;
+    rhs_scale(colmax[nrow >> 1], &S, &invS);
+    const float S2 = S * kMrhsLoScale;
+
+    auto load = [&](int it, float4 (&v)[3]) {
+      const int k = it / kMrhsStages, c = it - k * kMrhsStages;
+      const int slot = k % kNbrRing;
+      if (c < kG) mbar_wait(&bars.nfull[slot], ((uint32_t)k / kNbrRing) & 1u);   // this warp's first stage of site k
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        int term, c4;
+        if (c < 6) { term = 4 * c + cp; c4 = j; }
+        else { const int s = 4 * j + cp; term = 24 + s / 3; c4 = s - 3 * (s / 3); }
+        v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (term < kTerms) {
+          const int nn = sNbr[slot * 32 + term];
+          v[j] = __ldg(psi + (size_t)nn * (kMrhsVecSiteFloats / 4) + c4 * 24 + nrow);
+        }
+      }
+      if (c >= kMrhsStages - kG) {   // this warp's last stage of site k: the index slot may be refilled
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars.nempty[slot]);
+      }
+    };
+    auto store = [&](int it, const float4 (&v)[3]) {
+      const int st = it % kARing;
+      uint32_t h[3][4];   // [j][0,1] = hi pieces of columns 8j + 2cp, +1 ; [j][2,3] = lo pieces
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const float x0 = v[j].x * S, x1 = v[j].y * S, x2 = v[j].z * S, x3 = v[j].w * S;
+        const __half2 h01 = __floats2half2_rn(x0, x1), h23 = __floats2half2_rn(x2, x3);
+        const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
+        h[j][0] = *reinterpret_cast<const uint32_t*>(&h01);
+        h[j][1] = *reinterpret_cast<const uint32_t*>(&h23);
+        h[j][2] = pack_h2(fmaf(-kMrhsLoScale, f01.x, v[j].x * S2), fmaf(-kMrhsLoScale, f01.y, v[j].y * S2));
+        h[j][3] = pack_h2(fmaf(-kMrhsLoScale, f23.x, v[j].z * S2), fmaf(-kMrhsLoScale, f23.y, v[j].w * S2));
+      }
+      mbar_wait(&bars.aempty[st], (((uint32_t)it / kARing) & 1u) ^ 1u);
+      tc_fence_after();
+      const uint32_t t0 = tmem + lane_base + st * kACols;
+      asm volatile("tcgen05.st.sync.aligned.16x256b.x2.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(t0), "r"(h[0][0]), "r"(h[0][1]),
+                   "r"(h[0][2]), "r"(h[0][3]), "r"(h[1][0]), "r"(h[1][1]), "r"(h[1][2]), "r"(h[1][3])
+                   : "memory");
+      asm volatile("tcgen05.st.sync.aligned.16x256b.x1.b32 [%0], {%1,%2,%3,%4};" ::"r"(t0 + 16), "r"(h[2][0]), "r"(h[2][1]), "r"(h[2][2]),
+                   "r"(h[2][3])
+                   : "memory");
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.afull[st]);
+    };
+
+    float4 ra[3], rb[3];
+    if (gi < total) load(gi, ra);
+    for (int it = gi; it < total; it += 2 * kG) {
+      if (it + kG < total) load(it + kG, rb);
+      store(it, ra);
+      if (it + kG < total) {
+        if (it + 2 * kG < total) load(it + 2 * kG, ra);
+        store(it + kG, rb);
+      }
+    }
   }
 
   tc_fence_before();
@@ -354,18 +378,27 @@ apply_mrhs_kernel(const float* __restrict__ W, const float4* __restrict__ psi, f
 int launch_apply_mrhs(const ok_params* p, const void* W, const void* psi, void* out) {
   if (p->nrhs != 12 || p->precision != OK_FP32) return OK_EINVAL;
   static int sm_count = 0;
-  if (!g_moff_uploaded) {
+  static unsigned* colmax = nullptr;
+  if (!g_mrhs_ready) {
     OK_CUDA(cudaMemcpyToSymbol(c_moff, kOffsets, sizeof(kOffsets)));
     int dev = 0;
     OK_CUDA(cudaGetDevice(&dev));
     OK_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
     OK_CUDA(cudaFuncSetAttribute(apply_mrhs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
-    g_moff_uploaded = true;
+    OK_CUDA(cudaGetSymbolAddress(reinterpret_cast<void**>(&colmax), g_colmax));
+    g_mrhs_ready = true;
   }
   Geom g = make_geom(p);
-  const int grid = g.V < sm_count ? g.V : sm_count;   // one persistent CTA per SM (it owns all 512 TMEM columns)
-  apply_mrhs_kernel<<<grid, kThreads, kSmemBytes, ctx().stream>>>(static_cast<const float*>(W), static_cast<const float4*>(psi),
-                                                                 static_cast<float4*>(out), g);
+  cudaStream_t st = ctx().stream;
+  OK_CUDA(cudaMemsetAsync(colmax, 0, sizeof(unsigned) * 12, st));
+  const int cgrid = (g.V + 3) / 4 < sm_count * 8 ? (g.V + 3) / 4 : sm_count * 8;
+  colmax_kernel<<<cgrid, 288, 0, st>>>(static_cast<const float4*>(psi), g.V, colmax);
+  OK_LAUNCHED("colmax_kernel");
+  const int run = g.L[0] < 8 ? 8 : (g.L[0] > 32 ? 32 : g.L[0]);   // consecutive sites per work unit (an x line when 8 <= Lx <= 32)
+  const int nruns = (g.V + run - 1) / run;
+  const int grid = nruns < sm_count ? nruns : sm_count;   // one persistent CTA per SM (it owns all 512 TMEM columns)
+  apply_mrhs_kernel<<<grid, kThreads, kSmemBytes, st>>>(static_cast<const uint8_t*>(W), static_cast<const float4*>(psi),
+                                                        static_cast<float*>(out), g, run, colmax);
   OK_LAUNCHED("apply_mrhs_kernel");
   return OK_SUCCESS;
 }

@@ -6,7 +6,7 @@
 // tensor-core apply (ok_apply_mrhs.cu), one W stream for the 12 columns.
 //
 // Vector layout: per-site records of 36 units of 32 B = (re[4], im[4]) of components 4 c4 .. 4 c4 + 3
-// for one column (ok_internal.cuh, mrhs_vec_index): unit q = (ng*3 + c4)*4 + p, column j = 4 ng + p.
+// for one column (ok_internal.cuh, mrhs_vec_index): unit q = 12 c4 + j, column j = q % 12.
 // A thread keeps q (hence j) fixed and strides over sites, so per-column reductions need no atomics:
 // thread -> smem -> fixed-order sum per (column, quantity) -> one partial per CTA -> single-CTA final.
 #include <math.h>
@@ -62,17 +62,16 @@ __device__ __forceinline__ void column_reduce(const double (&d)[NQ], int unit, d
   __syncthreads();
   if (threadIdx.x < kN * NQ) {
     const int j = threadIdx.x / NQ, q = threadIdx.x % NQ;
-    const int ng = j >> 2, p = j & 3;
     double s = 0.0;
     for (int slot = 0; slot < 8; ++slot)
-      for (int c4 = 0; c4 < 3; ++c4) s += red[slot * 36 + (ng * 3 + c4) * 4 + p][q];
+      for (int c4 = 0; c4 < 3; ++c4) s += red[slot * 36 + c4 * 12 + j][q];
     out[j * 3 + q] = s;
   }
 }
 
 #define OK_MRHS_LOOP(site)                                                      \
   const int unit = threadIdx.x % 36, slot = threadIdx.x / 36;                   \
-  const int j = 4 * (unit / 12) + (unit & 3);                                   \
+  const int j = unit % 12;                                                      \
   const long long s0__ = (long long)blockIdx.x * kSitesPerCta;                  \
   long long s1__ = s0__ + kSitesPerCta;                                         \
   if (s1__ > V) s1__ = V;                                                       \

@@ -1,6 +1,7 @@
 // Internal declarations shared by the translation units of libokdirac (not part of the ABI).
 #pragma once
 
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -13,40 +14,60 @@ constexpr int kBlock = OK_SITE_BLOCK;   // sites per block (= warp width: lane <
 constexpr int kTerms = OK_NTERMS;
 constexpr uint32_t kMagic = 0x4F4B5731u;   // "OKW1"
 constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
-constexpr uint32_t kLayoutMrhs = 2;        // nrhs = 12: per-site tcgen05 A-operand tiles (ok_apply_mrhs.cu)
+constexpr uint32_t kLayoutMrhs = 3;        // nrhs = 12: per-site tcgen05 operand tiles, split fp16 (ok_apply_mrhs.cu)
 
-// ---- nrhs = 12 (tensor-core) layouts, fp32 only -------------------------------------------------
-// W: per site the real-split A operand [W_r ; W_i] (24 row-parts x K = 324), cut along K into 7 chunks of
-// 4 stencil terms (48 k; the last chunk holds 3 terms + 4 zero pad k = 40).  Inside a chunk the 24
-// row-parts are ordered for the four TMEM lane quarters of ok_apply_mrhs.cu: rp = 6*(row/3) + 2*(row%3)
-// + part (part 0 = Re, 1 = Im), each a contiguous run of 48 (40) floats.  Inside a run the k order is
-// permuted so that the 16 B a thread loads are exactly the 4 values it stores with tcgen05.st.16x256b:
-// float m = 16 J + 4 cp + 2 h + e  <->  TMEM column (= k in chunk) c = 16 J + 8 h + 2 cp + e
-// (columns 32..39 of the last chunk are stored in natural order).  31 488 B per site.
-constexpr int kMrhsChunkTerms = 4;
-constexpr int kMrhsChunks = 7;
-constexpr int kMrhsChunkK = 48;
-constexpr int kMrhsLastK = 40;
-constexpr int kMrhsChunkFloats = 24 * kMrhsChunkK;                          // 1152
-constexpr int kMrhsWSiteFloats = 6 * kMrhsChunkFloats + 24 * kMrhsLastK;    // 7872
-__host__ __device__ inline int mrhs_W_perm(int c) {   // column in chunk -> float position in the run
-  return (c & ~15) | (((c >> 1) & 3) << 2) | (((c >> 3) & 1) << 1) | (c & 1);
+// ---- nrhs = 12 (tensor-core) layouts, fp32 fields (ok_apply_mrhs.cu) -------------------------------
+// The per-site contraction Out[12 x 12] = sum_term W_term[12 x 12] Psi(x + o_term)[12 x 12] (complex) is run
+// real-split on tcgen05 kind::f16 as  D[n][w] = sum_k A[n][k] B[w][k]  with
+//   A (M side, tensor memory)  = Psi^T : row n = 2 rhs + part (part 0 = Re, 1 = Im), K = (term, component)
+//   B (N side, shared memory)  = W     : row w = 8 (row/4) + 2 (row%4) + part,       K = (term, column)
+// and every fp32 number carried as two fp16 pieces  x = hi + lo / 2048  (hi = rn(x), lo = rn((x - hi) 2048)),
+// 22 significant bits, stacked as extra rows on both sides.
+//
+// K order: 7 stages of 48 k (4 stencil terms each; the last stage has 3 terms + 12 zero pad k).
+//   stage c < 6 : k = 16 (comp/4) + 4 (term%4) + comp%4
+//   stage 6     : s = 3 (term - 24) + comp/4 ;  k = 16 (s/4) + 4 (s%4) + comp%4   (k = 36..47 are pad)
+// This is the order in which a spinor producer thread (row n, cp = lane%4) holds its three 16-byte loads.
+//
+// W tile (per site, fp16, 31 488 B): the UMMA canonical K-major no-swizzle layout of B,
+//   [stage 7][k chunk k/8 : 6][row group w48/8 : 6][w48 % 8][k % 8],   w48 = 24 hl + w  (hl 0 = hi, 1 = lo)
+// (core matrix = 8 rows x 16 B; SBO = 128 B between row groups, LBO = 768 B between k chunks); the all-pad
+// k chunk 5 of stage 6 is not stored.  One contiguous tile = one bulk copy into shared memory.
+constexpr int kMrhsStages = 7;
+constexpr int kMrhsStageK = 48;
+constexpr int kMrhsStageHalves = 48 * kMrhsStageK;                           // 2304 (4608 B)
+constexpr int kMrhsWSiteHalves = kMrhsStages * kMrhsStageHalves - 6 * 64;    // 15 744
+constexpr int kMrhsWSiteBytes = 2 * kMrhsWSiteHalves;                        // 31 488
+constexpr float kMrhsLoScale = 2048.f;                                       // lo pieces are stored x 2^11
+__host__ __device__ inline int mrhs_k(int term, int comp, int* stage) {
+  const int c = term >> 2;
+  *stage = c;
+  if (c < 6) return 16 * (comp >> 2) + 4 * (term & 3) + (comp & 3);
+  const int s = 3 * (term - 24) + (comp >> 2);
+  return 16 * (s >> 2) + 4 * (s & 3) + (comp & 3);
 }
-__host__ __device__ inline int mrhs_W_rowpart(int row, int part) { return 6 * (row / 3) + 2 * (row % 3) + part; }
-__host__ __device__ inline int mrhs_W_index(int term, int row, int col, int part) {
-  const int chunk = term >> 2, c = (term & 3) * 12 + col, rp = mrhs_W_rowpart(row, part);
-  if (chunk < 6) return chunk * kMrhsChunkFloats + rp * kMrhsChunkK + mrhs_W_perm(c);
-  return 6 * kMrhsChunkFloats + rp * kMrhsLastK + (c < 32 ? mrhs_W_perm(c) : c);
+__host__ __device__ inline int mrhs_W_row(int row, int part) { return 8 * (row >> 2) + 2 * (row & 3) + part; }
+__host__ __device__ inline int mrhs_W_half_index(int stage, int k, int w48) {
+  return stage * kMrhsStageHalves + (k >> 3) * 384 + (w48 >> 3) * 64 + (w48 & 7) * 8 + (k & 7);
 }
-__host__ __device__ inline int mrhs_W_pad_index(int q) {   // q = 0..95: the zero pad floats (k = 36..39 of the last chunk)
-  return 6 * kMrhsChunkFloats + (q >> 2) * kMrhsLastK + 36 + (q & 3);
+__host__ __device__ inline int mrhs_W_index(int term, int row, int col, int part, int hl) {
+  int stage;
+  const int k = mrhs_k(term, col, &stage);
+  return mrhs_W_half_index(stage, k, 24 * hl + mrhs_W_row(row, part));
 }
-// spinor: per site the B operand [Psi_r , Psi_i] (24 x 12) as 9 core matrices:
-// [n group n/8 = 0..2][k chunk c/4 = 0..2][n%8][c%4], n = 2*rhs + part, c = component.  1152 B per site.
+__host__ __device__ inline int mrhs_W_pad_index(int q) {   // q = 0..191: zero pad halves (k = 36..39 of stage 6, 48 rows)
+  return mrhs_W_half_index(6, 36 + (q & 3), q >> 2);
+}
+__host__ __device__ inline void mrhs_split(float x, __half* hi, __half* lo) {
+  const __half h = __float2half_rn(x);
+  *hi = h;
+  *lo = __float2half_rn((x - __half2float(h)) * kMrhsLoScale);
+}
+__host__ __device__ inline float mrhs_join(__half hi, __half lo) { return __half2float(hi) + __half2float(lo) * (1.f / kMrhsLoScale); }
+// spinor record (per site, fp32, 1152 B): [component/4 : 3][n = 2 rhs + part : 24][component%4]
 constexpr int kMrhsVecSiteFloats = 288;
 __host__ __device__ inline int mrhs_vec_index(int comp, int rhs, int part) {
-  const int n = 2 * rhs + part;
-  return ((n >> 3) * 3 + (comp >> 2)) * 32 + (n & 7) * 4 + (comp & 3);
+  return ((comp >> 2) * 24 + 2 * rhs + part) * 4 + (comp & 3);
 }
 
 struct Geom {

@@ -24,7 +24,7 @@ __global__ void pack_spinor_kernel(const vec_t* __restrict__ canon, vec_t* __res
   }
 }
 
-// nrhs = 12, fp32: canonical [n][comp][rhs][re,im] <-> per-site B-operand records (ok_internal.cuh,
+// nrhs = 12, fp32: canonical [n][comp][rhs][re,im] <-> per-site records (ok_internal.cuh,
 // mrhs_vec_index).  One thread per complex number.
 __global__ void pack_spinor_mrhs_kernel(const float2* __restrict__ canon, float* __restrict__ packed, int V, bool unpack) {
   long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -42,28 +42,30 @@ __global__ void pack_spinor_mrhs_kernel(const float2* __restrict__ canon, float*
   }
 }
 
-// nrhs = 12 W: canonical [n][27][12][12][re,im] <-> per-site A-operand tiles (mrhs_W_index); the
-// zero pad (k = 324..327 of every row-part) is written when packing.
-__global__ void pack_W_mrhs_kernel(const float2* __restrict__ canon, float* __restrict__ packed, int V, bool unpack) {
-  constexpr int kPer = kTerms * 144 + 96;
+// nrhs = 12 W: canonical [n][27][12][12][re,im] (fp32) <-> per-site split-fp16 B-operand tiles
+// (ok_internal.cuh: mrhs_W_index, mrhs_split).  Packing keeps 22 significant bits of every real
+// (|x - unpack(pack(x))| <= 2^-22 |x| for 2^-14 <= |x| <= 65504); the zero pad is written when packing.
+__global__ void pack_W_mrhs_kernel(const float2* __restrict__ canon, __half* __restrict__ packed, int V, bool unpack) {
+  constexpr int kPer = kTerms * 144 + 192;
   long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (u >= (long long)V * kPer) return;
   const int e = (int)(u % kPer);
   const long long n = u / kPer;
-  float* tile = packed + n * kMrhsWSiteFloats;
-  if (e >= kTerms * 144) {   // the 96 zero pad floats of the last chunk
-    if (!unpack) tile[mrhs_W_pad_index(e - kTerms * 144)] = 0.f;
+  __half* tile = packed + n * kMrhsWSiteHalves;
+  if (e >= kTerms * 144) {   // the 192 zero pad halves of the last stage
+    if (!unpack) tile[mrhs_W_pad_index(e - kTerms * 144)] = __float2half_rn(0.f);
     return;
   }
   const int col = e % 12, row = (e / 12) % 12, term = e / 144;
-  const int ir = mrhs_W_index(term, row, col, 0), ii = mrhs_W_index(term, row, col, 1);
+  const int rh = mrhs_W_index(term, row, col, 0, 0), rl = mrhs_W_index(term, row, col, 0, 1);
+  const int ih = mrhs_W_index(term, row, col, 1, 0), il = mrhs_W_index(term, row, col, 1, 1);
   const long long cu = n * (kTerms * 144) + e;
   if (unpack) {
-    const_cast<float2*>(canon)[cu] = make_float2(tile[ir], tile[ii]);
+    const_cast<float2*>(canon)[cu] = make_float2(mrhs_join(tile[rh], tile[rl]), mrhs_join(tile[ih], tile[il]));
   } else {
     const float2 v = canon[cu];
-    tile[ir] = v.x;
-    tile[ii] = v.y;
+    mrhs_split(v.x, &tile[rh], &tile[rl]);
+    mrhs_split(v.y, &tile[ih], &tile[il]);
   }
 }
 
@@ -117,9 +119,9 @@ __global__ void pack_W_kernel(const vec_t* __restrict__ canon, vec_t* __restrict
 int launch_pack_W(const ok_params* p, const void* canon, void* Wp, bool unpack) {
   Geom g = make_geom(p);
   if (p->nrhs == 12) {
-    long long tot = (long long)g.V * (kTerms * 144 + 96);
+    long long tot = (long long)g.V * (kTerms * 144 + 192);
     pack_W_mrhs_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx().stream>>>(static_cast<const float2*>(canon),
-                                                                                static_cast<float*>(Wp), g.V, unpack);
+                                                                                static_cast<__half*>(Wp), g.V, unpack);
     OK_LAUNCHED("pack_W_mrhs_kernel");
     return OK_SUCCESS;
   }

@@ -358,15 +358,15 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
     }
     unit_t* dst = Wt + (size_t)r * NC * kBlock;
     if constexpr (sizeof(real) == 4) {
-      if (a.mrhs) {   // A-operand tile of ok_apply_mrhs.cu (ok_internal.cuh: mrhs_W_index)
-        float* tile = reinterpret_cast<float*>(W) + (size_t)n * kMrhsWSiteFloats;
+      if (a.mrhs) {   // split-fp16 B-operand tile of ok_apply_mrhs.cu (ok_internal.cuh: mrhs_W_index); fp64 -> fp32 -> (hi, lo)
+        __half* tile = reinterpret_cast<__half*>(W) + (size_t)n * kMrhsWSiteHalves;
 #pragma unroll
         for (int col = 0; col < 12; ++col) {
-          tile[mrhs_W_index(term, r, col, 0)] = (float)row[col].x;
-          tile[mrhs_W_index(term, r, col, 1)] = (float)row[col].y;
+          mrhs_split((float)row[col].x, &tile[mrhs_W_index(term, r, col, 0, 0)], &tile[mrhs_W_index(term, r, col, 0, 1)]);
+          mrhs_split((float)row[col].y, &tile[mrhs_W_index(term, r, col, 1, 0)], &tile[mrhs_W_index(term, r, col, 1, 1)]);
         }
-        if (term == 0)   // zero pad k = 324..327 of the two row-parts of row r
-          for (int q = 0; q < 8; ++q) tile[mrhs_W_pad_index(4 * mrhs_W_rowpart(r, q >> 2) + (q & 3))] = 0.f;
+        if (term == 0)   // zero pad k = 36..39 of the last stage: 192 halves per site, 16 per row r
+          for (int q = 0; q < 16; ++q) tile[mrhs_W_pad_index(16 * r + q)] = __float2half_rn(0.f);
         continue;
       }
 #pragma unroll

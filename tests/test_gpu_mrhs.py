@@ -1,7 +1,7 @@
 """Parity of the 12-right-hand-side mode (BASELINE.json configs[3]) with the CPU oracle.
 
 The 12-RHS apply is Eq. (2.2) applied to 12 spinor fields at once: per site a complex
-12 x 324 by 324 x 12 contraction on the tensor cores (split TF32).  The oracle side is simply the
+12 x 324 by 324 x 12 contraction on the tensor cores (split fp16, kind::f16).  The oracle side is simply the
 single-RHS oracle called column by column.  Tolerance: relative L2 <= 2e-5 per column (north_star, fp32).
 """
 import numpy as np
@@ -17,6 +17,7 @@ import okgpu as G
 pytestmark = pytest.mark.gpu
 
 FP32_TOL = 2e-5
+W22_REL = 2.0 ** -22      # split-fp16 W storage: |x - (hi + lo/2048)| <= 2^-11 * 2^-11 |x| (two round-to-nearest fp16 steps)
 NR = 12
 SHAPES = [(4, 3, 3, 2), (2, 2, 2, 2), (4, 4, 4, 8), (5, 2, 3, 4)]
 
@@ -56,7 +57,11 @@ def test_mrhs_pack_unpack_roundtrip(dims):
     Wc = (rng.normal(size=(V, 27, 12, 12)) + 1j * rng.normal(size=(V, 27, 12, 12))).astype(np.complex64)
     W = B.alloc_W(p)
     B.ok_pack_W(p, G.to_dev(Wc), W)
-    assert np.array_equal(G.unpack_W(p, W, V).astype(np.complex64), Wc)
+    back = G.unpack_W(p, W, V)
+    # the 12-RHS W tile stores every real as two fp16 pieces (hi + lo / 2048): 22 significant bits
+    err = np.maximum(np.abs(back.real - Wc.real), np.abs(back.imag - Wc.imag))
+    ref = np.maximum(np.abs(Wc.real), np.abs(Wc.imag))
+    assert np.all(err <= W22_REL * ref + 2.0 ** -36)
     q = B.ok_W_params(W)
     assert list(q.dims) == list(dims) and q.nrhs == NR
 
@@ -87,7 +92,7 @@ def test_mrhs_precalc_layout_and_apply(dims):
     W = G.precalc(p, U)
     want_W = o.precalc_W()
     got_W = G.unpack_W(p, W, o.V)
-    assert np.abs(got_W - want_W).max() <= 2e-7 * np.abs(want_W).max()
+    assert np.abs(got_W - want_W).max() <= (2.0 ** -24 + W22_REL) * np.sqrt(2) * np.abs(want_W).max()
     psi = point_sources(dims)
     got = G.apply(p, W, psi)
     want = np.stack([o.apply_W(psi[:, :, j], W=want_W) for j in range(NR)], axis=2)
