@@ -12,11 +12,11 @@
 // weights 1, 2^-11, 2^-11, 2^-22 in fp32.  W is stored pre-split in HBM (4 bytes per real, like fp32), so it
 // goes HBM -> shared memory -> tensor core with no thread touching it.
 //
-// One persistent CTA per SM, 16 specialised warps; sites are dealt in runs of consecutive x (L1 reuse of the
+// One persistent CTA per SM, 20 specialised warps; sites are dealt in runs of consecutive x (L1 reuse of the
 // gathered spinor records), runs round-robin over the CTAs (so all CTAs sweep the lattice together and the
 // records stay in L2).  Per site 7 K-stages of 4 stencil terms (48 k = 24 TMEM columns):
 //   W loader   1 thread: one 31 488-B bulk copy (cp.async.bulk, L2 evict-first) per site into a 4-slot smem ring.
-//   A producers 9 warps (3 per TMEM lane quarter, quarter q = rows n = 8q..8q+7): gather the 4 neighbour records
+//   A producers 12 warps (4 per TMEM lane quarter, quarter q = rows n = 8q..8q+7): gather the 4 neighbour records
 //              of a stage (three 16-B loads per thread, L1/L2), scale, split into fp16 hi/lo and write rows g
 //              (hi) and g + 8 (lo) with tcgen05.st.16x256b into a 16-slot ring of 24 TMEM columns.
 //   MMA        1 thread: 3 tcgen05.mma (A from tensor memory, B from smem) per stage into one of two
@@ -35,7 +35,7 @@ static bool g_mrhs_ready = false;
 
 namespace {
 
-constexpr int kG = 3;                               // producer warps per lane quarter
+constexpr int kG = 4;                               // producer warps per lane quarter
 constexpr int kARing = 16;                          // A ring slots
 constexpr int kACols = 24;                          // TMEM columns per slot (48 fp16 k)
 constexpr int kWSlots = 4;                          // W ring (sites)
@@ -45,8 +45,9 @@ constexpr int kTmemCols = 512;
 constexpr int kNbrRing = 8;
 constexpr int kSBO = 128, kLBO = 768;
 
-constexpr int kWarpMma = 3, kWarpTma = 7, kWarpIdx = 11, kWarpEpi = 12;
-constexpr int kWarps = 16, kThreads = kWarps * 32;
+constexpr int kWarpMma = 3, kWarpTma = 7, kWarpIdx = 11, kWarpEpi = 4 * kG;   // warps 4i + 3 are free of TMEM lane duty
+constexpr int kWarps = 4 * kG + 4, kThreads = kWarps * 32;
+static_assert(kG >= 3 && kG <= 7, "producer groups");
 
 constexpr int kSmemW = kWSlots * kWSlotBytes;       // 129 024
 constexpr int kSmemNbr = kNbrRing * 32 * 4;
@@ -112,12 +113,19 @@ __device__ __forceinline__ void rhs_scale(unsigned maxbits, float* S, float* inv
   *invS = __uint_as_float((uint32_t)(254 - f) << 23);
 }
 
-// work distribution: runs of `run` consecutive sites, run u -> CTA u % gridDim.x; k = position in this CTA's sequence
-struct Sched {
-  int run, nsite;
-  __device__ __forceinline__ int site(int k) const {
-    const int ui = k / run, r = k - ui * run;
-    return ((int)blockIdx.x + ui * (int)gridDim.x) * run + r;
+__device__ __forceinline__ bool elect_one() {   // one lane of a converged warp
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(pred));
+  return pred != 0;
+}
+
+// work distribution: runs of `run` consecutive sites, run u -> CTA u % gridDim.x; iterates this CTA's site sequence
+struct SiteIter {
+  int n, r, run, skip;
+  __device__ __forceinline__ explicit SiteIter(int run_) : n((int)blockIdx.x * run_), r(0), run(run_), skip(((int)gridDim.x - 1) * run_) {}
+  __device__ __forceinline__ void next() {
+    ++n;
+    if (++r == run) { r = 0; n += skip; }
   }
 };
 
@@ -173,31 +181,32 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
   tc_fence_after();
   const uint32_t tmem = s_tmem;
 
-  Sched sch;
-  sch.run = run;
+  int nsite;   // sites of this CTA
   {
     const int nruns = (g.V + run - 1) / run, b = (int)blockIdx.x, G = (int)gridDim.x;
     const int mine = b < nruns ? (nruns - 1 - b) / G + 1 : 0;
-    int ns = mine * run;
-    if (mine > 0 && (nruns - 1) % G == b) ns -= nruns * run - g.V;   // this CTA owns the (possibly short) last run
-    sch.nsite = ns;
+    nsite = mine * run;
+    if (mine > 0 && (nruns - 1) % G == b) nsite -= nruns * run - g.V;   // this CTA owns the (possibly short) last run
   }
-  const int nsite = sch.nsite;
   const int total = nsite * kMrhsStages;   // stage iterations of this CTA
 
   if (warp == kWarpMma) {
-    // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
-      for (int k = 0, it = 0; k < nsite; ++k) {
-        const int d = k & 1, ws = k % kWSlots;
-        mbar_wait(&bars.dempty[d], (((uint32_t)k >> 1) & 1u) ^ 1u);   // epilogue drained this accumulator
-        mbar_wait(&bars.wfull[ws], ((uint32_t)k / kWSlots) & 1u);     // W tile landed
+    // ------------------------------------------------------------------ MMA issuer (one elected thread, warp-uniform path)
+    if (elect_one()) {
+      int st = 0;
+      uint32_t aph = 0, wph = 0, dph = 1;
+      int ws = 0;
+      for (int k = 0; k < nsite; ++k) {
+        const int d = k & 1;
+        mbar_wait(&bars.dempty[d], dph);          // epilogue drained this accumulator
+        dph ^= (uint32_t)d;                       // both accumulators used once -> next phase
+        mbar_wait(&bars.wfull[ws], wph);          // W tile landed
         tc_fence_after();
         const uint32_t dcol = tmem + kDCol0 + 64 * d;
         const uint32_t w0 = smem_u32(sW + ws * kWSlotBytes);
-        for (int c = 0; c < kMrhsStages; ++c, ++it) {
-          const int st = it % kARing;
-          mbar_wait(&bars.afull[st], ((uint32_t)it / kARing) & 1u);
+#pragma unroll
+        for (int c = 0; c < kMrhsStages; ++c) {
+          mbar_wait(&bars.afull[st], aph);
           tc_fence_after();
           const uint32_t a0 = tmem + st * kACols;
 #pragma unroll
@@ -211,36 +220,43 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
                 : "memory");
           }
           umma_commit(&bars.aempty[st]);
+          if (++st == kARing) { st = 0; aph ^= 1u; }
         }
         umma_commit(&bars.wempty[ws]);
         umma_commit(&bars.dfull[d]);
+        if (++ws == kWSlots) { ws = 0; wph ^= 1u; }
       }
     }
     __syncwarp();
   } else if (warp == kWarpTma) {
     // ------------------------------------------------------------------ W loader: HBM -> smem ring, one bulk copy per site
-    if (lane == 0) {
+    if (elect_one()) {
       uint64_t policy;
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
-      for (int k = 0; k < nsite; ++k) {
-        const int ws = k % kWSlots;
-        mbar_wait(&bars.wempty[ws], (((uint32_t)k / kWSlots) & 1u) ^ 1u);
+      SiteIter si(run);
+      int ws = 0;
+      uint32_t eph = 1;
+      for (int k = 0; k < nsite; ++k, si.next()) {
+        mbar_wait(&bars.wempty[ws], eph);
         mbar_expect_tx(&bars.wfull[ws], kMrhsWSiteBytes);
-        const uint8_t* src = W + (size_t)sch.site(k) * kMrhsWSiteBytes;
+        const uint8_t* src = W + (size_t)si.n * kMrhsWSiteBytes;
         asm volatile(
             "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
                 smem_u32(sW + ws * kWSlotBytes)),
             "l"(src), "r"(kMrhsWSiteBytes), "r"(smem_u32(&bars.wfull[ws])), "l"(policy)
             : "memory");
+        if (++ws == kWSlots) { ws = 0; eph ^= 1u; }
       }
     }
     __syncwarp();
   } else if (warp == kWarpIdx) {
     // ------------------------------------------------------------------ neighbour indices
-    for (int k = 0; k < nsite; ++k) {
-      const int slot = k % kNbrRing;
-      mbar_wait(&bars.nempty[slot], (((uint32_t)k / kNbrRing) & 1u) ^ 1u);
-      const int n = sch.site(k);
+    SiteIter si(run);
+    int slot = 0;
+    uint32_t eph = 1;
+    for (int k = 0; k < nsite; ++k, si.next()) {
+      mbar_wait(&bars.nempty[slot], eph);
+      const int n = si.n;
       const int x = n % g.L[0];
       int qq = n / g.L[0];
       const int y = qq % g.L[1];
@@ -256,6 +272,7 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars.nfull[slot]);
+      if (++slot == kNbrRing) { slot = 0; eph ^= 1u; }
     }
   } else if (warp >= kWarpEpi && warp < kWarpEpi + 3) {
     // ------------------------------------------------------------------ epilogue: TMEM -> out
@@ -266,9 +283,14 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
     float S, invS;
     rhs_scale(colmax[nrow >> 1], &S, &invS);
     const float kLo = 1.f / kMrhsLoScale;
-    for (int k = 0; k < nsite; ++k) {
+    const float sgn = (gq & 1) ? 1.f : -1.f;
+    float* obase = out + nrow * 4 + cp;
+    SiteIter si(run);
+    uint32_t fph = 0;
+    for (int k = 0; k < nsite; ++k, si.next()) {
       const int d = k & 1;
-      mbar_wait(&bars.dfull[d], ((uint32_t)k >> 1) & 1u);
+      mbar_wait(&bars.dfull[d], fph);
+      fph ^= (uint32_t)d;
       tc_fence_after();
       const uint32_t t0 = tmem + lane_base + kDCol0 + 64 * d;
       float r[24];   // r[4J + e] = D[row g (psi hi)][col 8J + 2cp + e], r[4J + 2 + e] = D[row g + 8 (psi lo)][same col]
@@ -283,7 +305,7 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars.dempty[d]);
-      // fold psi lo (rows g + 8) and W lo (columns 24..47 = J 3..5):  S[j][e] for W row w = 8 j + 2 cp + e = (c = 4 j + cp, part e)
+      // fold psi lo (rows g + 8) and W lo (columns 24..47 = J 3..5):  Sv[j][e] for W row w = 8 j + 2 cp + e = (c = 4 j + cp, part e)
       float Sv[3][2], O[3];
 #pragma unroll
       for (int j = 0; j < 3; ++j)
@@ -296,56 +318,69 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
 #pragma unroll
       for (int j = 0; j < 3; ++j) O[j] = __shfl_xor_sync(0xffffffffu, Sv[j][1], 4);   // partner row: Re <-> Im of psi
       // even g (psi_r): Out_r = W_r psi_r - W_i psi_i ; odd g (psi_i): Out_i = W_r psi_i + W_i psi_r
-      float* rec = out + (size_t)sch.site(k) * kMrhsVecSiteFloats + nrow * 4 + cp;
+      float* rec = obase + (size_t)si.n * kMrhsVecSiteFloats;
 #pragma unroll
-      for (int j = 0; j < 3; ++j) rec[j * 96] = (gq & 1) ? Sv[j][0] + O[j] : Sv[j][0] - O[j];
+      for (int j = 0; j < 3; ++j) rec[j * 96] = fmaf(sgn, O[j], Sv[j][0]);
     }
   } else if ((warp & 3) < 3 && warp < 4 * kG) {
     // ------------------------------------------------------------------ A producers: Psi (L1/L2) -> fp16 hi/lo -> TMEM
+    // warp (q, gi) handles the stages it = gi, gi + kG, ... of this CTA's stage sequence (it = 7 k + c) for rows 8q..8q+7
     const int q = warp & 3, gi = warp >> 2;
     const int gq = lane >> 2, cp = lane & 3;
     const int nrow = 8 * q + gq;
-    const uint32_t lane_base = (uint32_t)(32 * q) << 16;
     float S, invS;
     rhs_scale(colmax[nrow >> 1], &S, &invS);
     const float S2 = S * kMrhsLoScale;
+    const float4* pbase = psi + nrow;                       // + 72 nn + 24 c4
+    const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16);
+    const int nmine = total > gi ? (total - gi + kG - 1) / kG : 0;
 
-    auto load = [&](int it, float4 (&v)[3]) {
-      const int k = it / kMrhsStages, c = it - k * kMrhsStages;
-      const int slot = k % kNbrRing;
-      if (c < kG) mbar_wait(&bars.nfull[slot], ((uint32_t)k / kNbrRing) & 1u);   // this warp's first stage of site k
+    // load side state: stage c of the site in index-ring slot lslot
+    int lc = gi, lslot = 0;
+    uint32_t lph = 0;
+    auto load = [&](float4 (&v)[3]) {
+      if (lc < kG) mbar_wait(&bars.nfull[lslot], lph);      // this warp's first stage of the site
+      const int* nb = sNbr + lslot * 32;
+      if (lc < 6) {
+        const float4* rec = pbase + (size_t)nb[4 * lc + cp] * (kMrhsVecSiteFloats / 4);
+        v[0] = __ldg(rec);
+        v[1] = __ldg(rec + 24);
+        v[2] = __ldg(rec + 48);
+      } else {   // terms 24..26: slot s = 4 j + cp < 9 -> (term 24 + s/3, c4 = s%3)
 #pragma unroll
-      for (int j = 0; j < 3; ++j) {
-        int term, c4;
-        if (c < 6) { term = 4 * c + cp; c4 = j; }
-        else { const int s = 4 * j + cp; term = 24 + s / 3; c4 = s - 3 * (s / 3); }
-        v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (term < kTerms) {
-          const int nn = sNbr[slot * 32 + term];
-          v[j] = __ldg(psi + (size_t)nn * (kMrhsVecSiteFloats / 4) + c4 * 24 + nrow);
+        for (int j = 0; j < 3; ++j) {
+          const int s = 4 * j + cp;
+          v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (s < 9) v[j] = __ldg(pbase + (size_t)nb[24 + s / 3] * (kMrhsVecSiteFloats / 4) + (s % 3) * 24);
         }
       }
-      if (c >= kMrhsStages - kG) {   // this warp's last stage of site k: the index slot may be refilled
+      if (lc >= kMrhsStages - kG) {                         // this warp's last stage of the site: the index slot may be refilled
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bars.nempty[slot]);
+        if (lane == 0) mbar_arrive(&bars.nempty[lslot]);
+      }
+      lc += kG;
+      if (lc >= kMrhsStages) {
+        lc -= kMrhsStages;
+        if (++lslot == kNbrRing) { lslot = 0; lph ^= 1u; }
       }
     };
-    auto store = [&](int it, const float4 (&v)[3]) {
-      const int st = it % kARing;
+    // store side state: A ring slot
+    int st = gi;
+    uint32_t eph = 1;
+    auto store = [&](const float4 (&v)[3]) {
       uint32_t h[3][4];   // [j][0,1] = hi pieces of columns 8j + 2cp, +1 ; [j][2,3] = lo pieces
 #pragma unroll
       for (int j = 0; j < 3; ++j) {
-        const float x0 = v[j].x * S, x1 = v[j].y * S, x2 = v[j].z * S, x3 = v[j].w * S;
-        const __half2 h01 = __floats2half2_rn(x0, x1), h23 = __floats2half2_rn(x2, x3);
+        const __half2 h01 = __floats2half2_rn(v[j].x * S, v[j].y * S), h23 = __floats2half2_rn(v[j].z * S, v[j].w * S);
         const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
         h[j][0] = *reinterpret_cast<const uint32_t*>(&h01);
         h[j][1] = *reinterpret_cast<const uint32_t*>(&h23);
         h[j][2] = pack_h2(fmaf(-kMrhsLoScale, f01.x, v[j].x * S2), fmaf(-kMrhsLoScale, f01.y, v[j].y * S2));
         h[j][3] = pack_h2(fmaf(-kMrhsLoScale, f23.x, v[j].z * S2), fmaf(-kMrhsLoScale, f23.y, v[j].w * S2));
       }
-      mbar_wait(&bars.aempty[st], (((uint32_t)it / kARing) & 1u) ^ 1u);
+      mbar_wait(&bars.aempty[st], eph);
       tc_fence_after();
-      const uint32_t t0 = tmem + lane_base + st * kACols;
+      const uint32_t t0 = tbase + st * kACols;
       asm volatile("tcgen05.st.sync.aligned.16x256b.x2.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(t0), "r"(h[0][0]), "r"(h[0][1]),
                    "r"(h[0][2]), "r"(h[0][3]), "r"(h[1][0]), "r"(h[1][1]), "r"(h[1][2]), "r"(h[1][3])
                    : "memory");
@@ -356,16 +391,18 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars.afull[st]);
+      st += kG;
+      if (st >= kARing) { st -= kARing; eph ^= 1u; }
     };
 
     float4 ra[3], rb[3];
-    if (gi < total) load(gi, ra);
-    for (int it = gi; it < total; it += 2 * kG) {
-      if (it + kG < total) load(it + kG, rb);
-      store(it, ra);
-      if (it + kG < total) {
-        if (it + 2 * kG < total) load(it + 2 * kG, ra);
-        store(it + kG, rb);
+    if (nmine > 0) load(ra);
+    for (int i = 0; i < nmine; i += 2) {
+      if (i + 1 < nmine) load(rb);
+      store(ra);
+      if (i + 1 < nmine) {
+        if (i + 2 < nmine) load(ra);
+        store(rb);
       }
     }
   }
