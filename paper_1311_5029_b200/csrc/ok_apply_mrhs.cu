@@ -395,14 +395,19 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
       if (st >= kARing) { st -= kARing; eph ^= 1u; }
     };
 
-    float4 ra[3], rb[3];
+    float4 ra[3], rb[3], rc[3];   // two stages of gathers in flight behind the one being converted
     if (nmine > 0) load(ra);
-    for (int i = 0; i < nmine; i += 2) {
-      if (i + 1 < nmine) load(rb);
+    if (nmine > 1) load(rb);
+    for (int i = 0; i < nmine; i += 3) {
+      if (i + 2 < nmine) load(rc);
       store(ra);
       if (i + 1 < nmine) {
-        if (i + 2 < nmine) load(ra);
+        if (i + 3 < nmine) load(ra);
         store(rb);
+      }
+      if (i + 2 < nmine) {
+        if (i + 4 < nmine) load(rb);
+        store(rc);
       }
     }
   }
