@@ -361,12 +361,17 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
       if (a.mrhs) {   // split-fp16 B-operand tile of ok_apply_mrhs.cu (ok_internal.cuh: mrhs_W_index); fp64 -> fp32 -> (hi, lo)
         __half* tile = reinterpret_cast<__half*>(W) + (size_t)n * kMrhsWSiteHalves;
 #pragma unroll
-        for (int col = 0; col < 12; ++col) {
-          mrhs_split((float)row[col].x, &tile[mrhs_W_index(term, r, col, 0, 0)], &tile[mrhs_W_index(term, r, col, 0, 1)]);
-          mrhs_split((float)row[col].y, &tile[mrhs_W_index(term, r, col, 1, 0)], &tile[mrhs_W_index(term, r, col, 1, 1)]);
-        }
+        for (int j = 0; j < 3; ++j)   // columns 4j..4j+3 are 4 consecutive k: one 8-byte store per (part, piece)
+#pragma unroll
+          for (int part = 0; part < 2; ++part) {
+            __half hi[4], lo[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) mrhs_split((float)(part ? row[4 * j + i].y : row[4 * j + i].x), &hi[i], &lo[i]);
+            *reinterpret_cast<uint2*>(&tile[mrhs_W_index(term, r, 4 * j, part, 0)]) = *reinterpret_cast<const uint2*>(hi);
+            *reinterpret_cast<uint2*>(&tile[mrhs_W_index(term, r, 4 * j, part, 1)]) = *reinterpret_cast<const uint2*>(lo);
+          }
         if (term == 0)   // zero pad k = 36..39 of the last stage: 192 halves per site, 16 per row r
-          for (int q = 0; q < 16; ++q) tile[mrhs_W_pad_index(16 * r + q)] = __float2half_rn(0.f);
+          for (int q = 0; q < 4; ++q) *reinterpret_cast<uint2*>(&tile[mrhs_W_pad_index(16 * r + 4 * q)]) = make_uint2(0u, 0u);
         continue;
       }
 #pragma unroll
