@@ -1,0 +1,125 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs[2], configs[3]):
+20^3 x 64, fp32, the same seeded links (eps = 0.25) and sources as the bench workloads.
+
+The oracle cannot apply the operator to 512 000 sites in seconds, so the CUDA result is compared on SAMPLED
+sites that the oracle computes one by one (Oracle.precalc_W(idx) / apply_W(psi, idx=idx), Eq. (2.2),
+PAPER.md:53-55): lattice corners and faces (every wrap-around of the stencil, the antiperiodic time
+boundary, the last ragged 32-site block) plus evenly spaced and pseudo-random interior sites.
+BiCGStab is checked through a property that holds at any size: the residual b - M x,
+evaluated by the ORACLE on the sampled sites, extrapolates to a relative residual of the order of tol.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle.ok_oracle import Oracle
+from paper_1311_5029_b200 import binding as B
+from paper_1311_5029_b200 import inputs as I
+import okgpu as G
+
+pytestmark = pytest.mark.gpu
+
+DIMS = (20, 20, 20, 64)
+FP32_TOL = 2e-5
+NR = 12
+
+
+def sample_sites(dims, n_even=384, n_rand=384, seed=11):
+    Lx, Ly, Lz, T = dims
+    V = Lx * Ly * Lz * T
+
+    def site(x, y, z, t):
+        return x + Lx * (y + Ly * (z + Lz * t))
+
+    s = set()
+    for x in (0, 1, Lx - 2, Lx - 1):
+        for y in (0, 1, Ly - 2, Ly - 1):
+            for z in (0, 1, Lz - 2, Lz - 1):
+                for t in (0, 1, T - 2, T - 1):
+                    s.add(site(x, y, z, t))
+    s.update(range(V - 40, V))                                   # the tail of the site order
+    s.update((np.arange(n_even) * (V // n_even) + 7).tolist())   # evenly spread
+    s.update(np.random.default_rng(seed).integers(0, V, n_rand).tolist())
+    return np.array(sorted(s), dtype=np.int64)
+
+
+@pytest.fixture(scope="module")
+def big():
+    out = {}
+    for seed in (5, 7):                                          # configs[2] and configs[3] gauge seeds
+        U = I.near_identity_links(DIMS, 0.25, seed)
+        pd = I.make_params(DIMS, 0.10, I.tadpole_u0(I.mean_plaquette(DIMS, U)))
+        out[seed] = (U, pd, Oracle(U, pd))
+    return out
+
+
+def sampled_rel_l2(got, want):
+    return float(np.linalg.norm(got - want) / np.linalg.norm(want))
+
+
+def test_fullsize_single_rhs_apply_and_solve(big):
+    U, pd, o = big[5]
+    p = B.make_params(pd, B.OK_FP32)
+    idx = sample_sites(DIMS)
+    W = G.precalc(p, U)
+    # W on the sampled sites, element by element (fp32 rounding of the fp64 precalc)
+    want_W = o.precalc_W(idx)
+    canon = torch.empty((o.V, 27, 12, 12), dtype=torch.complex64, device=G.DEV)
+    B.ok_unpack_W(W, canon)
+    got_W = canon[torch.from_numpy(idx).to(G.DEV)].cpu().numpy().astype(np.complex128)
+    del canon
+    assert np.abs(got_W - want_W).max() <= 2e-7 * np.abs(want_W).max()
+    # apply: Gaussian source seed 6 (the bench workload)
+    psi = I.gaussian_spinor(DIMS, 6)
+    got = G.apply(p, W, psi)[idx]
+    want = o.apply_W(psi, idx=idx, W=want_W)
+    assert sampled_rel_l2(got, want) <= FP32_TOL
+    assert G.per_site_rel_err(got, want) <= 10 * FP32_TOL          # fp32: every sampled site individually close
+    # solve to 1e-6; the oracle evaluates the residual on the sampled sites
+    G.workspace(p)
+    src = G.pack_spinor(p, psi)
+    x = B.alloc_vec(p)
+    tol = 1e-6
+    st, it, res = B.ok_bicgstab(W, src, x, tol, 2000, raise_on_fail=False)
+    assert st == 0 and res <= tol and 10 <= it <= 200
+    xs = G.unpack_spinor(p, x, psi.shape)
+    r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
+    est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
+    assert est <= 5 * tol, est
+
+
+def test_fullsize_12rhs_apply_and_solve(big):
+    U, pd, o = big[7]
+    p = B.make_params(pd, B.OK_FP32, nrhs=NR)
+    idx = sample_sites(DIMS, n_even=192, n_rand=192)
+    W = G.precalc(p, U)
+    want_W = o.precalc_W(idx)
+    # Gaussian block: every site of the sample is exercised
+    psi = np.stack([I.gaussian_spinor(DIMS, 60 + j) for j in range(NR)], axis=2)
+    got = G.apply(p, W, psi)[idx]
+    want = o.apply_W(psi, idx=idx, W=want_W)
+    num = np.linalg.norm((got - want).reshape(-1, NR), axis=0)
+    den = np.linalg.norm(want.reshape(-1, NR), axis=0)
+    assert float((num / den).max()) <= FP32_TOL
+    del psi, got
+    # configs[3]: the 12 point sources at the origin
+    b = np.stack([I.point_source(DIMS, site=0, comp=j) for j in range(NR)], axis=2)
+    G.workspace(p)
+    src = G.pack_spinor(p, b)
+    x = B.alloc_vec(p)
+    tol = 1e-6
+    st, it, res = B.ok_bicgstab(W, src, x, tol, 2000, raise_on_fail=False)
+    assert st == 0 and res <= tol and 10 <= it <= 200
+    xs = G.unpack_spinor(p, x, b.shape)
+    # residual by the oracle: exactly on the origin's neighbourhood (where b lives and r is largest), and on a uniform
+    # random sample of the remaining sites, extrapolated to the whole lattice
+    rng = range(-3, 4)
+    near = np.unique(np.concatenate([o.sh(np.array([0]), np.array(off)) for off in
+                                     [(dx, dy, dz, dt) for dx in rng for dy in rng for dz in rng for dt in rng]]))
+    rn = b[near] - o.apply_W(xs, idx=near)
+    far = np.setdiff1d(np.random.default_rng(3).integers(0, o.V, 768), near)
+    rf = b[far] - o.apply_W(xs, idx=far)
+    n2 = np.linalg.norm(rn.reshape(-1, NR), axis=0) ** 2
+    f2 = (o.V - len(near)) / len(far) * np.linalg.norm(rf.reshape(-1, NR), axis=0) ** 2
+    est = np.sqrt(n2 + f2)                                                   # ||b_j|| = 1
+    assert est.max() <= 3 * tol, est
