@@ -42,7 +42,11 @@
  *                                                 fp64: c = 0..11, (re,im) of component c
  *   W       1024-byte header, then [block][term][row 0..11][c][site_in_block][16 bytes]
  *           with c pairing the COLUMNS of W exactly as the spinor pairs components.
- *   nrhs=12 spinor: [block][component 0..11][site_in_block][rhs 0..11][re,im] (fp32 only).
+ *   OK_W_BLOCK / OK_W_DS: header, then [block][unit][site_in_block][complex]; the unit order is the list of
+ *           stored colour-block rows in csrc/ok_sparse.cuh.  ok_pack_W drops what the format does not keep
+ *           (OK_W_DS keeps UL (else LR) as D and UR as S); ok_unpack_W rebuilds the full 12 x 12 matrices.
+ *   nrhs=12 (fp32, OK_W_DENSE only): spinor = per-site records [component/4][2*rhs+part][component%4] (1152 B);
+ *           W = per-site split-fp16 tensor-core tiles (31 488 B), see csrc/ok_internal.cuh.
  *   Use ok_pack_ and ok_unpack_ to convert; the sizes are given by ok_vec_bytes and ok_W_bytes.
  */
 #ifndef OK_H_
@@ -57,6 +61,14 @@ extern "C" {
 
 #define OK_FP32 0
 #define OK_FP64 1
+
+/* W storage formats (ok_params.storage).  All three hold the same operator, Eq. (2.2); the reduced ones
+ * exploit the fixed structure of the 27 matrices, W = [[UL,UR],[LL,LR]] over upper/lower spin with
+ * UL, LR in {0, D}, UR = S, LL = +-S (Eqs. 2.6-2.12) and fixed zero colour blocks
+ * (172 of the 432 per site).  nrhs = 12 supports OK_W_DENSE only. */
+#define OK_W_DENSE 0        /* 27 x 12 x 12 complex per site: 31 104 B (fp32)                              */
+#define OK_W_BLOCK 1        /* the 260 non-zero colour blocks, each quadrant on its own: 18 720 B (fp32)   */
+#define OK_W_DS 2           /* D and S once per term (132 colour blocks): 9 504 B (fp32)                   */
 
 #define OK_NTERMS 27        /* PAPER.md:53-55 */
 #define OK_SITE_BLOCK 32
@@ -79,6 +91,8 @@ typedef struct ok_params {
   double kappa, u0;   /* hopping parameter, tadpole factor (Eq. 2.6)                           */
   double zeta, rs;    /* Eqs. (2.6)-(2.8)                                                      */
   double cB, cE, cEE, c1, c2, c3, c4, c5;
+  int32_t storage;    /* OK_W_DENSE / OK_W_BLOCK / OK_W_DS: how W is held in device memory            */
+  int32_t reserved_;  /* 0                                                                            */
 } ok_params;
 
 /* ---- sizes (pure host arithmetic; 0 on invalid params) ---------------------------------- */

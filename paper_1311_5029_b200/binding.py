@@ -10,6 +10,7 @@ import ctypes as C
 import os
 
 OK_FP32, OK_FP64 = 0, 1
+OK_W_DENSE, OK_W_BLOCK, OK_W_DS = 0, 1, 2
 OK_NTERMS = 27
 OK_W_HEADER_BYTES = 1024
 
@@ -27,7 +28,8 @@ class ok_params(C.Structure):
     _fields_ = [("dims", C.c_int32 * 4), ("precision", C.c_int32), ("bc", C.c_int32 * 4), ("nrhs", C.c_int32),
                 ("kappa", C.c_double), ("u0", C.c_double), ("zeta", C.c_double), ("rs", C.c_double),
                 ("cB", C.c_double), ("cE", C.c_double), ("cEE", C.c_double), ("c1", C.c_double),
-                ("c2", C.c_double), ("c3", C.c_double), ("c4", C.c_double), ("c5", C.c_double)]
+                ("c2", C.c_double), ("c3", C.c_double), ("c4", C.c_double), ("c5", C.c_double),
+                ("storage", C.c_int32), ("reserved_", C.c_int32)]
 
 
 EXPORTS = {
@@ -86,9 +88,10 @@ def _check(status, where):
         raise OkError(status, where)
 
 
-def make_params(p: dict, precision: int, nrhs: int = 1) -> ok_params:
+def make_params(p: dict, precision: int, nrhs: int = 1, storage: int = 0) -> ok_params:
     """dict (inputs.make_params) -> C struct."""
     q = ok_params()
+    q.storage, q.reserved_ = storage, 0
     q.dims[:] = list(p["dims"])
     q.bc[:] = list(p["bc"])
     q.precision, q.nrhs = precision, nrhs

@@ -5,6 +5,7 @@
 #include <unordered_map>
 
 #include "ok_internal.cuh"
+#include "ok_sparse.cuh"
 
 namespace okd {
 
@@ -27,6 +28,11 @@ int fail_cuda(cudaError_t e, const char* where) {
   return OK_ECUDA;
 }
 
+static uint32_t layout_id(const ok_params* p) {
+  if (p->nrhs == 12) return kLayoutMrhs;
+  return p->storage == OK_W_BLOCK ? kLayoutBlock : p->storage == OK_W_DS ? kLayoutDS : kLayoutDense;
+}
+
 bool valid_params(const ok_params* p) {
   if (!p) return false;
   long long V = 1;
@@ -39,6 +45,8 @@ bool valid_params(const ok_params* p) {
   if (p->precision != OK_FP32 && p->precision != OK_FP64) return false;
   if (p->nrhs != 1 && p->nrhs != 12) return false;
   if (p->nrhs == 12 && p->precision != OK_FP32) return false;
+  if (p->storage != OK_W_DENSE && p->storage != OK_W_BLOCK && p->storage != OK_W_DS) return false;
+  if (p->nrhs == 12 && p->storage != OK_W_DENSE) return false;
   if (!(p->kappa > 0.0) || !(p->u0 > 0.0)) return false;
   return true;
 }
@@ -77,7 +85,7 @@ int lookup_W(const void* W, ok_params* p) {
   OK_CUDA(cudaMemcpyAsync(&h, W, sizeof(h), cudaMemcpyDeviceToHost, ctx().stream));
   OK_CUDA(cudaStreamSynchronize(ctx().stream));
   if (h.magic != kMagic || !valid_params(&h.p)) return OK_EINVAL;
-  if (h.layout != (h.p.nrhs == 12 ? kLayoutMrhs : kLayoutDense)) return OK_EINVAL;
+  if (h.layout != layout_id(&h.p)) return OK_EINVAL;
   remember_W(W, &h.p);
   *p = h.p;
   return OK_SUCCESS;
@@ -90,7 +98,7 @@ static int write_header(void* W, const ok_params* p) {
   memset(buf, 0, sizeof(buf));
   WHeader h;
   h.magic = kMagic;
-  h.layout = p->nrhs == 12 ? kLayoutMrhs : kLayoutDense;
+  h.layout = layout_id(p);
   h.p = *p;
   memcpy(buf, &h, sizeof(h));
   OK_CUDA(cudaMemcpyAsync(W, buf, sizeof(buf), cudaMemcpyHostToDevice, ctx().stream));
@@ -113,6 +121,8 @@ size_t ok_W_bytes(const ok_params* p) {
   if (!valid_params(p)) return 0;
   Geom g = make_geom(p);
   if (p->nrhs == 12) return OK_W_HEADER_BYTES + (size_t)g.V * kMrhsWSiteBytes;
+  if (p->storage != OK_W_DENSE)
+    return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * sparse_site_units(p->storage) * 2 * real_bytes(p);
   return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * kTerms * 144 * 2 * real_bytes(p);
 }
 

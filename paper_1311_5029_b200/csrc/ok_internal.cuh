@@ -14,6 +14,8 @@ constexpr int kBlock = OK_SITE_BLOCK;   // sites per block (= warp width: lane <
 constexpr int kTerms = OK_NTERMS;
 constexpr uint32_t kMagic = 0x4F4B5731u;   // "OKW1"
 constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
+constexpr uint32_t kLayoutBlock = 4;       // OK_W_BLOCK: [block][unit 2340][site][complex]   (ok_sparse.cuh)
+constexpr uint32_t kLayoutDS = 5;          // OK_W_DS:    [block][unit 1188][site][complex]
 constexpr uint32_t kLayoutMrhs = 3;        // nrhs = 12: per-site tcgen05 operand tiles, split fp16 (ok_apply_mrhs.cu)
 
 // ---- nrhs = 12 (tensor-core) layouts, fp32 fields (ok_apply_mrhs.cu) -------------------------------
@@ -129,6 +131,7 @@ int launch_pack_W(const ok_params* p, const void* canon, void* Wpayload, bool un
 int launch_apply(const ok_params* p, const void* Wpayload, const void* psi, void* out,
                  double* dot_partials /* nullable */, const void* dot_a, const void* dot_b);
 int launch_precalc(const ok_params* p, const void* links, void* Wpayload, void* work);
+int launch_apply_sparse(const ok_params* p, const void* Wpayload, const void* psi, void* out, double* dot_partials, const void* dot_a);
 size_t precalc_work_bytes(const ok_params* p);
 int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
                  int* iters, double* resid);

@@ -1,6 +1,7 @@
 // Layout conversion kernels: canonical (ok.h) <-> site-blocked SoA internal layouts.
 // One thread moves one 16-byte unit; the internal side is always the coalesced one.
 #include "ok_internal.cuh"
+#include "ok_sparse.cuh"
 
 namespace okd {
 
@@ -116,8 +117,55 @@ __global__ void pack_W_kernel(const vec_t* __restrict__ canon, vec_t* __restrict
   }
 }
 
+// Reduced formats (ok_sparse.cuh): canonical [n][27][12][12] <-> [block][unit][site 32][complex].  One thread per canonical
+// element of a (padded) site.  Packing drops what the format does not keep (structural zeros; for OK_W_DS the implied
+// quadrants LR, LL); unpacking rebuilds the full matrices (zeros, copies, LL = -S of W^0).
+__constant__ int c_prun[2][kTerms][2][4];
+static bool g_prun_ready = false;
+
+template <typename cx>
+__global__ void pack_W_sparse_kernel(const cx* __restrict__ canon, cx* __restrict__ packed, int V, int nblk, int fmt, bool unpack) {
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = (long long)nblk * kBlock * kTerms * 144;
+  if (e >= total) return;
+  const int col = (int)(e % 12), row = (int)((e / 12) % 12), term = (int)((e / 144) % kTerms);
+  const long long n = e / (144 * kTerms);
+  const SparseRef r = sparse_ref(fmt, term, row, col, c_prun[fmt - 1]);
+  cx* dst = r.unit < 0 ? nullptr : packed + ((size_t)(n >> 5) * sparse_site_units(fmt) + r.unit) * kBlock + (n & 31);
+  if (unpack) {
+    if (n >= V) return;
+    cx v = {};
+    if (dst) { v = *dst; v.x *= r.sign; v.y *= r.sign; }
+    const_cast<cx*>(canon)[e] = v;
+  } else if (dst && r.stored) {
+    cx v = {};
+    if (n < V) v = canon[e];
+    *dst = v;
+  }
+}
+
+static int launch_pack_W_sparse(const ok_params* p, const void* canon, void* Wp, bool unpack) {
+  if (!g_prun_ready) {
+    static int h[2][kTerms][2][4];
+    sparse_fill_runs(OK_W_BLOCK, h[0]);
+    sparse_fill_runs(OK_W_DS, h[1]);
+    OK_CUDA(cudaMemcpyToSymbol(c_prun, h, sizeof(h)));
+    g_prun_ready = true;
+  }
+  Geom g = make_geom(p);
+  const long long total = (long long)g.nblk * kBlock * kTerms * 144;
+  const unsigned grid = (unsigned)((total + 255) / 256);
+  if (p->precision == OK_FP64)
+    pack_W_sparse_kernel<double2><<<grid, 256, 0, ctx().stream>>>(static_cast<const double2*>(canon), static_cast<double2*>(Wp), g.V, g.nblk, p->storage, unpack);
+  else
+    pack_W_sparse_kernel<float2><<<grid, 256, 0, ctx().stream>>>(static_cast<const float2*>(canon), static_cast<float2*>(Wp), g.V, g.nblk, p->storage, unpack);
+  OK_LAUNCHED("pack_W_sparse_kernel");
+  return OK_SUCCESS;
+}
+
 int launch_pack_W(const ok_params* p, const void* canon, void* Wp, bool unpack) {
   Geom g = make_geom(p);
+  if (p->nrhs == 1 && p->storage != OK_W_DENSE) return launch_pack_W_sparse(p, canon, Wp, unpack);
   if (p->nrhs == 12) {
     long long tot = (long long)g.V * (kTerms * 144 + 192);
     pack_W_mrhs_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx().stream>>>(static_cast<const float2*>(canon),

@@ -20,6 +20,7 @@
 // Boundary conditions: U_mu(x) is multiplied by bc[mu] on the last slice of axis mu at load
 // time (DESIGN.md R-BC); closed loops are unaffected, every hop across the boundary gets one sign.
 #include "ok_internal.cuh"
+#include "ok_sparse.cuh"
 
 namespace okd {
 
@@ -32,6 +33,7 @@ struct PrecalcArgs {
   int bc[4];
   int Vpad;
   int mrhs;                    // 1: write the nrhs = 12 tensor-core tile layout (ok_internal.cuh)
+  int storage;                 // OK_W_DENSE / OK_W_BLOCK / OK_W_DS (ok_sparse.cuh)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
   double s4;                   // c_EE / (2 u0^4)      (Eq. 2.7)
@@ -41,6 +43,7 @@ struct PrecalcArgs {
 };
 
 __constant__ int8_t c_poff[kTerms][4];
+__constant__ int c_qrun[2][kTerms][2][4];   // run offsets of the reduced formats (ok_sparse.cuh)
 static bool g_poff_uploaded = false;
 
 // ------------------------------------------------------------------------- complex 3x3 algebra
@@ -286,8 +289,8 @@ __device__ __forceinline__ double2 pauli_entry(const P4& P, int al, int be, int 
 }
 
 template <typename real> struct WUnit;
-template <> struct WUnit<float> { using type = float4; static constexpr int NC = 6; };
-template <> struct WUnit<double> { using type = double2; static constexpr int NC = 12; };
+template <> struct WUnit<float> { using type = float4; using cx = float2; static constexpr int NC = 6; };
+template <> struct WUnit<double> { using type = double2; using cx = double2; static constexpr int NC = 12; };
 
 template <typename real>
 __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
@@ -300,6 +303,16 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
   const int n = blk * kBlock + lane;
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
   if (a.mrhs && n >= a.g.V) return;   // the tile layout has no padded sites
+  if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units this term keeps
+    using cx = typename WUnit<real>::cx;
+    cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units(a.storage) * kBlock + lane;
+    for (int r = 0; r < 12; ++r)
+      for (int col = 0; col < 12; ++col) {
+        const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
+        if (ref.unit >= 0 && ref.stored) Ws[(size_t)ref.unit * kBlock] = cx{};
+      }
+    return;
+  }
   if (n >= a.g.V) {   // padded site: zeros
     unit_t z = {};
     for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
@@ -356,6 +369,21 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
       }
       row[col] = v;
     }
+    if (a.storage != OK_W_DENSE) {   // reduced formats: keep only what the format stores (rounded once, like the dense W)
+      using cx = typename WUnit<real>::cx;
+      cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units(a.storage) * kBlock + lane;
+#pragma unroll
+      for (int col = 0; col < 12; ++col) {
+        const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
+        if (ref.unit >= 0 && ref.stored) {
+          cx v;
+          v.x = (real)row[col].x;
+          v.y = (real)row[col].y;
+          Ws[(size_t)ref.unit * kBlock] = v;
+        }
+      }
+      continue;
+    }
     unit_t* dst = Wt + (size_t)r * NC * kBlock;
     if constexpr (sizeof(real) == 4) {
       if (a.mrhs) {   // split-fp16 B-operand tile of ok_apply_mrhs.cu (ok_internal.cuh: mrhs_W_index); fp64 -> fp32 -> (hi, lo)
@@ -392,6 +420,10 @@ size_t precalc_work_bytes(const ok_params* p) {
 int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) {
   if (!g_poff_uploaded) {
     OK_CUDA(cudaMemcpyToSymbol(c_poff, kOffsets, sizeof(kOffsets)));
+    static int h[2][kTerms][2][4];
+    sparse_fill_runs(OK_W_BLOCK, h[0]);
+    sparse_fill_runs(OK_W_DS, h[1]);
+    OK_CUDA(cudaMemcpyToSymbol(c_qrun, h, sizeof(h)));
     g_poff_uploaded = true;
   }
   PrecalcArgs a;
@@ -399,6 +431,7 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   for (int d = 0; d < 4; ++d) a.bc[d] = p->bc[d];
   a.Vpad = a.g.nblk * kBlock;
   a.mrhs = p->nrhs == 12;
+  a.storage = p->storage;
   const double u0 = p->u0, u2 = u0 * u0, u3 = u2 * u0, u4 = u2 * u2;
   a.mass = u0 / (2.0 * p->kappa);
   a.d0 = -(p->cB * p->zeta + 16.0 * p->c5) / (2.0 * u3);

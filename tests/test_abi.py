@@ -35,8 +35,9 @@ def test_every_declared_symbol_is_exported_and_bound(lib):
 
 
 def test_struct_layout_matches_header():
-    # 10 int32 + 12 double, no padding surprises: 40 + 96 = 136 bytes
-    assert C.sizeof(B.ok_params) == 136
+    # 10 int32 + 12 double + storage, reserved_ (2 int32), no padding surprises: 40 + 96 + 8 = 144 bytes
+    assert C.sizeof(B.ok_params) == 144
+    assert B.ok_params.storage.offset == 136
 
 
 def test_sizes(lib):
@@ -52,6 +53,12 @@ def test_sizes(lib):
     assert B.ok_work_bytes(pr) > 0
     pm = B.make_params(I.make_params((4, 4, 4, 8), 0.1, 0.95), B.OK_FP32, nrhs=12)
     assert B.ok_vec_bytes(pm) == 512 * 12 * 12 * 8
+    # reduced storage formats: 260 resp. 132 colour blocks of 9 complex per site
+    pb = B.make_params(I.make_params((20, 20, 20, 64), 0.1, 0.95), B.OK_FP32, storage=B.OK_W_BLOCK)
+    assert B.ok_W_bytes(pb) == 1024 + V * 260 * 9 * 8            # 18 720 B/site
+    pds = B.make_params(I.make_params((20, 20, 20, 64), 0.1, 0.95), B.OK_FP32, storage=B.OK_W_DS)
+    assert B.ok_W_bytes(pds) == 1024 + V * 132 * 9 * 8           # 9 504 B/site
+    assert B.ok_W_bytes(B.make_params(I.make_params((4, 4, 4, 8), 0.1, 0.95), B.OK_FP32, nrhs=12, storage=B.OK_W_DS)) == 0
 
 
 def test_invalid_params_rejected(lib):
