@@ -56,15 +56,22 @@ WORKLOADS = {
     "4x4x4x8-fp32-rhs12": ((4, 4, 4, 8), 4, 0.25, 7, None, 0.10, 1e-6),     # quick check of the 12-RHS mode
 }
 NRHS = {"20x20x20x64-fp32-rhs12": 12, "4x4x4x8-fp32-rhs12": 12}
+# reduced W storage: same lattice, links, source as configs[2]
+WORKLOADS["20x20x20x64-fp32-block"] = WORKLOADS["20x20x20x64-fp32"]
+WORKLOADS["20x20x20x64-fp32-ds"] = WORKLOADS["20x20x20x64-fp32"]
+WORKLOADS["20x20x20x64-fp64-ds"] = WORKLOADS["20x20x20x64-fp64"]
+WORKLOADS["32x32x32x64-fp32-ds"] = WORKLOADS["32x32x32x64-fp32"]
+STORAGE = {"20x20x20x64-fp32-block": 1, "20x20x20x64-fp32-ds": 2, "20x20x20x64-fp64-ds": 2, "32x32x32x64-fp32-ds": 2}
+W_COMPLEX_PER_SITE = {0: 27 * 144, 1: 260 * 9, 2: 132 * 9}
 
 
 def make_links(dims, eps, lseed):
     return I.haar_links(dims, lseed) if eps is None else I.near_identity_links(dims, eps, lseed)
 
 
-def alg_bytes_per_site(sbytes, nrhs):
-    """W once + the spinor block read once + written once."""
-    return 27 * 144 * 2 * sbytes + 2 * 24 * sbytes * nrhs
+def alg_bytes_per_site(sbytes, nrhs, storage=0):
+    """W once (in its storage format) + the spinor block read once + written once."""
+    return W_COMPLEX_PER_SITE[storage] * 2 * sbytes + 2 * 24 * sbytes * nrhs
 
 
 def fallback_peaks():
@@ -229,7 +236,8 @@ def run_ours(args, wl):
     U = make_links(dims, eps, lseed)
     plaq = I.mean_plaquette(dims, U)
     pd = I.make_params(dims, kappa, I.tadpole_u0(plaq))
-    p = B.make_params(pd, prec, nrhs=nrhs)
+    storage = STORAGE.get(wl, 0)
+    p = B.make_params(pd, prec, nrhs=nrhs, storage=storage)
     V = int(np.prod(dims))
     cdt = torch.complex64 if sbytes == 4 else torch.complex128
     if nrhs == 1:
@@ -308,7 +316,7 @@ def run_ours(args, wl):
     # ---- max over ranks
     a_ms = float(np.mean(apply_ms))
     total_ms, a_ms, e2e_ms, s_s = max_over_ranks([total_ms, a_ms, e2e_ms, float(np.mean(solve_s))], dist, dev)
-    alg = V * alg_bytes_per_site(sbytes, nrhs)
+    alg = V * alg_bytes_per_site(sbytes, nrhs, storage)
     value = aggregate_value(world, alg, a_ms)
     peaks = measured_peaks()
 
@@ -327,7 +335,7 @@ def run_ours(args, wl):
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if sbytes == 4 else "f64", "data": "synthetic",
-            "config": {"workload": wl, "nrhs": nrhs, "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
+            "config": {"workload": wl, "nrhs": nrhs, "storage": ["dense", "block (260 colour blocks)", "ds (132 colour blocks)"][storage], "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
                        "sites": V, "l2_flush": "not needed: W (%.1f GB) >> L2 (126 MB)" % (B.ok_W_bytes(p) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "plaquette": plaq, "u0": pd["u0"]},
             "pct_of_peak": {"measured_copy": 100 * value / world / peaks["hbm_gbs"], "nominal_8000": 100 * value / world / 8000.0},
@@ -335,7 +343,7 @@ def run_ours(args, wl):
             "gflops": world * V * FLOP_PER_SITE * nrhs / (a_ms * 1e-3) / 1e9,
             "bicgstab_solve_s": s_s, "bicgstab_iters": int(np.max(iters_l)), "bicgstab_true_resid": float(np.max(resid_l)),
             "precalc_ms": float(np.mean(pre_ms)),
-            "roofline": {"bound": "hbm", "kernel": KERNEL_NAME[(sbytes, nrhs)], "achieved": alg / (a_ms * 1e-3) / 1e9,
+            "roofline": {"bound": "hbm", "kernel": KERNEL_NAME[(sbytes, nrhs)] if storage == 0 else "okd::apply_sparse_kernel<%s,%d>" % ("float" if sbytes == 4 else "double", storage), "achieved": alg / (a_ms * 1e-3) / 1e9,
                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": alg / (a_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                          "peak_source": peaks["_source"], "algorithmic_bytes_per_launch": alg, "traffic": traffic},
             "e2e": {"value": world * alg / (e2e_ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_apply": e2e_ms,
