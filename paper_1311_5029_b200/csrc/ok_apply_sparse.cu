@@ -107,12 +107,13 @@ __device__ __forceinline__ void term_body(int term, const SiteCtx<real>& c, cons
   const int* ro = c_srun[FMT - 1][term][c.a];
   cx w[3][2][3];
   if constexpr (FMT == OK_W_DS) {
-    if constexpr (MD != 0) {
-      load_rows<MD>(w, Wb + (size_t)ro[0] * kBlock);
-      if constexpr (UL) rows_times<real, MD>(acc_u, w, s, c.a, real(1));
-      if constexpr (LR) rows_times<real, MD>(acc_l, w, s + 6, c.a, real(1));
-    }
+    cx wd[3][2][3];
+    if constexpr (MD != 0) load_rows<MD>(wd, Wb + (size_t)ro[0] * kBlock);   // both runs in flight before the first use
     load_rows<MS>(w, Wb + (size_t)ro[1] * kBlock);
+    if constexpr (MD != 0) {
+      if constexpr (UL) rows_times<real, MD>(acc_u, wd, s, c.a, real(1));
+      if constexpr (LR) rows_times<real, MD>(acc_l, wd, s + 6, c.a, real(1));
+    }
     rows_times<real, MS>(acc_u, w, s + 6, c.a, real(1));
     rows_times<real, MS>(acc_l, w, s, c.a, NEG ? real(-1) : real(1));
   } else {
