@@ -13,6 +13,8 @@ What it computes, and the passage each function follows:
   apply_W            sum_y M_xy psi_y in collected form                     PAPER.md:53-55, Eq. (2.2)
   apply_direct       the same operator as raw gauge-link products           DESIGN.md R-DIRECT (the paper's "Naive")
   bicgstab           bi-stabilised CG, textbook van der Vorst               PAPER.md:114 ; DESIGN.md R-SOLVER
+  bicgstab_mixed     mixed-precision inversion: defect correction around    PAPER.md:114 ("mixed precision inversion by calling
+                     a low-precision bicgstab                               the inverter ... in single or double precision") ; R-MIXED
   dense_M            brute-force matrix of M (tiny lattices only)           PAPER.md:43-47, Eq. (2.1)
 
 Pins (tests/test_oracle_*.py, all -m "not gpu"): direct == W form (P1); free-field closed
@@ -389,7 +391,8 @@ def bicgstab(apply, b, tol, maxit):
 
     Returns (x, iters, true_relative_residual, status); status 0 ok, -3 breakdown, -4 maxit.
     """
-    dot = lambda a, c: np.vdot(a, c)
+    # reductions and scalars in fp64 whatever the storage precision of the vectors (R-SOLVER); vectors keep b's dtype
+    dot = lambda a, c: complex(np.vdot(a.astype(np.complex128, copy=False), c.astype(np.complex128, copy=False)))
     bnorm = np.sqrt(dot(b, b).real)
     x = np.zeros_like(b)
     if bnorm == 0.0:
@@ -437,3 +440,40 @@ def bicgstab(apply, b, tol, maxit):
         p = r + beta * (p - omega * v)
     rtrue = b - apply(x)
     return x, it, float(np.sqrt(dot(rtrue, rtrue).real) / bnorm), status
+
+
+def bicgstab_mixed(apply_hi, apply_lo, b, tol, inner_tol, maxit, max_outer=50, lo_dtype=np.complex64):
+    """R-MIXED.  PAPER.md:114 only says that a mixed precision inversion is done "by calling the QOPQDP inverter or
+    Dirac operation module in single or double precision, as appropriate".  Reading: classical defect correction
+    (iterative refinement) around the low-precision inverter,
+
+        x = 0 ; r = b                                   (high precision)
+        repeat:  stop when ||r|| <= tol ||b||
+                 e  = bicgstab(M_lo, r / ||r|| rounded to low precision, inner_tol)    (the inverter, low precision)
+                 x += ||r|| e ;  r = b - M_hi x                                        (the Dirac module, high precision)
+
+    apply_hi / apply_lo: the operator in the two precisions.  `maxit` bounds the TOTAL number of inner iterations.
+    Returns (x, inner_iters_total, outer_iters, true_relative_residual, status)."""
+    nrm = lambda a: float(np.sqrt(np.vdot(a, a).real))
+    bnorm = nrm(b)
+    x = np.zeros_like(b)
+    if bnorm == 0.0:
+        return x, 0, 0, 0.0, 0
+    r = b.copy()
+    total, outer, status = 0, 0, -4
+    while True:
+        rn = nrm(r)
+        if rn <= tol * bnorm:
+            status = 0
+            break
+        if outer >= max_outer or total >= maxit:
+            break
+        e, it, _, st = bicgstab(apply_lo, (r / rn).astype(lo_dtype), inner_tol, maxit - total)
+        total += it
+        outer += 1
+        if st == -3:
+            status = -3
+            break
+        x = x + rn * e.astype(b.dtype)
+        r = b - apply_hi(x)
+    return x, total, outer, nrm(b - apply_hi(x)) / bnorm, status

@@ -382,3 +382,33 @@ def test_bicgstab_textbook_small_matrix():
     # exact-arithmetic property: at most n iterations; breakdown code on a singular start
     x, it, res, st = oo.bicgstab(lambda v: 0 * v, b, 1e-12, 5)
     assert st == -3
+
+
+# ----------------------------------------------------------------------------- P8 mixed-precision inversion (R-MIXED)
+def test_P8_mixed_precision_vs_dense_LU_2p4():
+    """Defect correction around a complex64 BiCGStab reaches the fp64 solution of the dense matrix (LU), the inner
+    solver alone cannot; the number of outer corrections follows from the contraction factor inner_tol per correction."""
+    dims = (2, 2, 2, 2)
+    U = I.near_identity_links(dims, 0.3, 1)
+    o = Oracle(U, I.make_params(dims, 0.10, I.tadpole_u0(I.mean_plaquette(dims, U))))
+    M = o.dense_M()
+    b = I.gaussian_spinor(dims, 2)
+    W = o.precalc_W()
+    W32 = W.astype(np.complex64)
+    hi = lambda v: o.apply_W(v, W=W)
+    lo = lambda v: np.einsum("ntij,tnj->ni", W32, np.stack([v[o.sh(np.arange(o.V), off)] for off in oo.OFFSETS])).astype(np.complex64)
+    xs = np.linalg.solve(M, b.reshape(-1)).reshape(b.shape)
+    x, its, outer, res, st = oo.bicgstab_mixed(hi, lo, b, 1e-12, 1e-4, 1000)
+    assert st == 0 and res <= 1e-12 and rel(x, xs) < 1e-11
+    assert 3 <= outer <= 5                       # 1e-12 at 1e-4 (or better) per correction
+    # the low-precision inverter on its own stalls at single-precision level
+    x32, it32, res32, st32 = oo.bicgstab(lo, b.astype(np.complex64), 1e-12, 300)
+    assert rel(x32.astype(np.complex128), xs) > 1e-8
+    # exact low-precision operator (lo == hi): one correction of accuracy inner_tol per outer step
+    x, its, outer, res, st = oo.bicgstab_mixed(hi, hi, b, 1e-9, 1e-3, 1000, lo_dtype=np.complex128)
+    assert st == 0 and outer == 3 and rel(x, xs) < 1e-8
+    # zero right-hand side, and the iteration budget
+    x, its, outer, res, st = oo.bicgstab_mixed(hi, lo, 0 * b, 1e-12, 1e-4, 1000)
+    assert st == 0 and its == 0 and outer == 0 and np.all(x == 0)
+    x, its, outer, res, st = oo.bicgstab_mixed(hi, lo, b, 1e-12, 1e-4, 5)
+    assert st == -4 and its == 5 and res > 1e-12
