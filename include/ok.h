@@ -132,6 +132,19 @@ int ok_dirac_apply(const void* W, const void* psi, void* out);
  * *resid = max over columns.  iters/resid: HOST pointers.  Needs the workspace. */
 int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, int* iters, double* resid);
 
+/* Mixed-precision inversion, PAPER.md:114 ("We perform a mixed precision inversion by calling the ... inverter or
+ * Dirac operation module in single or double precision, as appropriate"): defect correction around the fp32
+ * BiCGStab with both sets of precalculation matrices resident,
+ *     x = 0, r = src;  repeat { stop if ||r|| <= tol ||src|| ;  e = ok_bicgstab(W32, r/||r|| in fp32, inner_tol) ;
+ *                               x += ||r|| e ;  r = src - M x with W64 }.
+ * W64: fp64 W, W32: fp32 W of the same lattice (any storage format each); src, x: fp64 internal spinor layout.
+ * maxit bounds the total number of fp32 BiCGStab iterations, max_outer the corrections.  *iters = total inner
+ * iterations, *outer = corrections done, *resid = fp64 true relative residual.  iters/outer/resid: HOST pointers.
+ * Needs a workspace of ok_mixed_work_bytes(p) bytes (p: the parameters of either W).  Synchronises the stream. */
+size_t ok_mixed_work_bytes(const ok_params* p);
+int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x, double tol, double inner_tol,
+                      int maxit, int max_outer, int* iters, int* outer, double* resid);
+
 /* Same apply with HOST spinors in the canonical layout (precision of W): copies psi to the
  * device, packs, applies, unpacks and copies back, synchronising the stream.  W stays
  * device-resident across calls (the paper keeps the precalculation matrices on the GPU and

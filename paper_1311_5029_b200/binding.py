@@ -48,6 +48,9 @@ EXPORTS = {
     "ok_bicgstab": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int,
                               C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_dirac_apply_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_mixed_work_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
+    "ok_bicgstab_mixed": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int,
+                                    C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_W_params": (C.c_int, [C.c_void_p, C.POINTER(ok_params)]),
     "ok_forget_W": (C.c_int, [C.c_void_p]),
     "ok_launch_count": (C.c_uint64, []),
@@ -170,6 +173,20 @@ def ok_bicgstab(W, src, x, tol, maxit, raise_on_fail=True):
     if st != 0 and raise_on_fail:
         raise OkError(st, "ok_bicgstab")
     return st, it.value, res.value
+
+
+def ok_mixed_work_bytes(p):
+    return lib().ok_mixed_work_bytes(C.byref(p))
+
+
+def ok_bicgstab_mixed(W64, W32, src, x, tol, inner_tol, maxit, max_outer=50, raise_on_fail=True):
+    """Returns (status, inner_iters_total, outer_corrections, true_relative_residual)."""
+    it, outer, res = C.c_int(0), C.c_int(0), C.c_double(0.0)
+    st = lib().ok_bicgstab_mixed(_ptr(W64), _ptr(W32), _ptr(src), _ptr(x), float(tol), float(inner_tol), int(maxit), int(max_outer),
+                                 C.byref(it), C.byref(outer), C.byref(res))
+    if st != 0 and raise_on_fail:
+        raise OkError(st, "ok_bicgstab_mixed")
+    return st, it.value, outer.value, res.value
 
 
 def ok_W_params(W):

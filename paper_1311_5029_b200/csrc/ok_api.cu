@@ -242,6 +242,27 @@ int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, 
   return run_bicgstab(&p, W_payload(W), src, x, tol, maxit, iters, resid);
 }
 
+size_t ok_mixed_work_bytes(const ok_params* p) {
+  if (!valid_params(p) || p->nrhs != 1) return 0;
+  return mixed_work_bytes(p) + 4096;
+}
+
+int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x, double tol, double inner_tol, int maxit,
+                      int max_outer, int* iters, int* outer, double* resid) {
+  if (!aligned16(src) || !aligned16(x) || src == x || !iters || !outer || !resid || !(tol > 0.0) || !(inner_tol > 0.0) || !(inner_tol < 1.0) ||
+      maxit < 1 || max_outer < 1)
+    return OK_EINVAL;
+  ok_params p64, p32;
+  int st = lookup_W(W64, &p64);
+  if (st) return st;
+  if ((st = lookup_W(W32, &p32))) return st;
+  if (p64.precision != OK_FP64 || p32.precision != OK_FP32 || p64.nrhs != 1 || p32.nrhs != 1) return OK_EINVAL;
+  for (int d = 0; d < 4; ++d)
+    if (p64.dims[d] != p32.dims[d]) return OK_EINVAL;
+  if (!ctx().work || ctx().work_bytes < mixed_work_bytes(&p64)) return OK_EWORKSPACE;
+  return run_bicgstab_mixed(&p64, W_payload(W64), &p32, W_payload(W32), src, x, tol, inner_tol, maxit, max_outer, iters, outer, resid);
+}
+
 const char* ok_strerror(int status) {
   switch (status) {
     case OK_SUCCESS: return "success";

@@ -136,6 +136,10 @@ size_t precalc_work_bytes(const ok_params* p);
 int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
                  int* iters, double* resid);
 size_t bicgstab_work_bytes(const ok_params* p);
+// mixed precision (ok_mixed.cu)
+size_t mixed_work_bytes(const ok_params* p);
+int run_bicgstab_mixed(const ok_params* p64, const void* W64payload, const ok_params* p32, const void* W32payload, const void* src, void* x,
+                       double tol, double inner_tol, int maxit, int max_outer, int* iters, int* outer, double* resid);
 // nrhs = 12
 int launch_apply_mrhs(const ok_params* p, const void* Wpayload, const void* psi, void* out);
 int run_bicgstab_mrhs(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
