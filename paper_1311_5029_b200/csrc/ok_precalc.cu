@@ -372,14 +372,31 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
     if (a.storage != OK_W_DENSE) {   // reduced formats: keep only what the format stores (rounded once, like the dense W)
       using cx = typename WUnit<real>::cx;
       cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units(a.storage) * kBlock + lane;
+      const TermDesc d = term_desc(term);
+      const int hr = r / 6, sa = (r % 6) / 3, cr = r % 3;
 #pragma unroll
-      for (int col = 0; col < 12; ++col) {
-        const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
-        if (ref.unit >= 0 && ref.stored) {
-          cx v;
-          v.x = (real)row[col].x;
-          v.y = (real)row[col].y;
-          Ws[(size_t)ref.unit * kBlock] = v;
+      for (int hc = 0; hc < 2; ++hc) {
+        const int quad = 2 * hr + hc;
+        const bool diag = hr == hc;
+        if (diag && !(quad == 0 ? d.ul : d.lr)) continue;
+        int m = quad;
+        if (a.storage == OK_W_DS) {
+          if (!(diag ? (quad == 0 || !d.ul) : quad == 1)) continue;   // LR = D and LL = +-S are implied
+          m = diag ? 0 : 1;
+        }
+        const int mr = mask_row(diag ? d.maskD : d.maskS, sa), nb = popc2(mr);
+        cx* run = Ws + (size_t)(c_qrun[a.storage - 1][term][sa][m] + cr * nb * 3) * kBlock;
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+          if (!((mr >> b) & 1)) continue;
+          const int bc = (b == 1 && (mr & 1)) ? 1 : 0;
+#pragma unroll
+          for (int cc = 0; cc < 3; ++cc) {
+            cx v;
+            v.x = (real)row[6 * hc + 3 * b + cc].x;
+            v.y = (real)row[6 * hc + 3 * b + cc].y;
+            run[(size_t)(bc * 3 + cc) * kBlock] = v;
+          }
         }
       }
       continue;
