@@ -69,6 +69,9 @@ extern "C" {
 #define OK_W_DENSE 0        /* 27 x 12 x 12 complex per site: 31 104 B (fp32)                              */
 #define OK_W_BLOCK 1        /* the 260 non-zero colour blocks, each quadrant on its own: 18 720 B (fp32)   */
 #define OK_W_DS 2           /* D and S once per term (132 colour blocks): 9 504 B (fp32)                   */
+#define OK_W_CONJ 3         /* OK_W_DS for W^0 and the 13 positive-direction terms only (70 colour blocks,  */
+                            /* 5 040 B fp32); the opposite-direction matrices are rebuilt from the          */
+                            /* neighbour site by the conjugation relations, Eqs. (2.3), (2.10) */
 
 #define OK_NTERMS 27
 #define OK_SITE_BLOCK 32

@@ -30,7 +30,7 @@ int fail_cuda(cudaError_t e, const char* where) {
 
 static uint32_t layout_id(const ok_params* p) {
   if (p->nrhs == 12) return kLayoutMrhs;
-  return p->storage == OK_W_BLOCK ? kLayoutBlock : p->storage == OK_W_DS ? kLayoutDS : kLayoutDense;
+  return p->storage == OK_W_BLOCK ? kLayoutBlock : p->storage == OK_W_DS ? kLayoutDS : p->storage == OK_W_CONJ ? kLayoutConj : kLayoutDense;
 }
 
 bool valid_params(const ok_params* p) {
@@ -45,7 +45,7 @@ bool valid_params(const ok_params* p) {
   if (p->precision != OK_FP32 && p->precision != OK_FP64) return false;
   if (p->nrhs != 1 && p->nrhs != 12) return false;
   if (p->nrhs == 12 && p->precision != OK_FP32) return false;
-  if (p->storage != OK_W_DENSE && p->storage != OK_W_BLOCK && p->storage != OK_W_DS) return false;
+  if (p->storage < OK_W_DENSE || p->storage > OK_W_CONJ) return false;
   if (p->nrhs == 12 && p->storage != OK_W_DENSE) return false;
   if (!(p->kappa > 0.0) || !(p->u0 > 0.0)) return false;
   return true;
@@ -122,7 +122,7 @@ size_t ok_W_bytes(const ok_params* p) {
   Geom g = make_geom(p);
   if (p->nrhs == 12) return OK_W_HEADER_BYTES + (size_t)g.V * kMrhsWSiteBytes;
   if (p->storage != OK_W_DENSE)
-    return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * sparse_site_units(p->storage) * 2 * real_bytes(p);
+    return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * sparse_site_units_rt(p->storage) * 2 * real_bytes(p);
   return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * kTerms * 144 * 2 * real_bytes(p);
 }
 

@@ -15,7 +15,7 @@
 namespace okd {
 
 __constant__ int8_t c_soff[kTerms][4];
-__constant__ int c_srun[2][kTerms][2][4];   // [format - 1][term][a][m] -> first complex unit of the run
+__constant__ int c_srun[3][kTerms][2][4];   // [format - 1][term][a][m] -> first complex unit of the run
 static bool g_sparse_ready = false;
 
 namespace {
@@ -69,6 +69,26 @@ __device__ __forceinline__ void load_rows(cx (&w)[3][2][3], const cx* run) {
       for (int cc = 0; cc < 3; ++cc) w[cr][j][cc] = __ldcs(run + (size_t)((cr * nb + j) * 3 + cc) * kBlock);
 }
 
+// OK_W_CONJ, opposite-direction term: rows a of M^dag from the partner's matrix M at the neighbour site,
+//   (M^dag)[a,cr][b,cc] = conj(M[b,cc][a,cr]) ; M[b,.][a,.] sits in the run of spin row b at (cc * nb + jj) * 3 + cr
+template <int MASK, typename cx>
+__device__ __forceinline__ void load_rows_conj(cx (&w)[3][2][3], const cx* Wn, const int (*runs)[4], int m, int a) {
+  constexpr int nb = NB<MASK>::v;
+  const int jj = MASK == kMaskFull ? a : 0;
+#pragma unroll
+  for (int j = 0; j < nb; ++j) {
+    const cx* run = Wn + (size_t)runs[spin_col<MASK>(a, j)][m] * kBlock;
+#pragma unroll
+    for (int cr = 0; cr < 3; ++cr)
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc) {
+        cx v = __ldg(run + (size_t)((cc * nb + jj) * 3 + cr) * kBlock);
+        v.y = -v.y;
+        w[cr][j][cc] = v;
+      }
+  }
+}
+
 }  // namespace
 
 namespace {
@@ -80,8 +100,8 @@ struct SiteCtx {
 };
 
 // one stencil term whose zero pattern is (MD, UL, LR, MS) and whose LL = -S when NEG
-template <typename real, int FMT, int MD, int UL, int LR, int MS, int NEG>
-__device__ __forceinline__ void term_body(int term, const SiteCtx<real>& c, const typename SV<real>::cx* __restrict__ Wb,
+template <typename real, int FMT, int MD, int UL, int LR, int MS, int NEG, int CONJ = 0>
+__device__ __forceinline__ void term_body(int term, const SiteCtx<real>& c, const typename SV<real>::cx* __restrict__ W0, const typename SV<real>::cx* __restrict__ Wb,
                                           const typename SV<real>::vec* __restrict__ psi, real (&acc_u)[3][2], real (&acc_l)[3][2]) {
   using cx = typename SV<real>::cx;
   using vec = typename SV<real>::vec;
@@ -106,7 +126,20 @@ __device__ __forceinline__ void term_body(int term, const SiteCtx<real>& c, cons
   }
   const int* ro = c_srun[FMT - 1][term][c.a];
   cx w[3][2][3];
-  if constexpr (FMT == OK_W_DS) {
+  if constexpr (CONJ) {
+    // W_term(x) = [[D^dag, -S^dag], [-S^dag, D^dag]] of the partner term at the neighbour site nn (the site psi comes from too)
+    const cx* Wn = W0 + (size_t)(nn >> 5) * sparse_site_units(FMT) * kBlock + (nn & 31);
+    const int (*runs)[4] = c_srun[FMT - 1][term];
+    cx wd[3][2][3];
+    if constexpr (MD != 0) load_rows_conj<MD>(wd, Wn, runs, 0, c.a);
+    load_rows_conj<MS>(w, Wn, runs, 1, c.a);
+    if constexpr (MD != 0) {
+      if constexpr (UL) rows_times<real, MD>(acc_u, wd, s, c.a, real(1));
+      if constexpr (LR) rows_times<real, MD>(acc_l, wd, s + 6, c.a, real(1));
+    }
+    rows_times<real, MS>(acc_u, w, s + 6, c.a, real(-1));
+    rows_times<real, MS>(acc_l, w, s, c.a, real(-1));
+  } else if constexpr (FMT != OK_W_BLOCK) {
     cx wd[3][2][3];
     if constexpr (MD != 0) load_rows<MD>(wd, Wb + (size_t)ro[0] * kBlock);   // both runs in flight before the first use
     load_rows<MS>(w, Wb + (size_t)ro[1] * kBlock);
@@ -161,20 +194,28 @@ apply_sparse_kernel(const typename SV<real>::cx* __restrict__ W, const typename 
 
   const cx* Wb = W + (size_t)blk * sparse_site_units(FMT) * kBlock + c.lane;
 
-  // term classes (ok_sparse.cuh: term_desc): the loops run over terms of one zero pattern
-  term_body<real, FMT, kMaskFull, 1, 1, kMaskFull, 1>(0, c, Wb, psi, acc_u, acc_l);
+  // term classes (ok_sparse.cuh: term_desc): the loops run over terms of one zero pattern; OK_W_CONJ takes the even
+  // (opposite-direction) terms from the partner matrix of the neighbour site
+  constexpr int CJ = FMT == OK_W_CONJ ? 1 : 0;
+#define OK_TERM(MD, UL, LR, MS, NEG, o) term_body<real, FMT, MD, UL, LR, MS, NEG, 0>(o, c, W, Wb, psi, acc_u, acc_l)
+#define OK_TERM_PAIR(MD, UL, LR, MS, o)                                                                      \
+  if (CJ && !((o) & 1)) term_body<real, FMT, MD, UL, LR, MS, 0, CJ>(o, c, W, Wb, psi, acc_u, acc_l);        \
+  else term_body<real, FMT, MD, UL, LR, MS, 0, 0>(o, c, W, Wb, psi, acc_u, acc_l)
+  OK_TERM(kMaskFull, 1, 1, kMaskFull, 1, 0);
 #pragma unroll 1
-  for (int o = 1; o <= 6; ++o) term_body<real, FMT, kMaskFull, 1, 1, kMaskFull, 0>(o, c, Wb, psi, acc_u, acc_l);
-  term_body<real, FMT, kMaskDiag, 0, 1, kMaskFull, 0>(7, c, Wb, psi, acc_u, acc_l);
-  term_body<real, FMT, kMaskDiag, 1, 0, kMaskFull, 0>(8, c, Wb, psi, acc_u, acc_l);
+  for (int o = 1; o <= 6; ++o) { OK_TERM_PAIR(kMaskFull, 1, 1, kMaskFull, o); }
+  OK_TERM(kMaskDiag, 0, 1, kMaskFull, 0, 7);
+  term_body<real, FMT, kMaskDiag, 1, 0, kMaskFull, 0, CJ>(8, c, W, Wb, psi, acc_u, acc_l);
 #pragma unroll 1
-  for (int o = 9; o <= 12; ++o) term_body<real, FMT, kMaskDiag, 1, 1, kMaskOff, 0>(o, c, Wb, psi, acc_u, acc_l);
+  for (int o = 9; o <= 12; ++o) { OK_TERM_PAIR(kMaskDiag, 1, 1, kMaskOff, o); }
 #pragma unroll 1
-  for (int o = 13; o <= 14; ++o) term_body<real, FMT, kMaskDiag, 1, 1, kMaskDiag, 0>(o, c, Wb, psi, acc_u, acc_l);
+  for (int o = 13; o <= 14; ++o) { OK_TERM_PAIR(kMaskDiag, 1, 1, kMaskDiag, o); }
 #pragma unroll 1
-  for (int o = 15; o <= 18; ++o) term_body<real, FMT, 0, 0, 0, kMaskOff, 0>(o, c, Wb, psi, acc_u, acc_l);
+  for (int o = 15; o <= 18; ++o) { OK_TERM_PAIR(0, 0, 0, kMaskOff, o); }
 #pragma unroll 1
-  for (int o = 19; o <= 26; ++o) term_body<real, FMT, 0, 0, 0, kMaskFull, 0>(o, c, Wb, psi, acc_u, acc_l);
+  for (int o = 19; o <= 26; ++o) { OK_TERM_PAIR(0, 0, 0, kMaskFull, o); }
+#undef OK_TERM
+#undef OK_TERM_PAIR
 
   // store: row -> (unit, sub) of the internal spinor layout
   real* ob = reinterpret_cast<real*>(out + (size_t)blk * NC * kBlock);
@@ -241,21 +282,21 @@ static int launch_sparse(const Geom& g, const void* W, const void* psi, void* ou
 }
 
 int launch_apply_sparse(const ok_params* p, const void* W, const void* psi, void* out, double* partials, const void* dot_a) {
-  if (p->nrhs != 1 || (p->storage != OK_W_BLOCK && p->storage != OK_W_DS)) return OK_EINVAL;
+  if (p->nrhs != 1 || p->storage < OK_W_BLOCK || p->storage > OK_W_CONJ) return OK_EINVAL;
   if (!g_sparse_ready) {
-    static int h_run[2][kTerms][2][4];
-    for (int f = 0; f < 2; ++f)
-      for (int t = 0; t < kTerms; ++t)
-        for (int a = 0; a < 2; ++a)
-          for (int m = 0; m < 4; ++m) h_run[f][t][a][m] = m < sparse_nmat(f + 1) ? sparse_run_offset(f + 1, t, a, m) : 0;
+    static int h_run[3][kTerms][2][4];
+    for (int f = 0; f < 3; ++f) sparse_fill_runs(f + 1, h_run[f]);
     OK_CUDA(cudaMemcpyToSymbol(c_srun, h_run, sizeof(h_run)));
     OK_CUDA(cudaMemcpyToSymbol(c_soff, kOffsets, sizeof(kOffsets)));
     g_sparse_ready = true;
   }
   Geom g = make_geom(p);
-  const bool f64 = p->precision == OK_FP64, ds = p->storage == OK_W_DS;
-  if (f64) return ds ? launch_sparse<double, OK_W_DS>(g, W, psi, out, partials, dot_a) : launch_sparse<double, OK_W_BLOCK>(g, W, psi, out, partials, dot_a);
-  return ds ? launch_sparse<float, OK_W_DS>(g, W, psi, out, partials, dot_a) : launch_sparse<float, OK_W_BLOCK>(g, W, psi, out, partials, dot_a);
+  const bool f64 = p->precision == OK_FP64;
+  switch (p->storage) {
+    case OK_W_BLOCK: return f64 ? launch_sparse<double, OK_W_BLOCK>(g, W, psi, out, partials, dot_a) : launch_sparse<float, OK_W_BLOCK>(g, W, psi, out, partials, dot_a);
+    case OK_W_DS: return f64 ? launch_sparse<double, OK_W_DS>(g, W, psi, out, partials, dot_a) : launch_sparse<float, OK_W_DS>(g, W, psi, out, partials, dot_a);
+    default: return f64 ? launch_sparse<double, OK_W_CONJ>(g, W, psi, out, partials, dot_a) : launch_sparse<float, OK_W_CONJ>(g, W, psi, out, partials, dot_a);
+  }
 }
 
 }  // namespace okd

@@ -15,6 +15,7 @@ constexpr int kTerms = OK_NTERMS;
 constexpr uint32_t kMagic = 0x4F4B5731u;   // "OKW1"
 constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
 constexpr uint32_t kLayoutBlock = 4;       // OK_W_BLOCK: [block][unit 2340][site][complex]   (ok_sparse.cuh)
+constexpr uint32_t kLayoutConj = 6;        // OK_W_CONJ:  [block][unit 630][site][complex]
 constexpr uint32_t kLayoutDS = 5;          // OK_W_DS:    [block][unit 1188][site][complex]
 constexpr uint32_t kLayoutMrhs = 3;        // nrhs = 12: per-site tcgen05 operand tiles, split fp16 (ok_apply_mrhs.cu)
 

@@ -120,22 +120,31 @@ __global__ void pack_W_kernel(const vec_t* __restrict__ canon, vec_t* __restrict
 // Reduced formats (ok_sparse.cuh): canonical [n][27][12][12] <-> [block][unit][site 32][complex].  One thread per canonical
 // element of a (padded) site.  Packing drops what the format does not keep (structural zeros; for OK_W_DS the implied
 // quadrants LR, LL); unpacking rebuilds the full matrices (zeros, copies, LL = -S of W^0).
-__constant__ int c_prun[2][kTerms][2][4];
+__constant__ int c_prun[3][kTerms][2][4];
+__constant__ int8_t c_pkoff[kTerms][4];
 static bool g_prun_ready = false;
 
 template <typename cx>
-__global__ void pack_W_sparse_kernel(const cx* __restrict__ canon, cx* __restrict__ packed, int V, int nblk, int fmt, bool unpack) {
+__global__ void pack_W_sparse_kernel(const cx* __restrict__ canon, cx* __restrict__ packed, int V, int nblk, int fmt, bool unpack, Geom g) {
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long total = (long long)nblk * kBlock * kTerms * 144;
   if (e >= total) return;
   const int col = (int)(e % 12), row = (int)((e / 12) % 12), term = (int)((e / 144) % kTerms);
   const long long n = e / (144 * kTerms);
   const SparseRef r = sparse_ref(fmt, term, row, col, c_prun[fmt - 1]);
-  cx* dst = r.unit < 0 ? nullptr : packed + ((size_t)(n >> 5) * sparse_site_units(fmt) + r.unit) * kBlock + (n & 31);
+  long long ns = n;   // site that holds the stored value
+  if (r.shift >= 0 && n < V) {   // OK_W_CONJ: the positive matrix of the neighbour site x + offset[term]
+    int xc[4], q = (int)n;
+    for (int dd = 0; dd < 3; ++dd) { xc[dd] = q % g.L[dd]; q /= g.L[dd]; }
+    xc[3] = q;
+    for (int dd = 0; dd < 4; ++dd) xc[dd] = (xc[dd] + c_pkoff[r.shift][dd] + g.L[dd]) % g.L[dd];
+    ns = xc[0] + g.L[0] * (xc[1] + g.L[1] * (xc[2] + (long long)g.L[2] * xc[3]));
+  }
+  cx* dst = r.unit < 0 ? nullptr : packed + ((size_t)(ns >> 5) * sparse_site_units_rt(fmt) + r.unit) * kBlock + (ns & 31);
   if (unpack) {
     if (n >= V) return;
     cx v = {};
-    if (dst) { v = *dst; v.x *= r.sign; v.y *= r.sign; }
+    if (dst) { v = *dst; v.x *= r.sign; v.y *= r.conj ? -r.sign : r.sign; }
     const_cast<cx*>(canon)[e] = v;
   } else if (dst && r.stored) {
     cx v = {};
@@ -146,19 +155,19 @@ __global__ void pack_W_sparse_kernel(const cx* __restrict__ canon, cx* __restric
 
 static int launch_pack_W_sparse(const ok_params* p, const void* canon, void* Wp, bool unpack) {
   if (!g_prun_ready) {
-    static int h[2][kTerms][2][4];
-    sparse_fill_runs(OK_W_BLOCK, h[0]);
-    sparse_fill_runs(OK_W_DS, h[1]);
+    static int h[3][kTerms][2][4];
+    for (int f = 0; f < 3; ++f) sparse_fill_runs(f + 1, h[f]);
     OK_CUDA(cudaMemcpyToSymbol(c_prun, h, sizeof(h)));
+    OK_CUDA(cudaMemcpyToSymbol(c_pkoff, kOffsets, sizeof(kOffsets)));
     g_prun_ready = true;
   }
   Geom g = make_geom(p);
   const long long total = (long long)g.nblk * kBlock * kTerms * 144;
   const unsigned grid = (unsigned)((total + 255) / 256);
   if (p->precision == OK_FP64)
-    pack_W_sparse_kernel<double2><<<grid, 256, 0, ctx().stream>>>(static_cast<const double2*>(canon), static_cast<double2*>(Wp), g.V, g.nblk, p->storage, unpack);
+    pack_W_sparse_kernel<double2><<<grid, 256, 0, ctx().stream>>>(static_cast<const double2*>(canon), static_cast<double2*>(Wp), g.V, g.nblk, p->storage, unpack, g);
   else
-    pack_W_sparse_kernel<float2><<<grid, 256, 0, ctx().stream>>>(static_cast<const float2*>(canon), static_cast<float2*>(Wp), g.V, g.nblk, p->storage, unpack);
+    pack_W_sparse_kernel<float2><<<grid, 256, 0, ctx().stream>>>(static_cast<const float2*>(canon), static_cast<float2*>(Wp), g.V, g.nblk, p->storage, unpack, g);
   OK_LAUNCHED("pack_W_sparse_kernel");
   return OK_SUCCESS;
 }

@@ -43,7 +43,7 @@ struct PrecalcArgs {
 };
 
 __constant__ int8_t c_poff[kTerms][4];
-__constant__ int c_qrun[2][kTerms][2][4];   // run offsets of the reduced formats (ok_sparse.cuh)
+__constant__ int c_qrun[3][kTerms][2][4];   // run offsets of the reduced formats (ok_sparse.cuh)
 static bool g_poff_uploaded = false;
 
 // ------------------------------------------------------------------------- complex 3x3 algebra
@@ -303,9 +303,10 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
   const int n = blk * kBlock + lane;
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
   if (a.mrhs && n >= a.g.V) return;   // the tile layout has no padded sites
+  if (a.storage == OK_W_CONJ && term_is_neg(term)) return;   // rebuilt at apply time from term - 1 of the neighbour site
   if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units this term keeps
     using cx = typename WUnit<real>::cx;
-    cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units(a.storage) * kBlock + lane;
+    cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units_rt(a.storage) * kBlock + lane;
     for (int r = 0; r < 12; ++r)
       for (int col = 0; col < 12; ++col) {
         const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
@@ -371,7 +372,7 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
     }
     if (a.storage != OK_W_DENSE) {   // reduced formats: keep only what the format stores (rounded once, like the dense W)
       using cx = typename WUnit<real>::cx;
-      cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units(a.storage) * kBlock + lane;
+      cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units_rt(a.storage) * kBlock + lane;
       const TermDesc d = term_desc(term);
       const int hr = r / 6, sa = (r % 6) / 3, cr = r % 3;
 #pragma unroll
@@ -380,7 +381,7 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
         const bool diag = hr == hc;
         if (diag && !(quad == 0 ? d.ul : d.lr)) continue;
         int m = quad;
-        if (a.storage == OK_W_DS) {
+        if (a.storage != OK_W_BLOCK) {
           if (!(diag ? (quad == 0 || !d.ul) : quad == 1)) continue;   // LR = D and LL = +-S are implied
           m = diag ? 0 : 1;
         }
@@ -437,9 +438,8 @@ size_t precalc_work_bytes(const ok_params* p) {
 int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) {
   if (!g_poff_uploaded) {
     OK_CUDA(cudaMemcpyToSymbol(c_poff, kOffsets, sizeof(kOffsets)));
-    static int h[2][kTerms][2][4];
-    sparse_fill_runs(OK_W_BLOCK, h[0]);
-    sparse_fill_runs(OK_W_DS, h[1]);
+    static int h[3][kTerms][2][4];
+    for (int f = 0; f < 3; ++f) sparse_fill_runs(f + 1, h[f]);
     OK_CUDA(cudaMemcpyToSymbol(c_qrun, h, sizeof(h)));
     g_poff_uploaded = true;
   }

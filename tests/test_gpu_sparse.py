@@ -1,7 +1,9 @@
 """Parity of the reduced W storage formats with the CPU oracle.
 
 OK_W_BLOCK keeps the 260 structurally non-zero colour blocks of a site (432 blocks, 172 vanish),
-OK_W_DS keeps D and S of W = [[D, S], [+-S, D]] once per term (Eqs. 2.6-2.12).  Both hold the same
+OK_W_DS keeps D and S of W = [[D, S], [+-S, D]] once per term (Eqs. 2.6-2.12), OK_W_CONJ keeps them for
+W^0 and the positive-direction terms only and rebuilds the opposite directions from the neighbour site by the conjugation
+relations (Eqs. 2.3, 2.10; the paper's own compression).  All hold the same
 operator as the dense Eq. (2.2) form, so the oracle side is unchanged: Oracle.precalc_W / apply_W / bicgstab.
 Tolerances as for the dense path (fp64 per-site 1e-12, fp32 relative L2 2e-5, iterations +-2).
 """
@@ -20,8 +22,8 @@ pytestmark = pytest.mark.gpu
 FP64_TOL = 1e-12
 FP32_TOL = 2e-5
 SHAPES = [(4, 3, 3, 2), (2, 2, 2, 2), (4, 4, 4, 8), (5, 2, 3, 4)]
-FORMATS = [B.OK_W_BLOCK, B.OK_W_DS]
-BLOCKS = {B.OK_W_BLOCK: 260, B.OK_W_DS: 132}
+FORMATS = [B.OK_W_BLOCK, B.OK_W_DS, B.OK_W_CONJ]
+BLOCKS = {B.OK_W_BLOCK: 260, B.OK_W_DS: 132, B.OK_W_CONJ: 70}
 
 
 def setup(dims, eps=0.3, seed=1, kappa=0.10, bc=(1, 1, 1, -1), haar=False):
@@ -87,6 +89,18 @@ def test_block_format_keeps_any_matrix_with_the_zero_pattern(fmt):
             if has_ul and has_lr:
                 want[:, t, 6:, 6:] = ul
             want[:, t, 6:, :6] = -ur if t == 0 else ur
+        if fmt == B.OK_W_CONJ:      # W^-_o(x) = [[D^dag, -S^dag], [-S^dag, D^dag]] of W^+_o(x - o), quadrant presence of term t
+            for t in range(2, 27, 2):
+                src = want[o.sh(np.arange(V), oo.OFFSETS[t]), t - 1]
+                D = src[:, :6, :6] if pattern[t - 1, :6, :6].any() else src[:, 6:, 6:]
+                Dd, Sd = np.conj(np.swapaxes(D, 1, 2)), np.conj(np.swapaxes(src[:, :6, 6:], 1, 2))
+                want[:, t] = 0
+                if pattern[t, :6, :6].any():
+                    want[:, t, :6, :6] = Dd
+                if pattern[t, 6:, 6:].any():
+                    want[:, t, 6:, 6:] = Dd
+                want[:, t, :6, 6:] = -Sd
+                want[:, t, 6:, :6] = -Sd
         assert np.array_equal(back, want)
     psi = I.gaussian_spinor(dims, 3)
     got = G.apply(p, W, psi)
