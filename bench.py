@@ -61,8 +61,10 @@ WORKLOADS["20x20x20x64-fp32-block"] = WORKLOADS["20x20x20x64-fp32"]
 WORKLOADS["20x20x20x64-fp32-ds"] = WORKLOADS["20x20x20x64-fp32"]
 WORKLOADS["20x20x20x64-fp64-ds"] = WORKLOADS["20x20x20x64-fp64"]
 WORKLOADS["32x32x32x64-fp32-ds"] = WORKLOADS["32x32x32x64-fp32"]
-STORAGE = {"20x20x20x64-fp32-block": 1, "20x20x20x64-fp32-ds": 2, "20x20x20x64-fp64-ds": 2, "32x32x32x64-fp32-ds": 2}
-W_COMPLEX_PER_SITE = {0: 27 * 144, 1: 260 * 9, 2: 132 * 9}
+WORKLOADS["20x20x20x64-fp32-conj"] = WORKLOADS["20x20x20x64-fp32"]
+WORKLOADS["20x20x20x64-fp64-conj"] = WORKLOADS["20x20x20x64-fp64"]
+STORAGE = {"20x20x20x64-fp32-conj": 3, "20x20x20x64-fp64-conj": 3, "20x20x20x64-fp32-block": 1, "20x20x20x64-fp32-ds": 2, "20x20x20x64-fp64-ds": 2, "32x32x32x64-fp32-ds": 2}
+W_COMPLEX_PER_SITE = {0: 27 * 144, 1: 260 * 9, 2: 132 * 9, 3: 70 * 9}
 
 
 def make_links(dims, eps, lseed):
@@ -357,7 +359,7 @@ def run_ours(args, wl):
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if sbytes == 4 else "f64", "data": "synthetic",
-            "config": {"workload": wl, "nrhs": nrhs, "storage": ["dense", "block (260 colour blocks)", "ds (132 colour blocks)"][storage], "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
+            "config": {"workload": wl, "nrhs": nrhs, "storage": ["dense", "block (260 colour blocks)", "ds (132 colour blocks)", "conj (70 colour blocks)"][storage], "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
                        "sites": V, "l2_flush": "not needed: W (%.1f GB) >> L2 (126 MB)" % (B.ok_W_bytes(p) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "plaquette": plaq, "u0": pd["u0"]},
             "pct_of_peak": {"measured_copy": 100 * value / world / peaks["hbm_gbs"], "nominal_8000": 100 * value / world / 8000.0},

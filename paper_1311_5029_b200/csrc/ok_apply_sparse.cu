@@ -58,7 +58,9 @@ __device__ __forceinline__ void rows_times(real (&acc)[3][2], const cx (&w)[3][2
   }
 }
 
-template <int MASK, typename cx>
+// STREAM: evict-first loads (W is read once); OK_W_CONJ reads every stored matrix twice (own site, neighbour's partner
+// term) and wants the second read served by L2, so it loads with the default policy
+template <int MASK, bool STREAM = true, typename cx>
 __device__ __forceinline__ void load_rows(cx (&w)[3][2][3], const cx* run) {
   constexpr int nb = NB<MASK>::v;
 #pragma unroll
@@ -66,7 +68,10 @@ __device__ __forceinline__ void load_rows(cx (&w)[3][2][3], const cx* run) {
 #pragma unroll
     for (int j = 0; j < nb; ++j)
 #pragma unroll
-      for (int cc = 0; cc < 3; ++cc) w[cr][j][cc] = __ldcs(run + (size_t)((cr * nb + j) * 3 + cc) * kBlock);
+      for (int cc = 0; cc < 3; ++cc) {
+        const cx* q = run + (size_t)((cr * nb + j) * 3 + cc) * kBlock;
+        w[cr][j][cc] = STREAM ? __ldcs(q) : __ldg(q);
+      }
 }
 
 // OK_W_CONJ, opposite-direction term: rows a of M^dag from the partner's matrix M at the neighbour site,
@@ -141,8 +146,9 @@ __device__ __forceinline__ void term_body(int term, const SiteCtx<real>& c, cons
     rows_times<real, MS>(acc_l, w, s, c.a, real(-1));
   } else if constexpr (FMT != OK_W_BLOCK) {
     cx wd[3][2][3];
-    if constexpr (MD != 0) load_rows<MD>(wd, Wb + (size_t)ro[0] * kBlock);   // both runs in flight before the first use
-    load_rows<MS>(w, Wb + (size_t)ro[1] * kBlock);
+    constexpr bool ST = FMT != OK_W_CONJ;
+    if constexpr (MD != 0) load_rows<MD, ST>(wd, Wb + (size_t)ro[0] * kBlock);   // both runs in flight before the first use
+    load_rows<MS, ST>(w, Wb + (size_t)ro[1] * kBlock);
     if constexpr (MD != 0) {
       if constexpr (UL) rows_times<real, MD>(acc_u, wd, s, c.a, real(1));
       if constexpr (LR) rows_times<real, MD>(acc_l, wd, s + 6, c.a, real(1));
