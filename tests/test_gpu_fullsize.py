@@ -123,3 +123,36 @@ def test_fullsize_12rhs_apply_and_solve(big):
     f2 = (o.V - len(near)) / len(far) * np.linalg.norm(rf.reshape(-1, NR), axis=0) ** 2
     est = np.sqrt(n2 + f2)                                                   # ||b_j|| = 1
     assert est.max() <= 3 * tol, est
+
+
+@pytest.mark.parametrize("fmt", [B.OK_W_DS, B.OK_W_CONJ])
+def test_fullsize_reduced_formats_apply_and_mixed_solve(big, fmt):
+    """The reduced W storage formats and the mixed-precision inversion (item 3) at the
+    bench size: sampled-site parity of the fp32 apply, then ok_bicgstab_mixed(W64, W32) to 1e-10 with the residual
+    evaluated by the oracle (fp64) on sampled sites."""
+    U, pd, o = big[5]
+    idx = sample_sites(DIMS)
+    want_W = o.precalc_W(idx)
+    p32 = B.make_params(pd, B.OK_FP32, storage=fmt)
+    p64 = B.make_params(pd, B.OK_FP64, storage=fmt)
+    W32 = G.precalc(p32, U)
+    psi = I.gaussian_spinor(DIMS, 6)
+    got = G.apply(p32, W32, psi)[idx]
+    want = o.apply_W(psi, idx=idx, W=want_W)
+    assert sampled_rel_l2(got, want) <= FP32_TOL
+    W64 = G.precalc(p64, U)
+    got64 = G.apply(p64, W64, psi)[idx]
+    assert G.per_site_rel_err(got64, want) <= 1e-12
+    need = B.ok_mixed_work_bytes(p64)
+    ws = B.alloc_bytes(need, G.DEV)
+    B.ok_set_workspace(ws, need)
+    src = G.pack_spinor(p64, psi)
+    x = B.alloc_vec(p64)
+    tol = 1e-10
+    st, it, outer, res = B.ok_bicgstab_mixed(W64, W32, src, x, tol, 1e-4, 2000, 50, raise_on_fail=False)
+    assert st == 0 and res <= tol and 2 <= outer <= 6 and 20 <= it <= 400
+    xs = G.unpack_spinor(p64, x, psi.shape)
+    r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
+    est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
+    assert est <= 3 * tol, est
+    B.ok_set_workspace(None)
