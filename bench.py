@@ -394,6 +394,52 @@ def run_ours(args, wl):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: apply-throughput sweep over lattice sizes (Haar links seed 8, kappa 0.08, fp32), single GPU.
+    One JSON line: per lattice and W storage format the mean device time of an ok_dirac_apply and the derived rates."""
+    import torch
+    from paper_1311_5029_b200 import binding as B
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    B.lib()
+    stream = torch.cuda.Stream(device=dev)
+    B.ok_set_stream(stream)
+    rows = []
+    for dims in [(8, 8, 8, 16), (12, 12, 12, 24), (16, 16, 16, 32), (20, 20, 20, 64), (24, 24, 24, 64), (32, 32, 32, 64)]:
+        U = I.haar_links(dims, 8)
+        pd = I.make_params(dims, 0.08, I.tadpole_u0(I.mean_plaquette(dims, U)))
+        links = torch.from_numpy(U).to(dev)
+        V = int(np.prod(dims))
+        psi = torch.from_numpy(I.gaussian_spinor(dims, 9)).to(torch.complex64).to(dev)
+        for storage in (0, 2, 3):
+            p = B.make_params(pd, B.OK_FP32, storage=storage)
+            W, work = B.alloc_W(p, dev), B.alloc_work(p, dev)
+            src, out = B.alloc_vec(p, dev), B.alloc_vec(p, dev)
+            B.ok_set_workspace(work)
+            with torch.cuda.stream(stream):
+                B.ok_precalc_W(links, p, W)
+                B.ok_pack_spinor(p, psi, src)
+                for _ in range(5):
+                    B.ok_dirac_apply(W, src, out)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                nrep = 200 if V < 200000 else 50
+                e0.record(stream)
+                for _ in range(nrep):
+                    B.ok_dirac_apply(W, src, out)
+                e1.record(stream)
+            stream.synchronize()
+            ms = e0.elapsed_time(e1) / nrep
+            alg = V * alg_bytes_per_site(4, 1, storage)
+            rows.append({"dims": "x".join(map(str, dims)), "sites": V, "storage": ["dense", "block", "ds", "conj"][storage],
+                         "W_GB": B.ok_W_bytes(p) / 1e9, "apply_ms": ms, "GBps": alg / ms / 1e6, "sites_per_s": V / ms * 1e3,
+                         "gflops": V * FLOP_PER_SITE / ms / 1e6})
+            B.ok_set_workspace(None)
+            B.ok_forget_W(W)
+            del W, work, src, out
+        del links, psi
+    print(json.dumps({"metric": "OK Dirac apply throughput sweep (fp32, Haar links seed 8, kappa 0.08)", "n_gpus": 1, "sweep": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -402,8 +448,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="20x20x20x64-fp32", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="configs[4]: apply throughput over lattice sizes (not the driver's contract line)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, args.workload)
     else:
         run_ours(args, args.workload)
