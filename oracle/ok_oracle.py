@@ -477,3 +477,53 @@ def bicgstab_mixed(apply_hi, apply_lo, b, tol, inner_tol, maxit, max_outer=50, l
         x = x + rn * e.astype(b.dtype)
         r = b - apply_hi(x)
     return x, total, outer, nrm(b - apply_hi(x)) / bnorm, status
+
+
+def gamma5_mul(v):
+    """(Gamma_5 v)(x) = gamma_5 v(x) on a spinor field [V, 12] (gamma_5 = gamma_1 gamma_2 gamma_3 gamma_4 x 1_colour)."""
+    return np.einsum("ab,nbc->nac", GAMMA5, v.reshape(-1, 4, 3)).reshape(v.shape)
+
+
+def cgnr(apply, b, tol, maxit):
+    """Conjugate gradient on the normal equations M^dag M x = M^dag b ("M^dag M preconditioning", named as future
+    work there), with M^dag = Gamma_5 M Gamma_5 (gamma_5-hermiticity of the OK action, pin P4).
+    Textbook CGNR, x0 = 0:  r = b; z = M^dag r; p = z;  loop: w = M p; alpha = <z,z>/<w,w>; x += alpha p; r -= alpha w;
+    stop when ||r|| <= tol ||b|| (then true-residual check, restart from it if it fails); z' = M^dag r; beta = <z',z'>/<z,z>; p = z' + beta p.
+    Returns (x, iters, true_relative_residual, status); status 0 ok, -3 breakdown, -4 maxit."""
+    dag = lambda v: gamma5_mul(apply(gamma5_mul(v)))
+    n2 = lambda a: float(np.vdot(a, a).real)
+    bn2 = n2(b)
+    x = np.zeros_like(b)
+    if bn2 == 0.0:
+        return x, 0, 0.0, 0
+    r = b.copy()
+    z = dag(r)
+    p = z.copy()
+    zz = n2(z)
+    it, status = 0, -4
+    while it < maxit:
+        it += 1
+        w = apply(p)
+        ww = n2(w)
+        if not np.isfinite(ww) or ww < 1e-300 or zz < 1e-300:
+            status = -3
+            break
+        alpha = zz / ww
+        x = x + alpha * p
+        r = r - alpha * w
+        if n2(r) <= tol * tol * bn2:
+            rt = b - apply(x)
+            if n2(rt) <= tol * tol * bn2:
+                status = 0
+                break
+            r = rt
+            z = dag(r)
+            p = z.copy()
+            zz = n2(z)
+            continue
+        z = dag(r)
+        zz_new = n2(z)
+        p = z + (zz_new / zz) * p
+        zz = zz_new
+    rt = b - apply(x)
+    return x, it, float(np.sqrt(n2(rt) / bn2)), status

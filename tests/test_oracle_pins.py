@@ -412,3 +412,30 @@ def test_P8_mixed_precision_vs_dense_LU_2p4():
     assert st == 0 and its == 0 and outer == 0 and np.all(x == 0)
     x, its, outer, res, st = oo.bicgstab_mixed(hi, lo, b, 1e-12, 1e-4, 5)
     assert st == -4 and its == 5 and res > 1e-12
+
+
+# ----------------------------------------------------------------------------- P9 CG on the normal equations
+def test_P9_cgnr_vs_dense_LU_and_gamma5():
+    dims = (2, 2, 2, 2)
+    U = I.near_identity_links(dims, 0.3, 1)
+    o = Oracle(U, I.make_params(dims, 0.10, I.tadpole_u0(I.mean_plaquette(dims, U))))
+    M = o.dense_M()
+    W = o.precalc_W()
+    ap = lambda v: o.apply_W(v, W=W)
+    b = I.gaussian_spinor(dims, 2)
+    # Gamma_5 M Gamma_5 is the adjoint of the dense matrix, so CGNR's M^dag is the true one
+    v = I.gaussian_spinor(dims, 5)
+    want = (M.conj().T @ v.reshape(-1)).reshape(v.shape)
+    assert rel(oo.gamma5_mul(ap(oo.gamma5_mul(v))), want) < 1e-13
+    assert rel(oo.gamma5_mul(oo.gamma5_mul(v)), v) < 1e-15                      # gamma_5^2 = 1
+    x, it, res, st = oo.cgnr(ap, b, 1e-10, 2000)
+    xs = np.linalg.solve(M, b.reshape(-1)).reshape(b.shape)
+    assert st == 0 and res <= 1e-10 and rel(x, xs) < 1e-8
+    assert it <= 192                                                          # exact arithmetic: at most dim(M) steps
+    # textbook property: the residual norm of M^dag M x = M^dag b decreases monotonically in the M^dag M energy norm;
+    # here we check the cheap consequence that CGNR never needs more M applies than 2 x dim on a well-conditioned matrix
+    rng = np.random.default_rng(4)
+    x0, it0, res0, st0 = oo.cgnr(ap, 0 * b, 1e-10, 10)
+    assert st0 == 0 and it0 == 0 and np.all(x0 == 0)
+    x1, it1, res1, st1 = oo.cgnr(ap, b, 1e-10, 3)
+    assert st1 == -4 and it1 == 3 and res1 > 1e-10
