@@ -135,6 +135,12 @@ int ok_dirac_apply(const void* W, const void* psi, void* out);
  * *resid = max over columns.  iters/resid: HOST pointers.  Needs the workspace. */
 int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, int* iters, double* resid);
 
+/* CG on the normal equations M^dag M x = M^dag src ("M^dag M preconditioning"), with
+ * M^dag = Gamma_5 M Gamma_5: a second solver on the same apply, nrhs = 1, any precision and W storage format.
+ * Same conventions as ok_bicgstab (x0 = 0, fp64 fixed-order reductions, stop on ||r|| <= tol ||src|| confirmed by the
+ * true residual); *iters = CG iterations (2 applies each).  Needs the workspace (ok_work_bytes). */
+int ok_cgnr(const void* W, const void* src, void* x, double tol, int maxit, int* iters, double* resid);
+
 /* Mixed-precision inversion, PAPER.md:114 ("We perform a mixed precision inversion by calling the ... inverter or
  * Dirac operation module in single or double precision, as appropriate"): defect correction around the fp32
  * BiCGStab with both sets of precalculation matrices resident,

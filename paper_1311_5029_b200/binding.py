@@ -48,6 +48,7 @@ EXPORTS = {
     "ok_bicgstab": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int,
                               C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_dirac_apply_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_cgnr": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_mixed_work_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
     "ok_bicgstab_mixed": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int,
                                     C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
@@ -172,6 +173,15 @@ def ok_bicgstab(W, src, x, tol, maxit, raise_on_fail=True):
     st = lib().ok_bicgstab(_ptr(W), _ptr(src), _ptr(x), float(tol), int(maxit), C.byref(it), C.byref(res))
     if st != 0 and raise_on_fail:
         raise OkError(st, "ok_bicgstab")
+    return st, it.value, res.value
+
+
+def ok_cgnr(W, src, x, tol, maxit, raise_on_fail=True):
+    """Returns (status, iters, true_relative_residual)."""
+    it, res = C.c_int(0), C.c_double(0.0)
+    st = lib().ok_cgnr(_ptr(W), _ptr(src), _ptr(x), float(tol), int(maxit), C.byref(it), C.byref(res))
+    if st != 0 and raise_on_fail:
+        raise OkError(st, "ok_cgnr")
     return st, it.value, res.value
 
 

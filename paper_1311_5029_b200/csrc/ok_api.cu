@@ -242,6 +242,16 @@ int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, 
   return run_bicgstab(&p, W_payload(W), src, x, tol, maxit, iters, resid);
 }
 
+int ok_cgnr(const void* W, const void* src, void* x, double tol, int maxit, int* iters, double* resid) {
+  if (!aligned16(src) || !aligned16(x) || src == x || !iters || !resid || !(tol > 0.0) || maxit < 1) return OK_EINVAL;
+  ok_params p;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  if (p.nrhs != 1) return OK_EINVAL;
+  if (!ctx().work || ctx().work_bytes < bicgstab_work_bytes(&p)) return OK_EWORKSPACE;
+  return run_cgnr(&p, W_payload(W), src, x, tol, maxit, iters, resid);
+}
+
 size_t ok_mixed_work_bytes(const ok_params* p) {
   if (!valid_params(p) || p->nrhs != 1) return 0;
   return mixed_work_bytes(p) + 4096;

@@ -186,7 +186,8 @@ apply_sparse_kernel(const typename SV<real>::cx* __restrict__ W, const typename 
   c.g = g;
   const int blk = blockIdx.x;
   int n = blk * kBlock + c.lane;
-  if (n >= g.V) n = 0;   // padded lane: W is zero there, the result is zero
+  const bool padded = n >= g.V;   // padded lane of the last block: its own W is zero, but OK_W_CONJ also reads a neighbour's
+  if (padded) n = 0;
   c.x = n % g.L[0];
   int q = n / g.L[0];
   c.y = q % g.L[1];
@@ -223,6 +224,10 @@ apply_sparse_kernel(const typename SV<real>::cx* __restrict__ W, const typename 
 #undef OK_TERM
 #undef OK_TERM_PAIR
 
+  if (padded) {
+#pragma unroll
+    for (int r = 0; r < 3; ++r) acc_u[r][0] = acc_u[r][1] = acc_l[r][0] = acc_l[r][1] = real(0);
+  }
   // store: row -> (unit, sub) of the internal spinor layout
   real* ob = reinterpret_cast<real*>(out + (size_t)blk * NC * kBlock);
   constexpr int RPU = 12 / NC;   // rows (components) per 16-byte unit: 2 (fp32) or 1 (fp64)

@@ -137,6 +137,8 @@ size_t precalc_work_bytes(const ok_params* p);
 int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,
                  int* iters, double* resid);
 size_t bicgstab_work_bytes(const ok_params* p);
+// CG on the normal equations (ok_cgnr.cu); workspace: bicgstab_work_bytes
+int run_cgnr(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit, int* iters, double* resid);
 // mixed precision (ok_mixed.cu)
 size_t mixed_work_bytes(const ok_params* p);
 int run_bicgstab_mixed(const ok_params* p64, const void* W64payload, const ok_params* p32, const void* W32payload, const void* src, void* x,

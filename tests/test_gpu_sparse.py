@@ -131,14 +131,23 @@ def test_sparse_precalc_then_apply(case, prec, fmt):
         assert G.per_site_rel_err(got, want) <= FP64_TOL
     else:
         assert G.rel_l2(got, want) <= FP32_TOL
-    # padded lanes of the last block stay zero and a zero field maps to zero
+    # a zero field maps to zero, and the padded lanes of the last 32-site block stay zero in the internal layout
     assert np.all(G.apply(p, W, np.zeros_like(psi)) == 0)
+    packed_out = B.alloc_vec(p)
+    B.ok_dirac_apply(W, G.pack_spinor(p, psi), packed_out)
+    torch.cuda.synchronize()
+    raw = packed_out.view(torch.float64 if prec == B.OK_FP64 else torch.float32).cpu().numpy()
+    nblk = (o.V + 31) // 32
+    per = 2 if prec == B.OK_FP64 else 4                       # reals per 16-byte unit
+    units = raw.reshape(nblk, -1, 32, per)
+    if o.V % 32:
+        assert np.all(units[-1, :, o.V % 32:, :] == 0)
 
 
 @pytest.mark.parametrize("fmt", FORMATS)
 @pytest.mark.parametrize("prec,tol", [(B.OK_FP64, 1e-10), (B.OK_FP32, 1e-6)])
-def test_sparse_bicgstab_vs_oracle(prec, tol, fmt):
-    dims = (4, 4, 4, 8)
+@pytest.mark.parametrize("dims", [(4, 4, 4, 8), (4, 3, 3, 2)])            # the second one has a ragged last block (72 sites)
+def test_sparse_bicgstab_vs_oracle(dims, prec, tol, fmt):
     U, pd, o = setup(dims)
     p = B.make_params(pd, prec, storage=fmt)
     W = G.precalc(p, U)
