@@ -208,25 +208,28 @@ struct P4 {
 // Positive blocks of the term family at site x.  A = diagonal block, B = off-diagonal block.
 //   fam 0: W^0 (Eq. 2.6)   fam 1: W^+_4 (2.7)   fam 2: W^+_i (2.8)   fam 3: W^++_ii (2.9)
 //   fam 4: W^++_ij (2.11)  fam 5: W^+-_ij (2.12)
-__device__ void positive_blocks(int fam, int i, int j, const Site& x, const double2* __restrict__ links,
-                                const cm3* __restrict__ FS, const PrecalcArgs& a, P4& A, P4& B) {
+template <int fam, int i, int j>
+__device__ __forceinline__ void positive_blocks(const Site& x, const double2* __restrict__ links,
+                                                const cm3* __restrict__ FS, const PrecalcArgs& a, P4& A, P4& B) {
 #pragma unroll
   for (int k = 0; k < 4; ++k) { A.c[k] = zero3(); B.c[k] = zero3(); }
-  if (fam == 0) {
+  if constexpr (fam == 0) {
+#pragma unroll
     for (int m = 0; m < 3; ++m) {
       axpy(A.c[m + 1], 0.0, a.d0, ldF(FS, m, x, a));       // D^0 = d0 * i sum sigma_m B_m
       axpy(B.c[m + 1], a.s0, 0.0, ldF(FS, 3 + m, x, a));   // S^0 = s0 * sum sigma_m E_m
     }
-  } else if (fam == 1) {
+  } else if constexpr (fam == 1) {
     const cm3 U = ldU(links, x, 3, a);
     const Site xp = shift(x, 3, 1, a.g);
+#pragma unroll
     for (int m = 0; m < 3; ++m) {
       axpy(B.c[m + 1], a.s4, 0.0, mul(U, ldF(FS, 3 + m, xp, a)));
       axpy(B.c[m + 1], -a.s4, 0.0, mul(ldF(FS, 3 + m, x, a), U));
     }
     axpy(A.c[0], -1.0, 0.0, U);
-  } else if (fam == 2) {
-    const int k = (i + 1) % 3, l = (i + 2) % 3;
+  } else if constexpr (fam == 2) {
+    constexpr int k = (i + 1) % 3, l = (i + 2) % 3;
     const cm3 U = ldU(links, x, i, a);
     const Site xp = shift(x, i, 1, a.g);
     axpy(B.c[i + 1], a.a1, 0.0, U);
@@ -247,6 +250,7 @@ __device__ void positive_blocks(int fam, int i, int j, const Site& x, const doub
       axpy(A.c[l + 1], 0.0, a.c5u, P); axpy(A.c[l + 1], 0.0, a.c5u, Q);
     }
     if (a.cg != 0.0) {
+#pragma unroll
       for (int q = 0; q < 2; ++q) {
         const int m = q ? l : k;           // staple direction
         const int tgt = q ? k : l;         // sigma index receiving G_m:  +i cg G_l -> C_k ; -i cg G_k -> C_l
@@ -262,11 +266,11 @@ __device__ void positive_blocks(int fam, int i, int j, const Site& x, const doub
         axpy(A.c[tgt + 1], 0.0, -sgn * a.cg, G);
       }
     }
-  } else if (fam == 3) {
+  } else if constexpr (fam == 3) {
     const cm3 P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), i, a));
     axpy(A.c[0], a.dii, 0.0, P);
     axpy(B.c[i + 1], a.sii, 0.0, P);
-  } else if (fam == 4) {
+  } else if constexpr (fam == 4) {
     cm3 P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), j, a));
     axpy(P, 1.0, 0.0, mul(ldU(links, x, j, a), ldU(links, shift(x, j, 1, a.g), i, a)));
     axpy(B.c[i + 1], a.sij, 0.0, P);
@@ -292,53 +296,20 @@ template <typename real> struct WUnit;
 template <> struct WUnit<float> { using type = float4; using cx = float2; static constexpr int NC = 6; };
 template <> struct WUnit<double> { using type = double2; using cx = double2; static constexpr int NC = 12; };
 
-template <typename real>
-__global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
-                                                            typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
+// One (site, term) with the family and directions as template arguments: Pauli components that vanish for the family are
+// never materialised, so the per-term register footprint stays far below the 8 colour matrices of the generic form.
+template <typename real, int fam, int i, int j>
+__device__ __noinline__ void assemble_term(const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                              typename WUnit<real>::type* __restrict__ W, typename WUnit<real>::type* __restrict__ Wt,
+                                              const PrecalcArgs& a, int term, bool neg, int n, int blk, int lane) {
   using unit_t = typename WUnit<real>::type;
   constexpr int NC = WUnit<real>::NC;
-  const int lane = threadIdx.x;
-  const int term = blockIdx.y * 9 + threadIdx.y;
-  const int blk = blockIdx.x;
-  const int n = blk * kBlock + lane;
-  unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
-  if (a.mrhs && n >= a.g.V) return;   // the tile layout has no padded sites
-  if (a.storage == OK_W_CONJ && term_is_neg(term)) return;   // rebuilt at apply time from term - 1 of the neighbour site
-  if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units this term keeps
-    using cx = typename WUnit<real>::cx;
-    cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units_rt(a.storage) * kBlock + lane;
-    for (int r = 0; r < 12; ++r)
-      for (int col = 0; col < 12; ++col) {
-        const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
-        if (ref.unit >= 0 && ref.stored) Ws[(size_t)ref.unit * kBlock] = cx{};
-      }
-    return;
-  }
-  if (n >= a.g.V) {   // padded site: zeros
-    unit_t z = {};
-    for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
-    return;
-  }
-  // term -> family, directions, sign of the hop
-  int fam, i = 0, j = 0;
-  bool neg = false;
-  if (term == 0) fam = 0;
-  else if (term <= 6) { fam = 2; i = (term - 1) >> 1; neg = ((term - 1) & 1); }
-  else if (term <= 8) { fam = 1; neg = (term == 8); }
-  else if (term <= 14) { fam = 3; i = (term - 9) >> 1; neg = ((term - 9) & 1); }
-  else {
-    const int q = (term - 15) >> 2, w = (term - 15) & 3;   // pair index, (++, --, +-, -+)
-    i = q == 2 ? 1 : 0;
-    j = q == 0 ? 1 : 2;
-    fam = (w < 2) ? 4 : 5;
-    neg = (w & 1);
-  }
   Site x = site_of(n, a.g);
   if (neg) {   // positive blocks at x - offset(term_positive) = x + offset(term)
     for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
   }
   P4 A, B;
-  positive_blocks(fam, i, j, x, links, FS, a, A, B);
+  positive_blocks<fam, i, j>(x, links, FS, a, A, B);
   if (neg) {   // Eqs. (2.3), (2.10): A -> A^dag, B -> -B^dag
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -354,6 +325,7 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
   const double llsgn = (fam == 0) ? -1.0 : 1.0;
   const double mass = (fam == 0) ? a.mass : 0.0;
 
+#pragma unroll
   for (int r = 0; r < 12; ++r) {
     const int alpha = r / 3, ca = r % 3, bi = alpha >> 1, al = alpha & 1;
     double2 row[12];
@@ -430,6 +402,65 @@ __global__ void __launch_bounds__(32 * 9) assemble_W_kernel(const double2* __res
   }
 }
 
+
+template <typename real>
+__global__ void __launch_bounds__(32 * 3) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                                            typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
+  using unit_t = typename WUnit<real>::type;
+  constexpr int NC = WUnit<real>::NC;
+  const int lane = threadIdx.x;
+  const int term = blockIdx.y * 3 + threadIdx.y;
+  const int blk = blockIdx.x;
+  const int n = blk * kBlock + lane;
+  unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
+  if (a.mrhs && n >= a.g.V) return;   // the tile layout has no padded sites
+  if (a.storage == OK_W_CONJ && term_is_neg(term)) return;   // rebuilt at apply time from term - 1 of the neighbour site
+  if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units this term keeps
+    using cx = typename WUnit<real>::cx;
+    cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units_rt(a.storage) * kBlock + lane;
+    for (int r = 0; r < 12; ++r)
+      for (int col = 0; col < 12; ++col) {
+        const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
+        if (ref.unit >= 0 && ref.stored) Ws[(size_t)ref.unit * kBlock] = cx{};
+      }
+    return;
+  }
+  if (n >= a.g.V) {   // padded site: zeros
+    unit_t z = {};
+    for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
+    return;
+  }
+  // term -> family, directions, sign of the hop (term order of ok.h)
+#define OK_ASM(F, I_, J_, NEG) assemble_term<real, F, I_, J_>(links, FS, W, Wt, a, term, NEG, n, blk, lane)
+  switch (term) {
+    case 0: OK_ASM(0, 0, 0, false); break;
+    case 1: OK_ASM(2, 0, 0, false); break;
+    case 2: OK_ASM(2, 0, 0, true); break;
+    case 3: OK_ASM(2, 1, 0, false); break;
+    case 4: OK_ASM(2, 1, 0, true); break;
+    case 5: OK_ASM(2, 2, 0, false); break;
+    case 6: OK_ASM(2, 2, 0, true); break;
+    case 7: OK_ASM(1, 0, 0, false); break;
+    case 8: OK_ASM(1, 0, 0, true); break;
+    case 9: OK_ASM(3, 0, 0, false); break;
+    case 10: OK_ASM(3, 0, 0, true); break;
+    case 11: OK_ASM(3, 1, 0, false); break;
+    case 12: OK_ASM(3, 1, 0, true); break;
+    case 13: OK_ASM(3, 2, 0, false); break;
+    case 14: OK_ASM(3, 2, 0, true); break;
+    default: {
+      const int q = (term - 15) >> 2, w = (term - 15) & 3;   // pair (x,y), (x,z), (y,z) ; (++, --, +-, -+)
+      const bool ng = (w & 1) != 0;
+      if (w < 2) {
+        if (q == 0) OK_ASM(4, 0, 1, ng); else if (q == 1) OK_ASM(4, 0, 2, ng); else OK_ASM(4, 1, 2, ng);
+      } else {
+        if (q == 0) OK_ASM(5, 0, 1, ng); else if (q == 1) OK_ASM(5, 0, 2, ng); else OK_ASM(5, 1, 2, ng);
+      }
+    }
+  }
+#undef OK_ASM
+}
+
 size_t precalc_work_bytes(const ok_params* p) {
   Geom g = make_geom(p);
   return (size_t)6 * g.nblk * kBlock * sizeof(cm3);
@@ -466,7 +497,7 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   cudaStream_t st = ctx().stream;
   field_strength_kernel<<<dim3((a.g.V + 127) / 128, 6), 128, 0, st>>>(static_cast<const double2*>(links), FS, a);
   OK_LAUNCHED("field_strength_kernel");
-  dim3 grid(a.g.nblk, 3), block(32, 9);
+  dim3 grid(a.g.nblk, 9), block(32, 3);
   if (p->precision == OK_FP64)
     assemble_W_kernel<double><<<grid, block, 0, st>>>(static_cast<const double2*>(links), FS, static_cast<double2*>(Wp), a);
   else
