@@ -404,7 +404,7 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
 
 
 template <typename real>
-__global__ void __launch_bounds__(32 * 3) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+__global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
                                                             typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
   using unit_t = typename WUnit<real>::type;
   constexpr int NC = WUnit<real>::NC;
