@@ -403,13 +403,16 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
 }
 
 
-template <typename real>
+// CLS splits the 27 terms into four launches so that every launch carries only the registers its families need:
+//   0: W^0, W^+-_4 (terms 0, 7, 8)   1: W^+-_i (1..6, the heavy one)   2: W^{++/--}_ii (9..14)   3: the 12 pair terms (15..26)
+template <typename real, int CLS>
 __global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
-                                                            typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
+                                                                           typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
   using unit_t = typename WUnit<real>::type;
   constexpr int NC = WUnit<real>::NC;
   const int lane = threadIdx.x;
-  const int term = blockIdx.y * 3 + threadIdx.y;
+  const int idx = blockIdx.y * 3 + threadIdx.y;
+  const int term = CLS == 0 ? (idx == 0 ? 0 : 6 + idx) : CLS == 1 ? 1 + idx : CLS == 2 ? 9 + idx : 15 + idx;
   const int blk = blockIdx.x;
   const int n = blk * kBlock + lane;
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
@@ -432,23 +435,16 @@ __global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __
   }
   // term -> family, directions, sign of the hop (term order of ok.h)
 #define OK_ASM(F, I_, J_, NEG) assemble_term<real, F, I_, J_>(links, FS, W, Wt, a, term, NEG, n, blk, lane)
-  switch (term) {
-    case 0: OK_ASM(0, 0, 0, false); break;
-    case 1: OK_ASM(2, 0, 0, false); break;
-    case 2: OK_ASM(2, 0, 0, true); break;
-    case 3: OK_ASM(2, 1, 0, false); break;
-    case 4: OK_ASM(2, 1, 0, true); break;
-    case 5: OK_ASM(2, 2, 0, false); break;
-    case 6: OK_ASM(2, 2, 0, true); break;
-    case 7: OK_ASM(1, 0, 0, false); break;
-    case 8: OK_ASM(1, 0, 0, true); break;
-    case 9: OK_ASM(3, 0, 0, false); break;
-    case 10: OK_ASM(3, 0, 0, true); break;
-    case 11: OK_ASM(3, 1, 0, false); break;
-    case 12: OK_ASM(3, 1, 0, true); break;
-    case 13: OK_ASM(3, 2, 0, false); break;
-    case 14: OK_ASM(3, 2, 0, true); break;
-    default: {
+  if constexpr (CLS == 0) {
+    if (term == 0) OK_ASM(0, 0, 0, false); else OK_ASM(1, 0, 0, term == 8);
+  } else if constexpr (CLS == 1) {
+    const bool ng = (term & 1) == 0;
+    if (term <= 2) OK_ASM(2, 0, 0, ng); else if (term <= 4) OK_ASM(2, 1, 0, ng); else OK_ASM(2, 2, 0, ng);
+  } else if constexpr (CLS == 2) {
+    const bool ng = (term & 1) == 0;
+    if (term <= 10) OK_ASM(3, 0, 0, ng); else if (term <= 12) OK_ASM(3, 1, 0, ng); else OK_ASM(3, 2, 0, ng);
+  } else {
+    {
       const int q = (term - 15) >> 2, w = (term - 15) & 3;   // pair (x,y), (x,z), (y,z) ; (++, --, +-, -+)
       const bool ng = (w & 1) != 0;
       if (w < 2) {
@@ -497,12 +493,19 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   cudaStream_t st = ctx().stream;
   field_strength_kernel<<<dim3((a.g.V + 127) / 128, 6), 128, 0, st>>>(static_cast<const double2*>(links), FS, a);
   OK_LAUNCHED("field_strength_kernel");
-  dim3 grid(a.g.nblk, 9), block(32, 3);
-  if (p->precision == OK_FP64)
-    assemble_W_kernel<double><<<grid, block, 0, st>>>(static_cast<const double2*>(links), FS, static_cast<double2*>(Wp), a);
-  else
-    assemble_W_kernel<float><<<grid, block, 0, st>>>(static_cast<const double2*>(links), FS, static_cast<float4*>(Wp), a);
-  OK_LAUNCHED("assemble_W_kernel");
+  const dim3 block(32, 3);
+  const double2* lk = static_cast<const double2*>(links);
+#define OK_ASM_LAUNCH(CLS, NY)                                                                                              \
+  do {                                                                                                                      \
+    if (p->precision == OK_FP64) assemble_W_kernel<double, CLS><<<dim3(a.g.nblk, NY), block, 0, st>>>(lk, FS, static_cast<double2*>(Wp), a); \
+    else assemble_W_kernel<float, CLS><<<dim3(a.g.nblk, NY), block, 0, st>>>(lk, FS, static_cast<float4*>(Wp), a);          \
+    OK_LAUNCHED("assemble_W_kernel");                                                                                       \
+  } while (0)
+  OK_ASM_LAUNCH(1, 2);   // the heavy class first
+  OK_ASM_LAUNCH(0, 1);
+  OK_ASM_LAUNCH(2, 2);
+  OK_ASM_LAUNCH(3, 4);
+#undef OK_ASM_LAUNCH
   return OK_SUCCESS;
 }
 
