@@ -168,6 +168,13 @@ int ok_W_params(const void* W, ok_params* p);
  * reusing its memory for anything else; a later W written there by ok_precalc_W / ok_pack_W is
  * recorded again.  Unknown pointers are ignored.  Returns OK_SUCCESS. */
 int ok_forget_W(const void* W);
+/* Layout query for the reduced storage formats (pure host arithmetic, no device needed): where element (row, col) of
+ * W_term is kept.  Returns the complex-unit index inside a site's OK_W_BLOCK / OK_W_DS / OK_W_CONJ record
+ * ([block][unit][site 32][complex]), or -1 when the element is structurally zero, or -2 on bad arguments.  info[0] = 1 if
+ * this element is the stored copy (0: implied by another quadrant / by the neighbour site), info[1] = sign (+1/-1) and
+ * info[2] = 1 if the value is the complex conjugate of the stored number, info[3] = term whose offset leads to the site
+ * holding it (-1: the same site).  info: HOST, 4 ints, may be NULL. */
+int ok_W_unit_index(int storage, int term, int row, int col, int* info);
 /* Number of kernels the library has launched since load (for launch accounting in benches). */
 uint64_t ok_launch_count(void);
 /* Select the apply kernel variant (0 = default).  Tuning knob; results are identical. */

@@ -49,6 +49,7 @@ EXPORTS = {
                               C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_dirac_apply_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "ok_cgnr": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double)]),
+    "ok_W_unit_index": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int)]),
     "ok_mixed_work_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
     "ok_bicgstab_mixed": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int,
                                     C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
@@ -183,6 +184,13 @@ def ok_cgnr(W, src, x, tol, maxit, raise_on_fail=True):
     if st != 0 and raise_on_fail:
         raise OkError(st, "ok_cgnr")
     return st, it.value, res.value
+
+
+def ok_W_unit_index(storage, term, row, col):
+    """Returns (unit, stored, sign, conj, shift_term); unit = -1 for a structural zero."""
+    info = (C.c_int * 4)()
+    u = lib().ok_W_unit_index(int(storage), int(term), int(row), int(col), info)
+    return u, info[0], info[1], info[2], info[3]
 
 
 def ok_mixed_work_bytes(p):

@@ -273,6 +273,13 @@ int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x
   return run_bicgstab_mixed(&p64, W_payload(W64), &p32, W_payload(W32), src, x, tol, inner_tol, maxit, max_outer, iters, outer, resid);
 }
 
+int ok_W_unit_index(int storage, int term, int row, int col, int* info) {
+  if (storage < OK_W_BLOCK || storage > OK_W_CONJ || term < 0 || term >= kTerms || row < 0 || row >= 12 || col < 0 || col >= 12) return -2;
+  const SparseRef r = sparse_ref(storage, term, row, col);
+  if (info) { info[0] = r.unit >= 0 ? r.stored : 0; info[1] = r.sign; info[2] = r.conj; info[3] = r.shift; }
+  return r.unit;
+}
+
 const char* ok_strerror(int status) {
   switch (status) {
     case OK_SUCCESS: return "success";
