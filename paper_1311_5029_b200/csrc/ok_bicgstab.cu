@@ -166,10 +166,25 @@ enum Stage { FIN_INIT = 0, FIN_V = 1, FIN_T = 2, FIN_XR = 3, FIN_RES = 4 };
 
 template <int STAGE>
 __global__ void __launch_bounds__(kVecThreads) k_finalize(const double* __restrict__ partials, int count, Scal* sc) {
+  // thread-serial sum in a fixed order; the loads of 8 consecutive strides are issued together (latency, not order, changes)
+  constexpr bool kThree = STAGE == FIN_V || STAGE == FIN_T || STAGE == FIN_XR;
   double d[3] = {0.0, 0.0, 0.0};
-  for (int i = threadIdx.x; i < count; i += kVecThreads) {
+  int i = threadIdx.x;
+  for (; i + 7 * kVecThreads < count; i += 8 * kVecThreads) {
+    double v[8][3];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const double* q = partials + (size_t)(i + u * kVecThreads) * 3;
+      v[u][0] = q[0];
+      v[u][1] = kThree ? q[1] : 0.0;
+      v[u][2] = kThree ? q[2] : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { d[0] += v[u][0]; d[1] += v[u][1]; d[2] += v[u][2]; }
+  }
+  for (; i < count; i += kVecThreads) {
     d[0] += partials[(size_t)i * 3 + 0];
-    if (STAGE == FIN_V || STAGE == FIN_T || STAGE == FIN_XR) {
+    if (kThree) {
       d[1] += partials[(size_t)i * 3 + 1];
       d[2] += partials[(size_t)i * 3 + 2];
     }
