@@ -20,6 +20,8 @@
  *     buffer the library has not seen (one 1 KiB header read), which synchronise that stream.
  *   - Return value: 0 (OK_SUCCESS) or a negative ok_status.  No exceptions, no aborts.
  *   - There is no CPU fallback: without a CUDA device every compute call returns OK_ECUDA.
+ *   - One device and one calling thread per process (the model is one process per GPU): the stream, the workspace,
+ *     the W handle table and a few device-side scratch symbols are process-wide state, not per-call arguments.
  *
  * Canonical (external) layouts, complex numbers interleaved (re, im):
  *   site index   n = x + Lx*(y + Ly*(z + Lz*t)),  dims = {Lx, Ly, Lz, T};  V = Lx*Ly*Lz*T
