@@ -156,3 +156,34 @@ def test_fullsize_reduced_formats_apply_and_mixed_solve(big, fmt):
     est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
     assert est <= 3 * tol, est
     B.ok_set_workspace(None)
+
+
+def test_fullsize_config5_haar_32x32x32x64():
+    """BASELINE.json configs[4]: 32^3 x 64 (2 097 152 sites), fp32 W (65 GB), Haar-random links seed 8, kappa 0.08, u0 = 1
+    (DESIGN.md R-U0HAAR): sampled-site apply parity, and the BiCGStab solution's residual evaluated by the oracle on sampled
+    sites (the oracle computes W on the fly for the sites it is asked about)."""
+    dims = (32, 32, 32, 64)
+    U = I.haar_links(dims, 8)
+    plaq = I.mean_plaquette(dims, U)
+    u0 = I.tadpole_u0(plaq)
+    assert abs(plaq) < 0.01 and u0 == 1.0
+    pd = I.make_params(dims, 0.08, u0)
+    o = Oracle(U, pd)
+    p = B.make_params(pd, B.OK_FP32)
+    idx = sample_sites(dims, n_even=256, n_rand=256)
+    want_W = o.precalc_W(idx)
+    W = G.precalc(p, U)
+    psi = I.gaussian_spinor(dims, 9)
+    got = G.apply(p, W, psi)[idx]
+    want = o.apply_W(psi, idx=idx, W=want_W)
+    assert sampled_rel_l2(got, want) <= FP32_TOL
+    G.workspace(p)
+    src = G.pack_spinor(p, psi)
+    x = B.alloc_vec(p)
+    tol = 1e-6
+    st, it, res = B.ok_bicgstab(W, src, x, tol, 2000, raise_on_fail=False)
+    assert st == 0 and res <= tol and 3 <= it <= 40           # strongly diagonally dominant at kappa = 0.08 (bench: 9 iterations)
+    xs = G.unpack_spinor(p, x, psi.shape)
+    r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
+    est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
+    assert est <= 5 * tol, est
