@@ -34,6 +34,7 @@ struct PrecalcArgs {
   int Vpad;
   int mrhs;                    // 1: write the nrhs = 12 tensor-core tile layout (ok_internal.cuh)
   int storage;                 // OK_W_DENSE / OK_W_BLOCK / OK_W_DS (ok_sparse.cuh)
+  int blk0;                    // first 32-site block of this launch (12-RHS: the dense W of a chunk goes to a bounce buffer)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
   double s4;                   // c_EE / (2 u0^4)      (Eq. 2.7)
@@ -376,22 +377,6 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
     }
     unit_t* dst = Wt + (size_t)r * NC * kBlock;
     if constexpr (sizeof(real) == 4) {
-      if (a.mrhs) {   // split-fp16 B-operand tile of ok_apply_mrhs.cu (ok_internal.cuh: mrhs_W_index); fp64 -> fp32 -> (hi, lo)
-        __half* tile = reinterpret_cast<__half*>(W) + (size_t)n * kMrhsWSiteHalves;
-#pragma unroll
-        for (int j = 0; j < 3; ++j)   // columns 4j..4j+3 are 4 consecutive k: one 8-byte store per (part, piece)
-#pragma unroll
-          for (int part = 0; part < 2; ++part) {
-            __half hi[4], lo[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) mrhs_split((float)(part ? row[4 * j + i].y : row[4 * j + i].x), &hi[i], &lo[i]);
-            *reinterpret_cast<uint2*>(&tile[mrhs_W_index(term, r, 4 * j, part, 0)]) = *reinterpret_cast<const uint2*>(hi);
-            *reinterpret_cast<uint2*>(&tile[mrhs_W_index(term, r, 4 * j, part, 1)]) = *reinterpret_cast<const uint2*>(lo);
-          }
-        if (term == 0)   // zero pad k = 36..39 of the last stage: 192 halves per site, 16 per row r
-          for (int q = 0; q < 4; ++q) *reinterpret_cast<uint2*>(&tile[mrhs_W_pad_index(16 * r + 4 * q)]) = make_uint2(0u, 0u);
-        continue;
-      }
 #pragma unroll
       for (int c = 0; c < 6; ++c)
         dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
@@ -413,10 +398,9 @@ __global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __
   const int lane = threadIdx.x;
   const int idx = blockIdx.y * 3 + threadIdx.y;
   const int term = CLS == 0 ? (idx == 0 ? 0 : 6 + idx) : CLS == 1 ? 1 + idx : CLS == 2 ? 9 + idx : 15 + idx;
-  const int blk = blockIdx.x;
-  const int n = blk * kBlock + lane;
+  const int blk = blockIdx.x;                        // block inside the output buffer
+  const int n = (blk + a.blk0) * kBlock + lane;      // lattice site
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
-  if (a.mrhs && n >= a.g.V) return;   // the tile layout has no padded sites
   if (a.storage == OK_W_CONJ && term_is_neg(term)) return;   // rebuilt at apply time from term - 1 of the neighbour site
   if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units this term keeps
     using cx = typename WUnit<real>::cx;
@@ -457,9 +441,67 @@ __global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __
 #undef OK_ASM
 }
 
+// ------------------------------------------------------------------------- 12-RHS tile writer
+// The 12-RHS W tile of a site (ok_internal.cuh) interleaves the four terms of a K stage inside 16-byte core-matrix rows,
+// so a (site, term) thread would write 8-byte pieces 31 KB apart.  Instead the dense fp32 W of a chunk of blocks is
+// assembled into a bounce buffer (workspace) and this kernel turns (block, stage) = 32 sites x 4 terms into the split-fp16
+// tile image in shared memory and writes every site's 4608-byte stage chunk with coalesced 16-byte stores
+// (CTA = 16 sites x one stage, 74 KB of smem, 3 CTAs per SM).
+constexpr int kTileSiteStride = kMrhsStageHalves * 2 + 16;   // bytes per site in smem (+16: spreads the sites over banks)
+constexpr int kTileSites = 16;                                // sites per CTA (half a block): 3 CTAs per SM overlap their phases
+constexpr int kTileSmem = kTileSites * kTileSiteStride;       // 73 984
+constexpr int kBounceBlockBytes = kBlock * kTerms * 144 * 8;  // dense fp32 W of one 32-site block
+constexpr int kBounceBlocksMax = 2048;                        // 2 GB chunks at most
+
+constexpr int kTileThreads = 256;
+
+__global__ void __launch_bounds__(kTileThreads) mrhs_tile_kernel(const float4* __restrict__ dense, __half* __restrict__ tiles, int blk0, int V) {
+  extern __shared__ __align__(16) uint8_t sm[];
+  const int blk = blockIdx.x >> 1, half = blockIdx.x & 1, stage = blockIdx.y, tid = threadIdx.x;
+  const int nterm = stage < 6 ? 4 : 3;
+  if (stage == 6) {   // the pad k = 36..39 of the last stage stays zero
+    for (int i = tid; i < kTileSmem / 16; i += kTileThreads) reinterpret_cast<uint4*>(sm)[i] = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+  }
+  // 16 threads per dense row [term][row][unit] (one half of its 32 sites): thread <-> site; the two columns of a unit are adjacent k, so every
+  // (part, piece) is one 4-byte store into the site's tile image
+  const int lane = tid & (kTileSites - 1), grp = tid / kTileSites;
+  uint8_t* mine = sm + lane * kTileSiteStride;
+  for (int c = grp; c < nterm * 72; c += kTileThreads / kTileSites) {
+    const int u = c % 6, row = (c / 6) % 12, tl = c / 72;
+    const int term = 4 * stage + tl;
+    const float4 v = __ldcs(dense + (((size_t)blk * kTerms + term) * 12 + row) * 6 * kBlock + u * kBlock + half * kTileSites + lane);
+    int k;   // K position of column 2u inside the stage (ok_internal.cuh: mrhs_k); column 2u + 1 is k + 1
+    if (stage < 6) k = 16 * (u >> 1) + 4 * tl + 2 * (u & 1);
+    else { const int sq = 3 * tl + (u >> 1); k = 16 * (sq >> 2) + 4 * (sq & 3) + 2 * (u & 1); }
+    const int kofs = (k >> 3) * 384 + (k & 7);
+    const float vals[2][2] = {{v.x, v.z}, {v.y, v.w}};   // [part][column 2u, 2u + 1]
+#pragma unroll
+    for (int part = 0; part < 2; ++part) {
+      __half h0, l0, h1, l1;
+      mrhs_split(vals[part][0], &h0, &l0);
+      mrhs_split(vals[part][1], &h1, &l1);
+      const int w = mrhs_W_row(row, part);
+      *reinterpret_cast<__half2*>(mine + 2 * (kofs + (w >> 3) * 64 + (w & 7) * 8)) = __halves2half2(h0, h1);
+      *reinterpret_cast<__half2*>(mine + 2 * (kofs + ((w + 24) >> 3) * 64 + ((w + 24) & 7) * 8)) = __halves2half2(l0, l1);
+    }
+  }
+  __syncthreads();
+  const int units = (stage < 6 ? kMrhsStageHalves * 2 : kMrhsStageHalves * 2 - 768) / 16;   // the all-pad k chunk 5 of stage 6 is not stored
+  for (int i = tid; i < kTileSites * units; i += kTileThreads) {
+    const int s = i / units, q = i - s * units;
+    const long long n = (long long)(blk0 + blk) * kBlock + half * kTileSites + s;
+    if (n < V)
+      reinterpret_cast<uint4*>(tiles + n * kMrhsWSiteHalves + stage * kMrhsStageHalves)[q] = reinterpret_cast<const uint4*>(sm + s * kTileSiteStride)[q];
+  }
+}
+
+static int mrhs_bounce_blocks(const Geom& g) { return g.nblk < kBounceBlocksMax ? g.nblk : kBounceBlocksMax; }
+
 size_t precalc_work_bytes(const ok_params* p) {
   Geom g = make_geom(p);
-  return (size_t)6 * g.nblk * kBlock * sizeof(cm3);
+  const size_t fs = (size_t)6 * g.nblk * kBlock * sizeof(cm3);
+  return p->nrhs == 12 ? fs + 256 + (size_t)mrhs_bounce_blocks(g) * kBounceBlockBytes : fs;
 }
 
 int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) {
@@ -495,16 +537,38 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   OK_LAUNCHED("field_strength_kernel");
   const dim3 block(32, 3);
   const double2* lk = static_cast<const double2*>(links);
-#define OK_ASM_LAUNCH(CLS, NY)                                                                                              \
+#define OK_ASM_LAUNCH(CLS, NY, NB, OUT)                                                                                     \
   do {                                                                                                                      \
-    if (p->precision == OK_FP64) assemble_W_kernel<double, CLS><<<dim3(a.g.nblk, NY), block, 0, st>>>(lk, FS, static_cast<double2*>(Wp), a); \
-    else assemble_W_kernel<float, CLS><<<dim3(a.g.nblk, NY), block, 0, st>>>(lk, FS, static_cast<float4*>(Wp), a);          \
+    if (p->precision == OK_FP64) assemble_W_kernel<double, CLS><<<dim3(NB, NY), block, 0, st>>>(lk, FS, static_cast<double2*>(OUT), a); \
+    else assemble_W_kernel<float, CLS><<<dim3(NB, NY), block, 0, st>>>(lk, FS, static_cast<float4*>(OUT), a);               \
     OK_LAUNCHED("assemble_W_kernel");                                                                                       \
   } while (0)
-  OK_ASM_LAUNCH(1, 2);   // the heavy class first
-  OK_ASM_LAUNCH(0, 1);
-  OK_ASM_LAUNCH(2, 2);
-  OK_ASM_LAUNCH(3, 4);
+  a.blk0 = 0;
+  if (a.mrhs) {   // dense fp32 W of a chunk of blocks -> bounce buffer -> split-fp16 tiles (mrhs_tile_kernel)
+    static bool attr_set = false;
+    if (!attr_set) {
+      OK_CUDA(cudaFuncSetAttribute(mrhs_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSmem));
+      attr_set = true;
+    }
+    const size_t fs = ((size_t)6 * a.g.nblk * kBlock * sizeof(cm3) + 255) / 256 * 256;
+    void* bounce = static_cast<char*>(work) + fs;
+    const int cap = mrhs_bounce_blocks(a.g);
+    for (int b0 = 0; b0 < a.g.nblk; b0 += cap) {
+      const int nb = a.g.nblk - b0 < cap ? a.g.nblk - b0 : cap;
+      a.blk0 = b0;
+      OK_ASM_LAUNCH(1, 2, nb, bounce);
+      OK_ASM_LAUNCH(0, 1, nb, bounce);
+      OK_ASM_LAUNCH(2, 2, nb, bounce);
+      OK_ASM_LAUNCH(3, 4, nb, bounce);
+      mrhs_tile_kernel<<<dim3(2 * nb, kMrhsStages), kTileThreads, kTileSmem, st>>>(static_cast<const float4*>(bounce), static_cast<__half*>(Wp), b0, a.g.V);
+      OK_LAUNCHED("mrhs_tile_kernel");
+    }
+    return OK_SUCCESS;
+  }
+  OK_ASM_LAUNCH(1, 2, a.g.nblk, Wp);   // the heavy class first
+  OK_ASM_LAUNCH(0, 1, a.g.nblk, Wp);
+  OK_ASM_LAUNCH(2, 2, a.g.nblk, Wp);
+  OK_ASM_LAUNCH(3, 4, a.g.nblk, Wp);
 #undef OK_ASM_LAUNCH
   return OK_SUCCESS;
 }
