@@ -34,6 +34,7 @@ struct PrecalcArgs {
   int Vpad;
   int mrhs;                    // 1: write the nrhs = 12 tensor-core tile layout (ok_internal.cuh)
   int storage;                 // OK_W_DENSE / OK_W_BLOCK / OK_W_DS (ok_sparse.cuh)
+  int pair;                    // 1: the thread of a positive-direction term also writes the opposite term of the neighbour site
   int blk0;                    // first 32-site block of this launch (12-RHS: the dense W of a chunk goes to a bounce buffer)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
@@ -311,7 +312,7 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
   }
   P4 A, B;
   positive_blocks<fam, i, j>(x, links, FS, a, A, B);
-  if (neg) {   // Eqs. (2.3), (2.10): A -> A^dag, B -> -B^dag
+  auto conjugate = [&]() {   // Eqs. (2.3), (2.10): A -> A^dag, B -> -B^dag
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       A.c[k] = adj(A.c[k]);
@@ -319,7 +320,10 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
 #pragma unroll
       for (int q = 0; q < 9; ++q) B.c[k].e[q] = make_double2(-t.e[q].x, -t.e[q].y);
     }
-  }
+  };
+  if (neg) conjugate();
+  // writes W_term (built from the current A, B) of the site that sits at (blk, lane) of the output buffer
+  auto emit = [&](int term, bool neg, unit_t* Wt, int blk, int lane) {
   // block pattern: UL, LR use A (or 0); UR uses B; LL uses +-B
   const bool ulA = !(fam == 4 || fam == 5) && !(fam == 1 && !neg);
   const bool lrA = !(fam == 4 || fam == 5) && !(fam == 1 && neg);
@@ -385,6 +389,16 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
       for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
     }
   }
+  };   // emit
+  emit(term, neg, Wt, blk, lane);
+  if (a.pair && fam != 0 && !neg) {
+    // the opposite-direction matrix of the site x + offset(term) is the conjugate of this one: W^-_o(y) from W^+_o(y - o)
+    Site y = x;
+    for (int mu = 0; mu < 4; ++mu) y = shift(y, mu, c_poff[term][mu], a.g);
+    const int n2 = index_of(y, a.g), blk2 = n2 >> 5, lane2 = n2 & 31;
+    conjugate();
+    emit(term + 1, true, W + ((size_t)blk2 * kTerms + term + 1) * 12 * NC * kBlock + lane2, blk2, lane2);
+  }
 }
 
 
@@ -402,19 +416,22 @@ __global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __
   const int n = (blk + a.blk0) * kBlock + lane;      // lattice site
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
   if (a.storage == OK_W_CONJ && term_is_neg(term)) return;   // rebuilt at apply time from term - 1 of the neighbour site
-  if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units this term keeps
+  if (a.pair && term_is_neg(term)) return;                   // written by the thread of term - 1 of the neighbour site
+  const int nzero = (a.pair && term > 0) ? 2 : 1;            // padded site: this term (and its partner) are zero
+  if (n >= a.g.V && a.storage != OK_W_DENSE) {   // padded site, reduced format: zero the units the terms keep
     using cx = typename WUnit<real>::cx;
     cx* Ws = reinterpret_cast<cx*>(W) + (size_t)blk * sparse_site_units_rt(a.storage) * kBlock + lane;
-    for (int r = 0; r < 12; ++r)
-      for (int col = 0; col < 12; ++col) {
-        const SparseRef ref = sparse_ref(a.storage, term, r, col, c_qrun[a.storage - 1]);
-        if (ref.unit >= 0 && ref.stored) Ws[(size_t)ref.unit * kBlock] = cx{};
-      }
+    for (int tz = term; tz < term + nzero; ++tz)
+      for (int r = 0; r < 12; ++r)
+        for (int col = 0; col < 12; ++col) {
+          const SparseRef ref = sparse_ref(a.storage, tz, r, col, c_qrun[a.storage - 1]);
+          if (ref.unit >= 0 && ref.stored) Ws[(size_t)ref.unit * kBlock] = cx{};
+        }
     return;
   }
   if (n >= a.g.V) {   // padded site: zeros
     unit_t z = {};
-    for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
+    for (int u = 0; u < 12 * NC * nzero; ++u) Wt[(size_t)u * kBlock] = z;
     return;
   }
   // term -> family, directions, sign of the hop (term order of ok.h)
@@ -518,6 +535,7 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   a.Vpad = a.g.nblk * kBlock;
   a.mrhs = p->nrhs == 12;
   a.storage = p->storage;
+  a.pair = (p->nrhs == 1 && p->storage != OK_W_CONJ) ? 1 : 0;   // 12-RHS assembles chunk by chunk: the partner site may be outside
   const double u0 = p->u0, u2 = u0 * u0, u3 = u2 * u0, u4 = u2 * u2;
   a.mass = u0 / (2.0 * p->kappa);
   a.d0 = -(p->cB * p->zeta + 16.0 * p->c5) / (2.0 * u3);
