@@ -35,6 +35,7 @@ struct PrecalcArgs {
   int mrhs;                    // 1: write the nrhs = 12 tensor-core tile layout (ok_internal.cuh)
   int storage;                 // OK_W_DENSE / OK_W_BLOCK / OK_W_DS (ok_sparse.cuh)
   int pair;                    // 1: the thread of a positive-direction term also writes the opposite term of the neighbour site
+  int posonly;                 // 1: grid over W^0 and the 13 positive-direction terms only (pair, or OK_W_CONJ)
   int blk0;                    // first 32-site block of this launch (12-RHS: the dense W of a chunk goes to a bounce buffer)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
@@ -411,7 +412,14 @@ __global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __
   constexpr int NC = WUnit<real>::NC;
   const int lane = threadIdx.x;
   const int idx = blockIdx.y * 3 + threadIdx.y;
-  const int term = CLS == 0 ? (idx == 0 ? 0 : 6 + idx) : CLS == 1 ? 1 + idx : CLS == 2 ? 9 + idx : 15 + idx;
+  // a.posonly: the grid covers W^0 and the positive-direction terms only (their threads write or imply the opposite ones)
+  int term;
+  if (a.posonly) {
+    term = CLS == 0 ? (idx == 0 ? 0 : 7) : CLS == 1 ? 1 + 2 * idx : CLS == 2 ? 9 + 2 * idx : 15 + 2 * idx;
+    if (CLS == 0 && idx > 1) return;
+  } else {
+    term = CLS == 0 ? (idx == 0 ? 0 : 6 + idx) : CLS == 1 ? 1 + idx : CLS == 2 ? 9 + idx : 15 + idx;
+  }
   const int blk = blockIdx.x;                        // block inside the output buffer
   const int n = (blk + a.blk0) * kBlock + lane;      // lattice site
   unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
@@ -536,6 +544,7 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   a.mrhs = p->nrhs == 12;
   a.storage = p->storage;
   a.pair = (p->nrhs == 1 && p->storage != OK_W_CONJ) ? 1 : 0;   // 12-RHS assembles chunk by chunk: the partner site may be outside
+  a.posonly = (a.pair || p->storage == OK_W_CONJ) ? 1 : 0;
   const double u0 = p->u0, u2 = u0 * u0, u3 = u2 * u0, u4 = u2 * u2;
   a.mass = u0 / (2.0 * p->kappa);
   a.d0 = -(p->cB * p->zeta + 16.0 * p->c5) / (2.0 * u3);
@@ -583,10 +592,10 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
     }
     return OK_SUCCESS;
   }
-  OK_ASM_LAUNCH(1, 2, a.g.nblk, Wp);   // the heavy class first
+  OK_ASM_LAUNCH(1, (a.posonly ? 1 : 2), a.g.nblk, Wp);   // the heavy class first
   OK_ASM_LAUNCH(0, 1, a.g.nblk, Wp);
-  OK_ASM_LAUNCH(2, 2, a.g.nblk, Wp);
-  OK_ASM_LAUNCH(3, 4, a.g.nblk, Wp);
+  OK_ASM_LAUNCH(2, (a.posonly ? 1 : 2), a.g.nblk, Wp);
+  OK_ASM_LAUNCH(3, (a.posonly ? 2 : 4), a.g.nblk, Wp);
 #undef OK_ASM_LAUNCH
   return OK_SUCCESS;
 }
