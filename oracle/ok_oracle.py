@@ -16,11 +16,13 @@ What it computes, and the passage each function follows:
   bicgstab_mixed     mixed-precision inversion: defect correction around    PAPER.md:114 ("mixed precision inversion by calling
                      a low-precision bicgstab                               the inverter ... in single or double precision") ; R-MIXED
   dense_M            brute-force matrix of M (tiny lattices only)           PAPER.md:43-47, Eq. (2.1)
+  gamma5_mul, cgnr   CG on M^dag M with M^dag = Gamma_5 M Gamma_5           PAPER.md:164 (future work there) ; pin P9
 
 Pins (tests/test_oracle_*.py, all -m "not gpu"): direct == W form (P1); free-field closed
 form and plane-wave eigen-relation (P2); gauge covariance (P3); gamma5-hermiticity and
 Eqs. (2.3)/(2.10) (P4); hand-coded Wilson / Wilson-clover special cases (P5); zero-block
-structure (P6); dense LU vs BiCGStab (P7); staple content of the c5 hop term (Eq. 2.8's 1/4).
+structure (P6); dense LU vs BiCGStab (P7); staple content of the c5 hop term (Eq. 2.8's 1/4);
+mixed-precision defect correction vs dense LU (P8); CG on the normal equations and Gamma_5 M Gamma_5 = M^dag (P9).
 Parity unpinned (conventions with no printed value to check, shared as input spec):
 trace subtraction in F (none), the Pauli basis, the coefficient values, sign E_i = F_4i.
 
