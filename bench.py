@@ -376,13 +376,13 @@ def run_ours(args, wl):
             "gpu_launches": int(launches), "clocks": clocks,
         }
         if nrhs == 12:
-            # tensor-pipe report for the multi-RHS mode (north_star): per site 21 tcgen05.mma of M=128, N=48, K=16 (24 cycles
+            # tensor-pipe report for the multi-RHS mode (north_star): per site 21 tcgen05.mma of M=64, N=48, K=16 (24 cycles
             # each on one SM's tensor pipe, measured), i.e. 504 busy cycles per site; useful flops are the complex contraction's
             sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
             busy = 21 * 24 * (V / 148.0) / (a_ms * 1e-3 * sm_mhz * 1e6)
             line["tensor"] = {"kind": "tcgen05.mma.kind::f16 (fp16 hi/lo split of fp32 operands), fp32 accumulate in TMEM",
-                              "mma_per_site": 21, "mma_shape": [128, 48, 16], "pipe_busy_frac_est": busy,
-                              "issued_tflops": world * V * 21 * 2 * 128 * 48 * 16 / (a_ms * 1e-3) / 1e12,
+                              "mma_per_site": 21, "mma_shape": [64, 48, 16], "pipe_busy_frac_est": busy,
+                              "issued_tflops": world * V * 21 * 2 * 64 * 48 * 16 / (a_ms * 1e-3) / 1e12,
                               "useful_tflops": world * V * FLOP_PER_SITE * nrhs / (a_ms * 1e-3) / 1e12,
                               "note": "the mode is HBM-bound (W streams once for 12 columns); ncu sm__pipe_tensor_cycles_active: profiles/"}
         if mixed is not None:

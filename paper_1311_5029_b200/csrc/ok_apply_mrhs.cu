@@ -7,7 +7,7 @@
 //   Out_r = D(psi_r, W_r) - D(psi_i, W_i),  Out_i = D(psi_i, W_r) + D(psi_r, W_i)             (epilogue).
 // Precision: every fp32 operand is carried as two fp16 pieces x = hi + lo / 2048 (22 significant bits; the
 // spinor is first scaled per right-hand side by a power of two so that |x| < 2^15).  hi and lo are STACKED
-// as rows on both sides, A = [Psi_hi ; Psi_lo] (48 rows of M = 128), B = [W_hi ; W_lo] (N = 48), so one series
+// as rows on both sides, A = [Psi_hi ; Psi_lo] (48 rows of M = 64), B = [W_hi ; W_lo] (N = 48), so one series
 // of 21 tcgen05.mma.kind::f16 (K = 16) per site yields all four products; the epilogue folds them with the
 // weights 1, 2^-11, 2^-11, 2^-22 in fp32.  W is stored pre-split in HBM (4 bytes per real, like fp32), so it
 // goes HBM -> shared memory -> tensor core with no thread touching it.
@@ -20,7 +20,7 @@
 //              of a stage (three 16-B loads per thread, L1/L2), scale, split into fp16 hi/lo and write rows g
 //              (hi) and g + 8 (lo) with tcgen05.st.16x256b into a 16-slot ring of 24 TMEM columns.
 //   MMA        1 thread: 3 tcgen05.mma (A from tensor memory, B from smem) per stage into one of two
-//              128-lane x 48-column fp32 accumulators; tcgen05.commit frees the stage / the W slot.
+//              64-row x 48-column fp32 accumulators; tcgen05.commit frees the stage / the W slot.
 //   epilogue   3 warps (one per lane quarter): tcgen05.ld.16x256b, fold pieces, combine Re/Im, coalesced stores.
 //   index      1 warp: the 27 neighbour site indices of upcoming sites into a small smem ring.
 // A first small kernel finds max |psi| per right-hand side (the power-of-two scales).
@@ -53,8 +53,9 @@ constexpr int kSmemW = kWSlots * kWSlotBytes;       // 129 024
 constexpr int kSmemNbr = kNbrRing * 32 * 4;
 constexpr int kSmemBytes = kSmemW + kSmemNbr;
 
-// D f32, A f16, B f16, both K-major, N = 48, M = 128
-constexpr uint32_t kIdesc = (1u << 4) | (0u << 7) | (0u << 10) | ((48u >> 3) << 17) | ((128u >> 4) << 24);
+// D f32, A f16, B f16, both K-major, N = 48, M = 64: row r of A and D sits in TMEM lane 32 (r / 16) + r % 16, i.e. the 16 lanes
+// (8 hi + 8 lo rows) each of the three producer quarters fills; M = 128 costs the same 24 cycles but reads 128 lanes
+constexpr uint32_t kIdesc = (1u << 4) | (0u << 7) | (0u << 10) | ((48u >> 3) << 17) | ((64u >> 4) << 24);
 
 struct Bars {
   uint64_t afull[kARing], aempty[kARing], wfull[kWSlots], wempty[kWSlots], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
