@@ -22,6 +22,11 @@
  *   - There is no CPU fallback: without a CUDA device every compute call returns OK_ECUDA.
  *   - One device and one calling thread per process (the model is one process per GPU): the stream, the workspace,
  *     the W handle table and a few device-side scratch symbols are process-wide state, not per-call arguments.
+ *     The library binds to the CUDA device that is current at its first compute call; a later call on another
+ *     device returns OK_EINVAL (its constant tables live on the bound device only).
+ *   - Errors of a kernel that faults while running surface at the next synchronising call.  With the environment
+ *     variable OK_SYNC_CHECK=1 every launch is followed by a stream synchronisation, so OK_ECUDA names the kernel
+ *     that faulted (debugging aid; serialises the stream).
  *
  * Canonical (external) layouts, complex numbers interleaved (re, im):
  *   site index   n = x + Lx*(y + Ly*(z + Lz*t)),  dims = {Lx, Ly, Lz, T};  V = Lx*Ly*Lz*T
@@ -47,7 +52,12 @@
  *   OK_W_BLOCK / OK_W_DS: header, then [block][unit][site_in_block][complex]; the unit order is the list of
  *           stored colour-block rows in csrc/ok_sparse.cuh.  ok_pack_W drops what the format does not keep
  *           (OK_W_DS keeps UL (else LR) as D and UR as S); ok_unpack_W rebuilds the full 12 x 12 matrices.
- *   nrhs=12 (fp32, OK_W_DENSE only): spinor = per-site records [component/4][2*rhs+part][component%4] (1152 B);
+ *   nrhs=12 (fp32, OK_W_DENSE only): spinor = 256-byte header, then per-site fp32 records [component/4][2*rhs+part][component%4]
+ *           (1152 B, the field), then per-site tensor-core operand records (1152 B: the same numbers scaled per right-hand
+ *           side by a power of two and split into two fp16 pieces).  The operand records are what ok_dirac_apply reads; they
+ *           are written by ok_pack_spinor and by the solver for its own vectors, and rebuilt on demand (two passes over the
+ *           field) when ok_dirac_apply is given a field whose header says they are stale, e.g. the `out` of an earlier
+ *           apply.  Never write such a buffer except through this library.
  *           W = per-site split-fp16 tensor-core tiles (31 488 B), see csrc/ok_internal.cuh.
  *   Use ok_pack_ and ok_unpack_ to convert; the sizes are given by ok_vec_bytes and ok_W_bytes.
  */
@@ -125,7 +135,9 @@ int ok_unpack_W(const void* W, void* canon_W);
 int ok_precalc_W(const void* links, const ok_params* params, void* W);
 
 /* Dirac apply, PAPER.md:53-55 (Eq. 2.2): out = M psi.  psi, out: internal spinor layout,
- * out must not alias psi.  Dimensions/precision are taken from W's header. */
+ * out must not alias psi.  Dimensions/precision are taken from W's header.
+ * nrhs = 12: psi's operand records are brought up to date first if its header marks them stale (the buffer behind the
+ * const pointer is written in that case); out gets fp32 records only. */
 int ok_dirac_apply(const void* W, const void* psi, void* out);
 
 /* BiCGStab: solves M x = src (x0 = 0; x on entry ignored), unpreconditioned,
@@ -163,12 +175,17 @@ int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x
 int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host);
 
 /* ---- diagnostics -------------------------------------------------------------------------- */
-/* Read the parameters stored in W's header back into *p (HOST). */
+/* Read the parameters stored in W's header back into *p (HOST).  Always reads the 1 KiB device header (synchronises the
+ * stream) and refreshes the library's host-side record of W from it. */
 int ok_W_params(const void* W, ok_params* p);
 /* Drop the library's host-side record of W (the header mirror that lets the three main calls run
  * without a params argument and without reading the device).  Call it before freeing the buffer or
  * reusing its memory for anything else; a later W written there by ok_precalc_W / ok_pack_W is
- * recorded again.  Unknown pointers are ignored.  Returns OK_SUCCESS. */
+ * recorded again.  Unknown pointers are ignored.  Returns OK_SUCCESS.
+ * Hazard this guards against: the record, not the device header, decides which kernels run.  ok_precalc_W / ok_pack_W
+ * drop every record whose byte range overlaps the W they write, so reusing memory THROUGH the library is safe; a W
+ * buffer overwritten by a plain device copy (say a checkpoint restore with other dims or storage) must be followed by
+ * ok_forget_W or ok_W_params, which re-reads the header. */
 int ok_forget_W(const void* W);
 /* Layout query for the reduced storage formats (pure host arithmetic, no device needed): where element (row, col) of
  * W_term is kept.  Returns the complex-unit index inside a site's OK_W_BLOCK / OK_W_DS / OK_W_CONJ record
@@ -179,8 +196,6 @@ int ok_forget_W(const void* W);
 int ok_W_unit_index(int storage, int term, int row, int col, int* info);
 /* Number of kernels the library has launched since load (for launch accounting in benches). */
 uint64_t ok_launch_count(void);
-/* Select the apply kernel variant (0 = default).  Tuning knob; results are identical. */
-int ok_set_apply_variant(int variant);
 const char* ok_strerror(int status);
 const char* ok_version(void);
 

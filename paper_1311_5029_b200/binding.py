@@ -56,7 +56,6 @@ EXPORTS = {
     "ok_W_params": (C.c_int, [C.c_void_p, C.POINTER(ok_params)]),
     "ok_forget_W": (C.c_int, [C.c_void_p]),
     "ok_launch_count": (C.c_uint64, []),
-    "ok_set_apply_variant": (C.c_int, [C.c_int]),
     "ok_strerror": (C.c_char_p, [C.c_int]),
     "ok_version": (C.c_char_p, []),
 }
@@ -219,10 +218,6 @@ def ok_forget_W(W):
 
 def ok_launch_count():
     return int(lib().ok_launch_count())
-
-
-def ok_set_apply_variant(v):
-    _check(lib().ok_set_apply_variant(int(v)), "ok_set_apply_variant")
 
 
 # ------------------------------------------------------------------ device-memory helpers (torch)

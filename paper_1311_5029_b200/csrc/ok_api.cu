@@ -1,6 +1,8 @@
 // C-ABI entry points of libokdirac (include/ok.h): argument checks, sizes, handle table.
 // Every step of the hot path runs in the CUDA kernels of the other translation units.
+#include <iterator>
 #include <mutex>
+#include <stdlib.h>
 #include <string.h>
 #include <unordered_map>
 
@@ -20,7 +22,24 @@ const int8_t kOffsets[kTerms][4] = {
 
 Ctx& ctx() {
   static Ctx c;
+  static bool init = [] {
+    const char* e = getenv("OK_SYNC_CHECK");
+    c.sync_check = e && e[0] == '1';
+    return true;
+  }();
+  (void)init;
   return c;
+}
+
+int bind_device() {
+  int dev = -1;
+  OK_CUDA(cudaGetDevice(&dev));
+  if (ctx().device < 0) ctx().device = dev;
+  if (ctx().device != dev) {
+    snprintf(ctx().err, sizeof(ctx().err), "libokdirac is bound to CUDA device %d; this call arrived on device %d", ctx().device, dev);
+    return OK_EINVAL;
+  }
+  return OK_SUCCESS;
 }
 
 int fail_cuda(cudaError_t e, const char* where) {
@@ -67,12 +86,36 @@ static std::unordered_map<const void*, ok_params> g_table;
 
 int remember_W(const void* W, const ok_params* p) {
   std::lock_guard<std::mutex> lk(g_mu);
+  // a W written here invalidates every record whose bytes it overwrites (a buffer handed out again by a caching
+  // allocator without ok_forget_W, or a W carved out of a larger arena)
+  const uintptr_t lo = reinterpret_cast<uintptr_t>(W), hi = lo + ok_W_bytes(p);
+  for (auto it = g_table.begin(); it != g_table.end();) {
+    const uintptr_t a = reinterpret_cast<uintptr_t>(it->first), b = a + ok_W_bytes(&it->second);
+    it = (a < hi && lo < b) ? g_table.erase(it) : std::next(it);
+  }
   g_table[W] = *p;
+  return OK_SUCCESS;
+}
+
+int refresh_W(const void* W, ok_params* p) {
+  if (!aligned16(W)) return OK_EINVAL;
+  WHeader h;
+  OK_CUDA(cudaMemcpyAsync(&h, W, sizeof(h), cudaMemcpyDeviceToHost, ctx().stream));
+  OK_CUDA(cudaStreamSynchronize(ctx().stream));
+  if (h.magic != kMagic || !valid_params(&h.p) || h.layout != layout_id(&h.p)) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_table.erase(W);
+    return OK_EINVAL;
+  }
+  remember_W(W, &h.p);
+  *p = h.p;
   return OK_SUCCESS;
 }
 
 int lookup_W(const void* W, ok_params* p) {
   if (!aligned16(W)) return OK_EINVAL;
+  int st = bind_device();
+  if (st) return st;
   {
     std::lock_guard<std::mutex> lk(g_mu);
     auto it = g_table.find(W);
@@ -81,14 +124,7 @@ int lookup_W(const void* W, ok_params* p) {
       return OK_SUCCESS;
     }
   }
-  WHeader h;
-  OK_CUDA(cudaMemcpyAsync(&h, W, sizeof(h), cudaMemcpyDeviceToHost, ctx().stream));
-  OK_CUDA(cudaStreamSynchronize(ctx().stream));
-  if (h.magic != kMagic || !valid_params(&h.p)) return OK_EINVAL;
-  if (h.layout != layout_id(&h.p)) return OK_EINVAL;
-  remember_W(W, &h.p);
-  *p = h.p;
-  return OK_SUCCESS;
+  return refresh_W(W, p);
 }
 
 static int write_header(void* W, const ok_params* p) {
@@ -114,7 +150,9 @@ extern "C" {
 size_t ok_vec_bytes(const ok_params* p) {
   if (!valid_params(p)) return 0;
   Geom g = make_geom(p);
-  return (size_t)g.nblk * kBlock * 12 * 2 * real_bytes(p) * (size_t)p->nrhs;
+  if (p->nrhs == 12)   // header + fp32 records + tensor-core operand records (ok_internal.cuh)
+    return (kMrhsVecHeaderBytes + (size_t)g.V * (kMrhsVecSiteFloats * 4 + kMrhsOpSiteHalves * 2) + 255) / 256 * 256;
+  return (size_t)g.nblk * kBlock * 12 * 2 * real_bytes(p);
 }
 
 size_t ok_W_bytes(const ok_params* p) {
@@ -146,27 +184,25 @@ int ok_set_workspace(void* dev, size_t bytes) {
   return OK_SUCCESS;
 }
 
-int ok_set_apply_variant(int v) {
-  if (v < 0 || v > 63) return OK_EINVAL;
-  ctx().apply_variant = v;
-  return OK_SUCCESS;
-}
-
 uint64_t ok_launch_count(void) { return ctx().launches; }
 
 int ok_pack_spinor(const ok_params* p, const void* canon, void* packed) {
   if (!valid_params(p) || !aligned16(canon) || !aligned16(packed)) return OK_EINVAL;
+  if (int st = bind_device()) return st;
   return launch_pack_spinor(p, canon, packed, false);
 }
 
 int ok_unpack_spinor(const ok_params* p, const void* packed, void* canon) {
   if (!valid_params(p) || !aligned16(canon) || !aligned16(packed)) return OK_EINVAL;
+  if (int st = bind_device()) return st;
   return launch_pack_spinor(p, canon, const_cast<void*>(packed), true);
 }
 
 int ok_pack_W(const ok_params* p, const void* canon, void* W) {
   if (!valid_params(p) || !aligned16(canon) || !aligned16(W)) return OK_EINVAL;
-  int st = write_header(W, p);
+  int st = bind_device();
+  if (st) return st;
+  st = write_header(W, p);
   if (st) return st;
   return launch_pack_W(p, canon, W_payload(W), false);
 }
@@ -187,13 +223,17 @@ int ok_forget_W(const void* W) {
 
 int ok_W_params(const void* W, ok_params* p) {
   if (!p) return OK_EINVAL;
-  return lookup_W(W, p);
+  int st = bind_device();
+  if (st) return st;
+  return refresh_W(W, p);   // always from the device header, so a W refilled behind the library's back is seen
 }
 
 int ok_precalc_W(const void* links, const ok_params* p, void* W) {
   if (!valid_params(p) || !aligned16(links) || !aligned16(W)) return OK_EINVAL;
   if (!ctx().work || ctx().work_bytes < precalc_work_bytes(p)) return OK_EWORKSPACE;
-  int st = write_header(W, p);
+  int st = bind_device();
+  if (st) return st;
+  st = write_header(W, p);
   if (st) return st;
   return launch_precalc(p, links, W_payload(W), ctx().work);
 }
@@ -203,7 +243,7 @@ int ok_dirac_apply(const void* W, const void* psi, void* out) {
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
-  if (p.nrhs == 12) return launch_apply_mrhs(&p, W_payload(W), psi, out);
+  if (p.nrhs == 12) return mrhs_apply_vec(&p, W_payload(W), const_cast<void*>(psi), out);
   return launch_apply(&p, W_payload(W), psi, out, nullptr, nullptr, nullptr);
 }
 
@@ -220,7 +260,7 @@ int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host) {
   char *canon_in = w, *packed_in = w + vb, *packed_out = w + 2 * vb, *canon_out = w + 3 * vb;
   OK_CUDA(cudaMemcpyAsync(canon_in, psi_host, cb, cudaMemcpyHostToDevice, ctx().stream));
   if ((st = launch_pack_spinor(&p, canon_in, packed_in, false))) return st;
-  st = p.nrhs == 12 ? launch_apply_mrhs(&p, W_payload(W), packed_in, packed_out)
+  st = p.nrhs == 12 ? mrhs_apply_vec(&p, W_payload(W), packed_in, packed_out)
                     : launch_apply(&p, W_payload(W), packed_in, packed_out, nullptr, nullptr, nullptr);
   if (st) return st;
   if ((st = launch_pack_spinor(&p, canon_out, packed_out, true))) return st;

@@ -158,17 +158,7 @@ static int launch_direct(const Geom& g, const void* W, const void* psi, void* ou
   return OK_SUCCESS;
 }
 
-template <typename real>
-static int dispatch(int variant, const Geom& g, const void* W, const void* psi, void* out, double* partials,
-                    const void* dot_a) {
-  switch (variant) {
-    case 1: return launch_direct<real, 2>(g, W, psi, out, partials, dot_a);
-    case 2: return launch_direct<real, 4>(g, W, psi, out, partials, dot_a);
-    case 3: return launch_direct<real, 6>(g, W, psi, out, partials, dot_a);
-    case 4: return launch_direct<real, 1>(g, W, psi, out, partials, dot_a);
-    default: return launch_direct<real, 3>(g, W, psi, out, partials, dot_a);
-  }
-}
+constexpr int kRowsPerWarp = 3;   // 4 warps per CTA, 40 registers: the measured optimum (profiles/r01_apply.md)
 
 int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, double* partials,
                  const void* dot_a, const void* /*unused*/) {
@@ -177,8 +167,8 @@ int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, 
   int st = upload_offsets();
   if (st) return st;
   Geom g = make_geom(p);
-  if (p->precision == OK_FP64) return dispatch<double>(ctx().apply_variant, g, W, psi, out, partials, dot_a);
-  return dispatch<float>(ctx().apply_variant, g, W, psi, out, partials, dot_a);
+  if (p->precision == OK_FP64) return launch_direct<double, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
+  return launch_direct<float, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
 }
 
 }  // namespace okd

@@ -7,58 +7,68 @@
 //   Out_r = D(psi_r, W_r) - D(psi_i, W_i),  Out_i = D(psi_i, W_r) + D(psi_r, W_i)             (epilogue).
 // Precision: every fp32 operand is carried as two fp16 pieces x = hi + lo / 2048 (22 significant bits; the
 // spinor is first scaled per right-hand side by a power of two so that |x| < 2^15).  hi and lo are STACKED
-// as rows on both sides, A = [Psi_hi ; Psi_lo] (48 rows of M = 64), B = [W_hi ; W_lo] (N = 48), so one series
-// of 21 tcgen05.mma.kind::f16 (K = 16) per site yields all four products; the epilogue folds them with the
-// weights 1, 2^-11, 2^-11, 2^-22 in fp32.  W is stored pre-split in HBM (4 bytes per real, like fp32), so it
-// goes HBM -> shared memory -> tensor core with no thread touching it.
+// as rows on both sides, A = [Psi_hi ; Psi_lo], B = [W_hi ; W_lo] (N = 48), so one series of 21
+// tcgen05.mma.kind::f16 (K = 16) per site yields all four products; the epilogue folds them with the
+// weights 1, 2^-11, 2^-11, 2^-22 in fp32.
 //
-// One persistent CTA per SM, 20 specialised warps; sites are dealt in runs of consecutive x (L1 reuse of the
-// gathered spinor records), runs round-robin over the CTAs (so all CTAs sweep the lattice together and the
-// records stay in L2).  Per site 7 K-stages of 4 stencil terms (48 k = 24 TMEM columns):
-//   W loader   1 thread: one 31 488-B bulk copy (cp.async.bulk, L2 evict-first) per site into a 4-slot smem ring.
-//   A producers 12 warps (4 per TMEM lane quarter, quarter q = rows n = 8q..8q+7): gather the 4 neighbour records
-//              of a stage (three 16-B loads per thread, L1/L2), scale, split into fp16 hi/lo and write rows g
-//              (hi) and g + 8 (lo) with tcgen05.st.16x256b into a 16-slot ring of 24 TMEM columns.
-//   MMA        1 thread: 3 tcgen05.mma (A from tensor memory, B from smem) per stage into one of two
-//              64-row x 48-column fp32 accumulators; tcgen05.commit frees the stage / the W slot.
-//   epilogue   3 warps (one per lane quarter): tcgen05.ld.16x256b, fold pieces, combine Re/Im, coalesced stores.
-//   index      1 warp: the 27 neighbour site indices of upcoming sites into a small smem ring.
-// A first small kernel finds max |psi| per right-hand side (the power-of-two scales).
-// Layouts of W and of the spinor records: ok_internal.cuh.
+// BOTH operands are kept pre-split in HBM (4 bytes per real, like fp32; layouts in ok_internal.cuh):
+//   W   per-site UMMA tile, HBM -> shared memory by one bulk copy, read by the tensor core; no thread touches it.
+//   Psi per-site operand record written by whoever produced the vector (ok_pack_spinor, the BiCGStab update
+//       kernels, mrhs_ensure_operand).  The producer warps only MOVE it: 8-byte loads with lane <-> A row (192
+//       contiguous bytes per warp load, 2-3 L1 wavefronts) straight into tensor memory with tcgen05.st.32x32b --
+//       no conversion arithmetic, no column-maximum pass in the apply.
+//
+// One persistent CTA per SM, 18 warps; sites are dealt in runs of consecutive x (L1 reuse of the gathered records),
+// runs round-robin over the CTAs (all CTAs sweep the lattice together, so the records stay in L2).  Per site 7
+// K-stages of 4 stencil terms (48 k = 24 TMEM columns):
+//   W loader    1 thread: one 31 488-B bulk copy (cp.async.bulk, L2 evict-first) per site into a 4-slot smem ring.
+//   A producers 8 warps, 4 per TMEM lane quarter (quarter q holds the rows of n = 12q .. 12q+11): gather the 4
+//               neighbour records of a stage (12 LDG.64 per lane), three stages in flight, 3 x tcgen05.st.32x32b.x8
+//               into a 16-slot ring of 24 TMEM columns.
+//   MMA         1 thread: 3 tcgen05.mma (M = 128: A rows = TMEM lanes; A from tensor memory, B from smem) per stage
+//               into one of two 48-column fp32 accumulators; tcgen05.commit frees the stage / the W slot.
+//   epilogue    2 warps (one per lane quarter): tcgen05.ld.16x256b (hi and lo row of an n in one thread), fold the
+//               pieces, combine Re/Im with one shuffle, coalesced 128-B stores; optionally the per-column reductions
+//               <a, out>, ||out||^2 of BiCGStab in fp64 with a fixed order.
+//   index       1 warp: the 27 neighbour site indices of upcoming sites into a small smem ring.
 #include "ok_internal.cuh"
 
 namespace okd {
 
 __constant__ int8_t c_moff[kTerms][4];
-__device__ unsigned g_colmax[12];   // bit patterns of max |psi| per right-hand side (atomicMax on non-negative floats)
 static bool g_mrhs_ready = false;
+static int g_sm_count = 0;
 
 namespace {
 
-constexpr int kG = 4;                               // producer warps per lane quarter
-constexpr int kARing = 16;                          // A ring slots
-constexpr int kACols = 24;                          // TMEM columns per slot (48 fp16 k)
+constexpr int kG = 4;                               // producer warps per lane quarter: (site slot 0/1) x (stages 0-3 / 4-6)
+constexpr int kASites = 2;                          // A ring: two whole sites
+constexpr int kACols = 24;                          // TMEM columns per stage (48 fp16 k)
+constexpr int kASiteCols = kMrhsStages * kACols;    // 168
 constexpr int kWSlots = 4;                          // W ring (sites)
 constexpr int kWSlotBytes = kMrhsStages * kMrhsStageHalves * 2;   // 32 256 (the last 768 B stay zero)
-constexpr int kDCol0 = kARing * kACols;             // 384: accumulator 0; accumulator 1 at +64
+constexpr int kDCol0 = 384;                         // accumulator 0; accumulator 1 at +64 (A uses columns 0..335)
 constexpr int kTmemCols = 512;
 constexpr int kNbrRing = 8;
 constexpr int kSBO = 128, kLBO = 768;
 
-constexpr int kWarpMma = 3, kWarpTma = 7, kWarpIdx = 11, kWarpEpi = 4 * kG;   // warps 4i + 3 are free of TMEM lane duty
-constexpr int kWarps = 4 * kG + 4, kThreads = kWarps * 32;
-static_assert(kG >= 3 && kG <= 7, "producer groups");
+// warp w may touch TMEM lanes 32 (w % 4) ..; the A rows live in quarters 0 and 1
+constexpr int kWarpMma = 2, kWarpTma = 3, kWarpIdx = 6, kWarpEpi = 4 * kG;
+constexpr int kWarps = 4 * kG + 2, kThreads = kWarps * 32;
+static_assert(kG == 2 * kASites && kASites * kASiteCols <= kDCol0, "A ring layout");
 
 constexpr int kSmemW = kWSlots * kWSlotBytes;       // 129 024
 constexpr int kSmemNbr = kNbrRing * 32 * 4;
 constexpr int kSmemBytes = kSmemW + kSmemNbr;
 
-// D f32, A f16, B f16, both K-major, N = 48, M = 64: row r of A and D sits in TMEM lane 32 (r / 16) + r % 16, i.e. the 16 lanes
-// (8 hi + 8 lo rows) each of the three producer quarters fills; M = 128 costs the same 24 cycles but reads 128 lanes
-constexpr uint32_t kIdesc = (1u << 4) | (0u << 7) | (0u << 10) | ((48u >> 3) << 17) | ((64u >> 4) << 24);
+// D f32, A f16, B f16, both K-major, N = 48, M = 128: row r of A and D = TMEM lane r (rows 64..127 are never written or read;
+// M = 64 costs the same 24 cycles but uses only the lower 16 lanes of a quarter)
+constexpr uint32_t kIdesc = (1u << 4) | (0u << 7) | (0u << 10) | ((48u >> 3) << 17) | ((128u >> 4) << 24);
 
+// Every barrier is waited on, phase after phase, by the same threads: a try_wait by parity cannot tell phase u from phase
+// u - 2, so a warp that skipped a phase of a barrier (a slot that other warps fill in between) could pass early.
 struct Bars {
-  uint64_t afull[kARing], aempty[kARing], wfull[kWSlots], wempty[kWSlots], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
+  uint64_t afull[kASites], aempty[kASites], wfull[kWSlots], wempty[kWSlots], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -99,21 +109,6 @@ __device__ __forceinline__ int wrapc(int x, int L) {
   return x;
 }
 
-__device__ __forceinline__ uint32_t pack_h2(float lo_elem, float hi_elem) {   // low 16 bits = first argument
-  const __half2 h = __floats2half2_rn(lo_elem, hi_elem);
-  return *reinterpret_cast<const uint32_t*>(&h);
-}
-
-// power-of-two scale for one right-hand side from the bit pattern of max |psi|: max * S in [2^14, 2^15)
-__device__ __forceinline__ void rhs_scale(unsigned maxbits, float* S, float* invS) {
-  int e = (int)(maxbits >> 23);        // biased exponent, max in [2^(e-127), 2^(e-126))
-  int f = 268 - e;                     // biased exponent of S = 2^(141 - e)
-  f = f > 227 ? 227 : f;
-  if (maxbits == 0u) f = 127;
-  *S = __uint_as_float((uint32_t)f << 23);
-  *invS = __uint_as_float((uint32_t)(254 - f) << 23);
-}
-
 __device__ __forceinline__ bool elect_one() {   // one lane of a converged warp
   uint32_t pred;
   asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(pred));
@@ -130,10 +125,14 @@ struct SiteIter {
   }
 };
 
+__device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+
 }  // namespace
 
-// max |psi| per right-hand side: block = 4 sites x 72 float4 units; unit u of a record holds row n = u % 24
-__global__ void __launch_bounds__(288) colmax_kernel(const float4* __restrict__ psi, int V, unsigned* __restrict__ colmax) {
+// ------------------------------------------------------------------ fp32 records -> operand records
+// max |psi| per right-hand side into header.maxbits: block = 4 sites x 72 float4 units; unit u of a record holds row n = u % 24
+__global__ void __launch_bounds__(288) mrhs_colmax_kernel(const float4* __restrict__ psi, int V, MrhsVecHeader* __restrict__ hdr) {
+  if (hdr->valid) return;
   __shared__ unsigned smax[12];
   if (threadIdx.x < 12) smax[threadIdx.x] = 0u;
   __syncthreads();
@@ -149,12 +148,42 @@ __global__ void __launch_bounds__(288) colmax_kernel(const float4* __restrict__ 
   }
   atomicMax(&smax[rhs], m);
   __syncthreads();
-  if (threadIdx.x < 12 && smax[threadIdx.x]) atomicMax(&colmax[threadIdx.x], smax[threadIdx.x]);
+  if (threadIdx.x < 12 && smax[threadIdx.x]) atomicMax(&hdr->maxbits[threadIdx.x], smax[threadIdx.x]);
 }
 
+// mode 0: scales from header.maxbits (skips if header.valid), the last CTA sets header.scale / valid; mode 1: given scales
+template <int MODE>
+__global__ void __launch_bounds__(288) mrhs_split_kernel(const float* __restrict__ f32, __half* __restrict__ op, int V,
+                                                          MrhsVecHeader* __restrict__ hdr, const float* __restrict__ scale) {
+  if (MODE == 0 && hdr->valid) return;
+  const int unit = threadIdx.x % 36, slot = threadIdx.x / 36;
+  const int rhs = unit % 12, c4 = unit / 12;
+  const float S = MODE == 0 ? mrhs_scale_from_bound(__uint_as_float(hdr->maxbits[rhs])) : scale[rhs];
+  for (long long s = (long long)blockIdx.x * 8 + slot; s < V; s += (long long)gridDim.x * 8) {
+    const float* src = f32 + s * kMrhsVecSiteFloats + unit * 8;
+    mrhs_store_operand(op + s * kMrhsOpSiteHalves, c4, rhs, *reinterpret_cast<const float4*>(src), *reinterpret_cast<const float4*>(src + 4), S);
+  }
+  if (MODE == 0) {
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      if (atomicAdd(&hdr->done, 1u) + 1u == gridDim.x) {      // last CTA: publish
+        for (int j = 0; j < 12; ++j) {
+          hdr->scale[j] = mrhs_scale_from_bound(__uint_as_float(hdr->maxbits[j]));
+          hdr->maxbits[j] = 0u;
+        }
+        hdr->done = 0u;
+        __threadfence();
+        hdr->valid = 1u;
+      }
+    }
+  }
+}
+
+template <bool DOT>
 __global__ void __launch_bounds__(kThreads, 1)
-apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi, float* __restrict__ out, Geom g, int run,
-                  const unsigned* __restrict__ colmax) {
+apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_op, const float* __restrict__ psi_scale, float* __restrict__ out,
+                  Geom g, int run, MrhsVecHeader* __restrict__ out_hdr, const float* __restrict__ dot_a, double* __restrict__ partials) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ uint32_t s_tmem;
   __shared__ __align__(8) Bars bars;
@@ -163,11 +192,16 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
   int* sNbr = reinterpret_cast<int*>(smem + kSmemW);
 
   if (tid == 0) {
-    for (int i = 0; i < kARing; ++i) { mbar_init(&bars.afull[i], 3); mbar_init(&bars.aempty[i], 1); }
+    for (int i = 0; i < kASites; ++i) { mbar_init(&bars.aempty[i], 1); mbar_init(&bars.afull[i], 4); }
     for (int i = 0; i < kWSlots; ++i) { mbar_init(&bars.wfull[i], 1); mbar_init(&bars.wempty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&bars.dfull[i], 1); mbar_init(&bars.dempty[i], 3); }
-    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], 3 * kG); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&bars.dfull[i], 1); mbar_init(&bars.dempty[i], 2); }
+    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], 4); }
     asm volatile("fence.mbarrier_init.release.cluster;");
+    if (blockIdx.x == 0 && out_hdr) {   // out's operand records no longer match; leave a clean header behind
+      out_hdr->valid = 0u;
+      out_hdr->done = 0u;
+      for (int j = 0; j < 12; ++j) out_hdr->maxbits[j] = 0u;
+    }
   }
   // the never-copied tail of every W slot (k chunk 5 of the last stage) must read as zero
   for (int i = tid; i < kWSlots * 48; i += kThreads)
@@ -194,22 +228,21 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
   if (warp == kWarpMma) {
     // ------------------------------------------------------------------ MMA issuer (one elected thread, warp-uniform path)
     if (elect_one()) {
-      int st = 0;
-      uint32_t aph = 0, wph = 0, dph = 1;
+      // One wait per site and resource (a try_wait costs ~90 cycles even when the phase is complete)
+      uint32_t wph = 0, dph = 1;
       int ws = 0;
       for (int k = 0; k < nsite; ++k) {
-        const int d = k & 1;
+        const int d = k & 1, as = k & (kASites - 1);
         mbar_wait(&bars.dempty[d], dph);          // epilogue drained this accumulator
         dph ^= (uint32_t)d;                       // both accumulators used once -> next phase
         mbar_wait(&bars.wfull[ws], wph);          // W tile landed
+        mbar_wait(&bars.afull[as], (uint32_t)(k / kASites) & 1u);   // the site's 7 A stages are in tensor memory
         tc_fence_after();
         const uint32_t dcol = tmem + kDCol0 + 64 * d;
         const uint32_t w0 = smem_u32(sW + ws * kWSlotBytes);
+        const uint32_t a0 = tmem + as * kASiteCols;
 #pragma unroll
         for (int c = 0; c < kMrhsStages; ++c) {
-          mbar_wait(&bars.afull[st], aph);
-          tc_fence_after();
-          const uint32_t a0 = tmem + st * kACols;
 #pragma unroll
           for (int j = 0; j < 3; ++j) {
             const uint64_t db = umma_desc(w0 + c * (kMrhsStageHalves * 2) + j * (2 * kLBO));
@@ -217,12 +250,11 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
             asm volatile(
                 "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, {%5, %5, %5, %5}, p;\n\t}\n" ::"r"(dcol),
-                "r"(a0 + 8 * j), "l"(db), "r"(kIdesc), "r"(acc), "r"(zero)
+                "r"(a0 + c * kACols + 8 * j), "l"(db), "r"(kIdesc), "r"(acc), "r"(zero)
                 : "memory");
           }
-          umma_commit(&bars.aempty[st]);
-          if (++st == kARing) { st = 0; aph ^= 1u; }
         }
+        umma_commit(&bars.aempty[as]);
         umma_commit(&bars.wempty[ws]);
         umma_commit(&bars.dfull[d]);
         if (++ws == kWSlots) { ws = 0; wph ^= 1u; }
@@ -275,141 +307,184 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
       if (lane == 0) mbar_arrive(&bars.nfull[slot]);
       if (++slot == kNbrRing) { slot = 0; eph ^= 1u; }
     }
-  } else if (warp >= kWarpEpi && warp < kWarpEpi + 3) {
-    // ------------------------------------------------------------------ epilogue: TMEM -> out
+  } else if (warp >= kWarpEpi) {
+    // ------------------------------------------------------------------ epilogue: TMEM -> out (+ fused reductions)
+    // thread (gq, cp) of half h: rows n%12 = gq + 8h (hi in TMEM lane 16h + gq, lo 8 lanes further), D columns 8i + 2cp + e
     const int q = warp & 3;
     const int gq = lane >> 2, cp = lane & 3;
     const uint32_t lane_base = (uint32_t)(32 * q) << 16;
-    const int nrow = 8 * q + gq;                 // n = 2 rhs + part
-    float S, invS;
-    rhs_scale(colmax[nrow >> 1], &S, &invS);
+    const int n0 = 12 * q + gq, n1 = 12 * q + 8 + gq;        // n = 2 rhs + part of the two halves (n1 valid for gq < 4)
+    const bool on1 = gq < 4;
+    const float invS0 = 1.f / psi_scale[n0 >> 1], invS1 = on1 ? 1.f / psi_scale[n1 >> 1] : 0.f;
     const float kLo = 1.f / kMrhsLoScale;
     const float sgn = (gq & 1) ? 1.f : -1.f;
-    float* obase = out + nrow * 4 + cp;
+    const int off0 = n0 * 4 + cp, off1 = n1 * 4 + cp, pof0 = (n0 ^ 1) * 4 + cp, pof1 = (n1 ^ 1) * 4 + cp;
+    double acc[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
     SiteIter si(run);
     uint32_t fph = 0;
     for (int k = 0; k < nsite; ++k, si.next()) {
       const int d = k & 1;
+      float a_own[2][3], a_par[2][3];
+      if (DOT) {   // prefetch the other vector of the reductions while the MMAs of this site finish
+        const float* ar = dot_a + (size_t)si.n * kMrhsVecSiteFloats;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          a_own[0][j] = __ldg(ar + j * 96 + off0);
+          a_par[0][j] = __ldg(ar + j * 96 + pof0);
+          a_own[1][j] = on1 ? __ldg(ar + j * 96 + off1) : 0.f;
+          a_par[1][j] = on1 ? __ldg(ar + j * 96 + pof1) : 0.f;
+        }
+      }
       mbar_wait(&bars.dfull[d], fph);
       fph ^= (uint32_t)d;
       tc_fence_after();
       const uint32_t t0 = tmem + lane_base + kDCol0 + 64 * d;
-      float r[24];   // r[4J + e] = D[row g (psi hi)][col 8J + 2cp + e], r[4J + 2 + e] = D[row g + 8 (psi lo)][same col]
-      asm volatile("tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                   : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]), "=f"(r[8]),
-                     "=f"(r[9]), "=f"(r[10]), "=f"(r[11]), "=f"(r[12]), "=f"(r[13]), "=f"(r[14]), "=f"(r[15])
-                   : "r"(t0));
-      asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                   : "=f"(r[16]), "=f"(r[17]), "=f"(r[18]), "=f"(r[19]), "=f"(r[20]), "=f"(r[21]), "=f"(r[22]), "=f"(r[23])
-                   : "r"(t0 + 32));
+      float r[2][24];   // r[h][4J + e] = D[hi row][col 8J + 2cp + e], r[h][4J + 2 + e] = D[lo row][same col]
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const uint32_t th = t0 + ((uint32_t)(16 * h) << 16);
+        asm volatile("tcgen05.ld.sync.aligned.16x256b.x4.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=f"(r[h][0]), "=f"(r[h][1]), "=f"(r[h][2]), "=f"(r[h][3]), "=f"(r[h][4]), "=f"(r[h][5]), "=f"(r[h][6]), "=f"(r[h][7]),
+                       "=f"(r[h][8]), "=f"(r[h][9]), "=f"(r[h][10]), "=f"(r[h][11]), "=f"(r[h][12]), "=f"(r[h][13]), "=f"(r[h][14]), "=f"(r[h][15])
+                     : "r"(th));
+        asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=f"(r[h][16]), "=f"(r[h][17]), "=f"(r[h][18]), "=f"(r[h][19]), "=f"(r[h][20]), "=f"(r[h][21]), "=f"(r[h][22]), "=f"(r[h][23])
+                     : "r"(th + 32));
+      }
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&bars.dempty[d]);
-      // fold psi lo (rows g + 8) and W lo (columns 24..47 = J 3..5):  Sv[j][e] for W row w = 8 j + 2 cp + e = (c = 4 j + cp, part e)
-      float Sv[3][2], O[3];
+      float* rec = out + (size_t)si.n * kMrhsVecSiteFloats;
 #pragma unroll
-      for (int j = 0; j < 3; ++j)
+      for (int h = 0; h < 2; ++h) {
+        // fold psi lo (second row) and W lo (columns 24..47 = J 3..5):  Sv[j][e] for W row w = 8 j + 2 cp + e = (c = 4 j + cp, part e)
+        const float invS = h ? invS1 : invS0;
+        float Sv[3][2], O[3];
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          const float hi = fmaf(r[4 * j + 2 + e], kLo, r[4 * j + e]);
-          const float lo = fmaf(r[4 * (j + 3) + 2 + e], kLo, r[4 * (j + 3) + e]);
-          Sv[j][e] = fmaf(lo, kLo, hi) * invS;
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const float hi = fmaf(r[h][4 * j + 2 + e], kLo, r[h][4 * j + e]);
+            const float lo = fmaf(r[h][4 * (j + 3) + 2 + e], kLo, r[h][4 * (j + 3) + e]);
+            Sv[j][e] = fmaf(lo, kLo, hi) * invS;
+          }
+#pragma unroll
+        for (int j = 0; j < 3; ++j) O[j] = __shfl_xor_sync(0xffffffffu, Sv[j][1], 4);   // partner row: Re <-> Im of psi
+        // even n (psi_r): Out_r = W_r psi_r - W_i psi_i ; odd n (psi_i): Out_i = W_r psi_i + W_i psi_r
+        if (h == 0 || on1) {
+          const int off = h ? off1 : off0;
+#pragma unroll
+          for (int j = 0; j < 3; ++j) {
+            const float o = fmaf(sgn, O[j], Sv[j][0]);
+            rec[j * 96 + off] = o;
+            if (DOT) {   // this thread holds one part (Re for even n, Im for odd n) of out: <a,out> = sum conj(a) out
+              const double od = (double)o;
+              acc[h][0] += (double)a_own[h][j] * od;            // Re: a_r o_r + a_i o_i
+              acc[h][1] += (double)(sgn * a_par[h][j]) * od;    // Im: a_r o_i - a_i o_r
+              acc[h][2] += od * od;
+            }
+          }
         }
-#pragma unroll
-      for (int j = 0; j < 3; ++j) O[j] = __shfl_xor_sync(0xffffffffu, Sv[j][1], 4);   // partner row: Re <-> Im of psi
-      // even g (psi_r): Out_r = W_r psi_r - W_i psi_i ; odd g (psi_i): Out_i = W_r psi_i + W_i psi_r
-      float* rec = obase + (size_t)si.n * kMrhsVecSiteFloats;
-#pragma unroll
-      for (int j = 0; j < 3; ++j) rec[j * 96] = fmaf(sgn, O[j], Sv[j][0]);
+      }
     }
-  } else if ((warp & 3) < 3 && warp < 4 * kG) {
-    // ------------------------------------------------------------------ A producers: Psi (L1/L2) -> fp16 hi/lo -> TMEM
-    // warp (q, gi) handles the stages it = gi, gi + kG, ... of this CTA's stage sequence (it = 7 k + c) for rows 8q..8q+7
-    const int q = warp & 3, gi = warp >> 2;
-    const int gq = lane >> 2, cp = lane & 3;
-    const int nrow = 8 * q + gq;
-    float S, invS;
-    rhs_scale(colmax[nrow >> 1], &S, &invS);
-    const float S2 = S * kMrhsLoScale;
-    const float4* pbase = psi + nrow;                       // + 72 nn + 24 c4
-    const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16);
-    const int nmine = total > gi ? (total - gi + kG - 1) / kG : 0;
-
-    // load side state: stage c of the site in index-ring slot lslot
-    int lc = gi, lslot = 0;
-    uint32_t lph = 0;
-    auto load = [&](float4 (&v)[3]) {
-      if (lc < kG) mbar_wait(&bars.nfull[lslot], lph);      // this warp's first stage of the site
-      const int* nb = sNbr + lslot * 32;
-      if (lc < 6) {
-        const float4* rec = pbase + (size_t)nb[4 * lc + cp] * (kMrhsVecSiteFloats / 4);
-        v[0] = __ldg(rec);
-        v[1] = __ldg(rec + 24);
-        v[2] = __ldg(rec + 48);
-      } else {   // terms 24..26: slot s = 4 j + cp < 9 -> (term 24 + s/3, c4 = s%3)
+    if (DOT) {
+      // the 8 lanes (n, n^1) x cp of a right-hand side: fixed-order butterfly, then one partial row per CTA
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const int s = 4 * j + cp;
-          v[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (s < 9) v[j] = __ldg(pbase + (size_t)nb[24 + s / 3] * (kMrhsVecSiteFloats / 4) + (s % 3) * 24);
+      for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          double v = acc[h][c];
+          v += shfl_xor_d(v, 1);
+          v += shfl_xor_d(v, 2);
+          v += shfl_xor_d(v, 4);
+          acc[h][c] = v;
+        }
+      if ((lane & 7) == 0) {
+        double* row = partials + (size_t)blockIdx.x * 36;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          row[(n0 >> 1) * 3 + c] = acc[0][c];
+          if (on1) row[(n1 >> 1) * 3 + c] = acc[1][c];
         }
       }
-      if (lc >= kMrhsStages - kG) {                         // this warp's last stage of the site: the index slot may be refilled
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bars.nempty[lslot]);
-      }
-      lc += kG;
-      if (lc >= kMrhsStages) {
-        lc -= kMrhsStages;
-        if (++lslot == kNbrRing) { lslot = 0; lph ^= 1u; }
-      }
-    };
-    // store side state: A ring slot
-    int st = gi;
-    uint32_t eph = 1;
-    auto store = [&](const float4 (&v)[3]) {
-      uint32_t h[3][4];   // [j][0,1] = hi pieces of columns 8j + 2cp, +1 ; [j][2,3] = lo pieces
+    }
+  } else if ((warp & 3) < 2) {
+    // ------------------------------------------------------------------ A producers: operand records (L1/L2) -> TMEM
+    // warp (q, as, h): A rows of lane quarter q, sites k = as, as + 2, ... of this CTA (A ring slot as), stages 0-3 (h = 0) or
+    // 4-6 (h = 1).  Per stage one LDS.128 (4 neighbour indices), 12 LDG.64, 3 tcgen05.st; all loads of the warp's stages are
+    // issued before it waits for the ring slot, so the gathers of site k + 2 fly while the tensor core works on site k.
+    // Lanes 20-23 and 28-31 own no A row: they re-read a neighbouring lane's row (any finite numbers do; their TMEM lanes are
+    // never read), so no lane is predicated off.
+    const int q = warp & 3, as = (warp >> 2) & 1, h = warp >> 3;
+    const int slot = lane < 20 ? lane : (lane < 28 ? lane - 4 : lane - 8);
+    const uint2* pbase = psi_op + q * 72 + slot;               // + 144 site + 24 g   (8-byte units)
+    const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16) + as * kASiteCols;
+    for (int k = as; k < nsite; k += kASites) {
+      const int ns = k & (kNbrRing - 1);
+      mbar_wait(&bars.nfull[ns], (uint32_t)(k / kNbrRing) & 1u);
+      const int* nb = sNbr + ns * 32;
+      auto load = [&](int c, uint2 (&w)[12]) {   // w[pair]: TMEM columns 2 pair, 2 pair + 1 of stage c
+        const int4 t = *reinterpret_cast<const int4*>(nb + 4 * c);
+        if (c < 6) {       // pair = 4 g + t4: term 4 c + t4, components 4 g .. 4 g + 3
+          const uint2* r0 = pbase + (size_t)t.x * 144;
+          const uint2* r1 = pbase + (size_t)t.y * 144;
+          const uint2* r2 = pbase + (size_t)t.z * 144;
+          const uint2* r3 = pbase + (size_t)t.w * 144;
 #pragma unroll
-      for (int j = 0; j < 3; ++j) {
-        const __half2 h01 = __floats2half2_rn(v[j].x * S, v[j].y * S), h23 = __floats2half2_rn(v[j].z * S, v[j].w * S);
-        const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
-        h[j][0] = *reinterpret_cast<const uint32_t*>(&h01);
-        h[j][1] = *reinterpret_cast<const uint32_t*>(&h23);
-        h[j][2] = pack_h2(fmaf(-kMrhsLoScale, f01.x, v[j].x * S2), fmaf(-kMrhsLoScale, f01.y, v[j].y * S2));
-        h[j][3] = pack_h2(fmaf(-kMrhsLoScale, f23.x, v[j].z * S2), fmaf(-kMrhsLoScale, f23.y, v[j].w * S2));
+          for (int gg = 0; gg < 3; ++gg) {
+            w[4 * gg + 0] = __ldg(r0 + 24 * gg);
+            w[4 * gg + 1] = __ldg(r1 + 24 * gg);
+            w[4 * gg + 2] = __ldg(r2 + 24 * gg);
+            w[4 * gg + 3] = __ldg(r3 + 24 * gg);
+          }
+        } else {           // terms 24..26: pair = s = 3 (term - 24) + g, s < 9; pairs 9..11 are the zero pad (W's pad is zero too)
+          const uint2* r0 = pbase + (size_t)t.x * 144;
+          const uint2* r1 = pbase + (size_t)t.y * 144;
+          const uint2* r2 = pbase + (size_t)t.z * 144;
+#pragma unroll
+          for (int gg = 0; gg < 3; ++gg) {
+            w[gg] = __ldg(r0 + 24 * gg);
+            w[3 + gg] = __ldg(r1 + 24 * gg);
+            w[6 + gg] = __ldg(r2 + 24 * gg);
+          }
+          w[9] = w[10] = w[11] = make_uint2(0u, 0u);
+        }
+      };
+      auto store = [&](int c, const uint2 (&w)[12]) {
+        const uint32_t t0 = tbase + c * kACols;
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+          asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(t0 + 8 * j), "r"(w[4 * j].x), "r"(w[4 * j].y),
+                       "r"(w[4 * j + 1].x), "r"(w[4 * j + 1].y), "r"(w[4 * j + 2].x), "r"(w[4 * j + 2].y), "r"(w[4 * j + 3].x), "r"(w[4 * j + 3].y)
+                       : "memory");
+      };
+      auto indices_read = [&]() {     // this warp is done with the index slot
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars.nempty[ns]);
+      };
+      auto slot_free = [&]() {        // the tensor core has finished the site that used this ring slot
+        mbar_wait(&bars.aempty[as], ((uint32_t)(k / kASites) & 1u) ^ 1u);
+        tc_fence_after();
+      };
+      uint2 v[3][12];
+      if (h == 0) {
+        load(0, v[0]); load(1, v[1]); load(2, v[2]);
+        slot_free();
+        store(0, v[0]);
+        load(3, v[0]);
+        indices_read();
+        store(1, v[1]); store(2, v[2]); store(3, v[0]);
+      } else {
+        load(4, v[0]); load(5, v[1]); load(6, v[2]);
+        indices_read();
+        slot_free();
+        store(4, v[0]); store(5, v[1]); store(6, v[2]);
       }
-      mbar_wait(&bars.aempty[st], eph);
-      tc_fence_after();
-      const uint32_t t0 = tbase + st * kACols;
-      asm volatile("tcgen05.st.sync.aligned.16x256b.x2.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(t0), "r"(h[0][0]), "r"(h[0][1]),
-                   "r"(h[0][2]), "r"(h[0][3]), "r"(h[1][0]), "r"(h[1][1]), "r"(h[1][2]), "r"(h[1][3])
-                   : "memory");
-      asm volatile("tcgen05.st.sync.aligned.16x256b.x1.b32 [%0], {%1,%2,%3,%4};" ::"r"(t0 + 16), "r"(h[2][0]), "r"(h[2][1]), "r"(h[2][2]),
-                   "r"(h[2][3])
-                   : "memory");
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&bars.afull[st]);
-      st += kG;
-      if (st >= kARing) { st -= kARing; eph ^= 1u; }
-    };
-
-    float4 ra[3], rb[3], rc[3];   // two stages of gathers in flight behind the one being converted
-    if (nmine > 0) load(ra);
-    if (nmine > 1) load(rb);
-    for (int i = 0; i < nmine; i += 3) {
-      if (i + 2 < nmine) load(rc);
-      store(ra);
-      if (i + 1 < nmine) {
-        if (i + 3 < nmine) load(ra);
-        store(rb);
-      }
-      if (i + 2 < nmine) {
-        if (i + 4 < nmine) load(rb);
-        store(rc);
-      }
+      if (lane == 0) mbar_arrive(&bars.afull[as]);
     }
   }
 
@@ -418,32 +493,75 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const float4* __restrict__ psi,
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTmemCols));
 }
 
-int launch_apply_mrhs(const ok_params* p, const void* W, const void* psi, void* out) {
+static int mrhs_init() {
+  if (g_mrhs_ready) return OK_SUCCESS;
+  OK_CUDA(cudaMemcpyToSymbol(c_moff, kOffsets, sizeof(kOffsets)));
+  int dev = 0;
+  OK_CUDA(cudaGetDevice(&dev));
+  OK_CUDA(cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev));
+  OK_CUDA(cudaFuncSetAttribute(apply_mrhs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+  OK_CUDA(cudaFuncSetAttribute(apply_mrhs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+  g_mrhs_ready = true;
+  return OK_SUCCESS;
+}
+
+int mrhs_max_apply_ctas() {
+  if (mrhs_init()) return 1024;
+  return g_sm_count;
+}
+
+int launch_apply_mrhs(const ok_params* p, const void* W, const __half* psi_op, const float* psi_scale, float* out, MrhsVecHeader* out_hdr,
+                      const float* dot_a, double* partials, int* npartials) {
   if (p->nrhs != 12 || p->precision != OK_FP32) return OK_EINVAL;
-  static int sm_count = 0;
-  static unsigned* colmax = nullptr;
-  if (!g_mrhs_ready) {
-    OK_CUDA(cudaMemcpyToSymbol(c_moff, kOffsets, sizeof(kOffsets)));
-    int dev = 0;
-    OK_CUDA(cudaGetDevice(&dev));
-    OK_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
-    OK_CUDA(cudaFuncSetAttribute(apply_mrhs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
-    OK_CUDA(cudaGetSymbolAddress(reinterpret_cast<void**>(&colmax), g_colmax));
-    g_mrhs_ready = true;
-  }
+  int st = mrhs_init();
+  if (st) return st;
   Geom g = make_geom(p);
-  cudaStream_t st = ctx().stream;
-  OK_CUDA(cudaMemsetAsync(colmax, 0, sizeof(unsigned) * 12, st));
-  const int cgrid = (g.V + 3) / 4 < sm_count * 8 ? (g.V + 3) / 4 : sm_count * 8;
-  colmax_kernel<<<cgrid, 288, 0, st>>>(static_cast<const float4*>(psi), g.V, colmax);
-  OK_LAUNCHED("colmax_kernel");
   const int run = g.L[0] < 8 ? 8 : (g.L[0] > 32 ? 32 : g.L[0]);   // consecutive sites per work unit (an x line when 8 <= Lx <= 32)
   const int nruns = (g.V + run - 1) / run;
-  const int grid = nruns < sm_count ? nruns : sm_count;   // one persistent CTA per SM (it owns all 512 TMEM columns)
-  apply_mrhs_kernel<<<grid, kThreads, kSmemBytes, st>>>(static_cast<const uint8_t*>(W), static_cast<const float4*>(psi),
-                                                        static_cast<float*>(out), g, run, colmax);
+  const int grid = nruns < g_sm_count ? nruns : g_sm_count;   // one persistent CTA per SM (it owns all 512 TMEM columns)
+  if (dot_a) {
+    apply_mrhs_kernel<true><<<grid, kThreads, kSmemBytes, ctx().stream>>>(static_cast<const uint8_t*>(W), reinterpret_cast<const uint2*>(psi_op),
+                                                                          psi_scale, out, g, run, out_hdr, dot_a, partials);
+    if (npartials) *npartials = grid;
+  } else {
+    apply_mrhs_kernel<false><<<grid, kThreads, kSmemBytes, ctx().stream>>>(static_cast<const uint8_t*>(W), reinterpret_cast<const uint2*>(psi_op),
+                                                                           psi_scale, out, g, run, out_hdr, nullptr, nullptr);
+  }
   OK_LAUNCHED("apply_mrhs_kernel");
   return OK_SUCCESS;
+}
+
+int mrhs_ensure_operand(const ok_params* p, void* vec) {
+  int st = mrhs_init();
+  if (st) return st;
+  Geom g = make_geom(p);
+  MrhsVecHeader* hdr = static_cast<MrhsVecHeader*>(vec);
+  const int cgrid = (g.V + 3) / 4 < g_sm_count * 8 ? (g.V + 3) / 4 : g_sm_count * 8;
+  mrhs_colmax_kernel<<<cgrid, 288, 0, ctx().stream>>>(reinterpret_cast<const float4*>(mrhs_f32(vec)), g.V, hdr);
+  OK_LAUNCHED("mrhs_colmax_kernel");
+  const int sgrid = (g.V + 7) / 8 < g_sm_count * 8 ? (g.V + 7) / 8 : g_sm_count * 8;
+  mrhs_split_kernel<0><<<sgrid, 288, 0, ctx().stream>>>(mrhs_f32(vec), mrhs_op(vec, g.V), g.V, hdr, nullptr);
+  OK_LAUNCHED("mrhs_split_kernel");
+  return OK_SUCCESS;
+}
+
+int mrhs_write_operand(const ok_params* p, const float* f32, __half* op, const float* scale) {
+  int st = mrhs_init();
+  if (st) return st;
+  Geom g = make_geom(p);
+  const int sgrid = (g.V + 7) / 8 < g_sm_count * 8 ? (g.V + 7) / 8 : g_sm_count * 8;
+  mrhs_split_kernel<1><<<sgrid, 288, 0, ctx().stream>>>(f32, op, g.V, nullptr, scale);
+  OK_LAUNCHED("mrhs_split_kernel");
+  return OK_SUCCESS;
+}
+
+int mrhs_apply_vec(const ok_params* p, const void* W, void* psi_vec, void* out_vec) {
+  Geom g = make_geom(p);
+  int st = mrhs_ensure_operand(p, psi_vec);
+  if (st) return st;
+  const MrhsVecHeader* hin = static_cast<const MrhsVecHeader*>(psi_vec);
+  return launch_apply_mrhs(p, W, mrhs_op(psi_vec, g.V), hin->scale, mrhs_f32(out_vec), static_cast<MrhsVecHeader*>(out_vec), nullptr, nullptr,
+                           nullptr);
 }
 
 }  // namespace okd

@@ -9,6 +9,13 @@
 // for one column (ok_internal.cuh, mrhs_vec_index): unit q = 12 c4 + j, column j = q % 12.
 // A thread keeps q (hence j) fixed and strides over sites, so per-column reductions need no atomics:
 // thread -> smem -> fixed-order sum per (column, quantity) -> one partial per CTA -> single-CTA final.
+//
+// The two vectors the operator is applied to, p and s, are ALSO written in the tensor-core operand form (split fp16,
+// ok_internal.cuh) by the kernels that update them, so the apply never converts or scans its input.  Their per-column
+// power-of-two scales come from norm bounds that are known before the update runs (||x||_2 >= max |x_i|):
+//   ||s|| <= ||r|| + |alpha| ||v||          ||p'|| <= ||r'|| + |beta| (||p|| + |omega| ||v||)
+// with ||v||^2 from the apply's epilogue and ||p||^2 reduced by the p update itself.  <rhat,v>, ||v||^2, <s,t>, ||t||^2 come
+// out of the apply's epilogue (ok_apply_mrhs.cu), so an iteration is 2 applies + 3 vector kernels.
 #include <math.h>
 
 #include "ok_internal.cuh"
@@ -25,6 +32,8 @@ constexpr double kTinyM = 1e-300;
 struct ScalM {
   double rho[kN][2], alpha[kN][2], omega[kN][2], beta[kN][2];
   double rr[kN], bnorm2[kN];
+  double vv[kN], pp[kN];   // ||v||^2 of the last apply of p, ||p||^2 after the last p update
+  float sscale[kN], pscale[kN], xscale[kN];   // power-of-two scales of the operand records of s, p (and x for the true residual)
   int breakdown[kN];
   int active[kN];     // written by the host: 1 = iterating, 0 = frozen
   int restart[kN];    // written by the host before k_residual: 1 = take r = rhat = p = true residual
@@ -97,27 +106,12 @@ m_init(const float* __restrict__ b, float* __restrict__ x, float* __restrict__ r
   column_reduce<1>(d, unit, partials + (size_t)blockIdx.x * 36);
 }
 
-// partials: ( Re<a,b>, Im<a,b>, ||b||^2 ) per column
 __global__ void __launch_bounds__(kThreads)
-m_dot(const float* __restrict__ a, const float* __restrict__ b, long long V, double* __restrict__ partials) {
-  double d[3] = {0.0, 0.0, 0.0};
-  OK_MRHS_LOOP(site) {
-    const V8 av = ld8(OK_AT(a, site)), bv = ld8(OK_AT(b, site));
-    OK_FOR4(k) {
-      const double ar = f4(av.re, k), ai = f4(av.im, k), br = f4(bv.re, k), bi = f4(bv.im, k);
-      d[0] += ar * br + ai * bi;
-      d[1] += ar * bi - ai * br;
-      d[2] += br * br + bi * bi;
-    }
-  }
-  (void)j;
-  column_reduce<3>(d, unit, partials + (size_t)blockIdx.x * 36);
-}
-
-__global__ void __launch_bounds__(kThreads)
-m_s_update(const float* __restrict__ r, const float* __restrict__ v, float* __restrict__ s, long long V, const ScalM* __restrict__ sc) {
+m_s_update(const float* __restrict__ r, const float* __restrict__ v, float* __restrict__ s, __half* __restrict__ s_op, long long V,
+           const ScalM* __restrict__ sc) {
   OK_MRHS_LOOP(site) {
     const double ar = sc->alpha[j][0], ai = sc->alpha[j][1];
+    const float S = sc->sscale[j];
     const V8 rv = ld8(OK_AT(r, site)), vv = ld8(OK_AT(v, site));
     V8 o;
     OK_FOR4(k) {
@@ -125,6 +119,7 @@ m_s_update(const float* __restrict__ r, const float* __restrict__ v, float* __re
       f4(o.im, k) = (float)((double)f4(rv.im, k) - (ar * f4(vv.im, k) + ai * f4(vv.re, k)));
     }
     st8(OK_AT(s, site), o);
+    mrhs_store_operand(s_op + site * kMrhsOpSiteHalves, unit / 12, j, o.re, o.im, S);
   }
 }
 
@@ -157,10 +152,14 @@ m_xr_update(float* __restrict__ x, const float* __restrict__ p, const float* __r
   column_reduce<3>(d, unit, partials + (size_t)blockIdx.x * 36);
 }
 
+// p = r + beta (p - omega v), its operand records, and the partial ||p||^2 per column (slot 0 of the 3)
 __global__ void __launch_bounds__(kThreads)
-m_p_update(float* __restrict__ p, const float* __restrict__ r, const float* __restrict__ v, long long V, const ScalM* __restrict__ sc) {
+m_p_update(float* __restrict__ p, __half* __restrict__ p_op, const float* __restrict__ r, const float* __restrict__ v, long long V,
+           const ScalM* __restrict__ sc, double* __restrict__ partials) {
+  double d[1] = {0.0};
   OK_MRHS_LOOP(site) {
     const double br = sc->beta[j][0], bi = sc->beta[j][1], wr = sc->omega[j][0], wi = sc->omega[j][1];
+    const float S = sc->pscale[j];
     const V8 pv = ld8(OK_AT(p, site)), rv = ld8(OK_AT(r, site)), vv = ld8(OK_AT(v, site));
     V8 o;
     OK_FOR4(k) {
@@ -168,9 +167,12 @@ m_p_update(float* __restrict__ p, const float* __restrict__ r, const float* __re
       const double qi = (double)f4(pv.im, k) - (wr * f4(vv.im, k) + wi * f4(vv.re, k));
       f4(o.re, k) = (float)((double)f4(rv.re, k) + (br * qr - bi * qi));
       f4(o.im, k) = (float)((double)f4(rv.im, k) + (br * qi + bi * qr));
+      d[0] += (double)f4(o.re, k) * f4(o.re, k) + (double)f4(o.im, k) * f4(o.im, k);
     }
     st8(OK_AT(p, site), o);
+    mrhs_store_operand(p_op + site * kMrhsOpSiteHalves, unit / 12, j, o.re, o.im, S);
   }
+  column_reduce<1>(d, unit, partials + (size_t)blockIdx.x * 36);
 }
 
 // true residual b - Mx: columns flagged restart take r = rhat = p = it; partial ||b - Mx||^2 for every column
@@ -195,7 +197,7 @@ m_residual(const float* __restrict__ b, const float* __restrict__ Mx, float* __r
   column_reduce<1>(d, unit, partials + (size_t)blockIdx.x * 36);
 }
 
-enum StageM { MF_INIT = 0, MF_V = 1, MF_T = 2, MF_XR = 3, MF_RES = 4 };
+enum StageM { MF_INIT = 0, MF_V = 1, MF_T = 2, MF_XR = 3, MF_RES = 4, MF_P = 5 };
 
 // single CTA: fixed-order sum of the per-CTA partials (36 doubles each), then the per-column scalars
 template <int STAGE>
@@ -217,26 +219,45 @@ __global__ void __launch_bounds__(kThreads) m_finalize(const double* __restrict_
   const int j = threadIdx.x;
   const double t0 = tot[3 * j], t1 = tot[3 * j + 1], t2 = tot[3 * j + 2];
   const bool on = sc->active[j] != 0;
-  if (STAGE == MF_INIT) {
+  if (STAGE == MF_INIT) {         // p = r = b
     sc->bnorm2[j] = t0; sc->rr[j] = t0;
     sc->rho[j][0] = t0; sc->rho[j][1] = 0.0;
     sc->breakdown[j] = 0;
-  } else if (STAGE == MF_RES) {   // t0 = ||b - Mx||^2 ; restart columns also reset rho
+    sc->pp[j] = t0;
+    sc->pscale[j] = mrhs_scale_from_bound((float)sqrt(t0));
+  } else if (STAGE == MF_RES) {   // t0 = ||b - Mx||^2 ; restart columns also reset rho and take p = r = b - Mx
     res_out[j] = t0;
-    if (sc->restart[j]) { sc->rr[j] = t0; sc->rho[j][0] = t0; sc->rho[j][1] = 0.0; sc->breakdown[j] = 0; }
+    if (sc->restart[j]) {
+      sc->rr[j] = t0; sc->rho[j][0] = t0; sc->rho[j][1] = 0.0; sc->breakdown[j] = 0;
+      sc->pp[j] = t0;
+      sc->pscale[j] = mrhs_scale_from_bound((float)sqrt(t0));
+    }
+  } else if (STAGE == MF_P) {     // t0 = ||p||^2 after the p update
+    sc->pp[j] = t0;
   } else if (STAGE == MF_V) {     // (Re<rhat,v>, Im<rhat,v>, ||v||^2)
-    if (!on) { sc->alpha[j][0] = sc->alpha[j][1] = 0.0; return; }
+    sc->vv[j] = t2;
+    if (!on) {                    // frozen column: s = r
+      sc->alpha[j][0] = sc->alpha[j][1] = 0.0;
+      sc->sscale[j] = mrhs_scale_from_bound((float)sqrt(sc->rr[j]));
+      return;
+    }
     if (badm(t0, t1) || badm(sc->rho[j][0], sc->rho[j][1])) sc->breakdown[j] |= 1;
     const double den = t0 * t0 + t1 * t1;
     sc->alpha[j][0] = (sc->rho[j][0] * t0 + sc->rho[j][1] * t1) / den;
     sc->alpha[j][1] = (sc->rho[j][1] * t0 - sc->rho[j][0] * t1) / den;
+    // ||s|| = ||r - alpha v|| <= ||r|| + |alpha| ||v||  >= max |s_i|: the scale of s's operand records
+    sc->sscale[j] = mrhs_scale_from_bound((float)(sqrt(sc->rr[j]) + hypot(sc->alpha[j][0], sc->alpha[j][1]) * sqrt(t2)));
   } else if (STAGE == MF_T) {     // (Re<s,t>, Im<s,t>, ||t||^2) ; <t,s> = conj<s,t>
     if (!on) { sc->omega[j][0] = sc->omega[j][1] = 0.0; return; }
     if (badm(t2, 0.0)) sc->breakdown[j] |= 2;
     sc->omega[j][0] = t0 / t2;
     sc->omega[j][1] = -t1 / t2;
   } else if (STAGE == MF_XR) {    // (||r||^2, Re<rhat,r>, Im<rhat,r>)
-    if (!on) { sc->beta[j][0] = sc->beta[j][1] = 0.0; return; }
+    if (!on) {                    // frozen column: p = r
+      sc->beta[j][0] = sc->beta[j][1] = 0.0;
+      sc->pscale[j] = mrhs_scale_from_bound((float)sqrt(sc->rr[j]));
+      return;
+    }
     sc->rr[j] = t0;
     if (badm(sc->omega[j][0], sc->omega[j][1]) || badm(t1, t2)) sc->breakdown[j] |= 4;
     const double r0 = sc->rho[j][0], r1 = sc->rho[j][1];
@@ -248,6 +269,8 @@ __global__ void __launch_bounds__(kThreads) m_finalize(const double* __restrict_
     sc->beta[j][0] = q0 * a0 - q1 * a1;
     sc->beta[j][1] = q0 * a1 + q1 * a0;
     sc->rho[j][0] = t1; sc->rho[j][1] = t2;
+    // ||p'|| = ||r' + beta (p - omega v)|| <= ||r'|| + |beta| (||p|| + |omega| ||v||)
+    sc->pscale[j] = mrhs_scale_from_bound((float)(sqrt(t0) + hypot(sc->beta[j][0], sc->beta[j][1]) * (sqrt(sc->pp[j]) + hypot(w0, w1) * sqrt(sc->vv[j]))));
   }
 }
 
@@ -257,18 +280,21 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 size_t bicgstab_mrhs_work_bytes(const ok_params* p) {
   Geom g = make_geom(p);
-  const size_t vb = align_up((size_t)g.nblk * kBlock * kMrhsVecSiteFloats * sizeof(float), 256);
-  const size_t ncta = ((size_t)g.V + kSitesPerCta - 1) / kSitesPerCta;
-  return 6 * vb + align_up(ncta * 36 * sizeof(double), 256) + align_up(sizeof(ScalM), 256) + 256;
+  const size_t vb = align_up((size_t)g.V * kMrhsVecSiteFloats * sizeof(float), 256);
+  size_t ncta = ((size_t)g.V + kSitesPerCta - 1) / kSitesPerCta;
+  if (ncta < 1024) ncta = 1024;   // also holds the apply's partial rows (one per persistent CTA)
+  return 8 * vb + align_up(ncta * 36 * sizeof(double), 256) + align_up(sizeof(ScalM), 256) + 256;
 }
 
+// src, xout: nrhs = 12 spinor fields (header + fp32 records + operand records, ok_internal.cuh)
 int run_bicgstab_mrhs(const ok_params* p, const void* W, const void* src, void* xout, double tol, int maxit, int* iters,
                       double* resid) {
   Geom g = make_geom(p);
   cudaStream_t st = ctx().stream;
   const long long V = g.V;
-  const size_t vb = align_up((size_t)g.nblk * kBlock * kMrhsVecSiteFloats * sizeof(float), 256);
+  const size_t vb = align_up((size_t)g.V * kMrhsVecSiteFloats * sizeof(float), 256);
   const int ncta = (int)((V + kSitesPerCta - 1) / kSitesPerCta);
+  size_t prow = (size_t)ncta < 1024 ? 1024 : (size_t)ncta;
   char* w = static_cast<char*>(ctx().work);
   float* r = reinterpret_cast<float*>(w + 0 * vb);
   float* rhat = reinterpret_cast<float*>(w + 1 * vb);
@@ -276,12 +302,15 @@ int run_bicgstab_mrhs(const ok_params* p, const void* W, const void* src, void* 
   float* v = reinterpret_cast<float*>(w + 3 * vb);
   float* s = reinterpret_cast<float*>(w + 4 * vb);
   float* t = reinterpret_cast<float*>(w + 5 * vb);
-  double* partials = reinterpret_cast<double*>(w + 6 * vb);
-  char* after = w + 6 * vb + align_up((size_t)ncta * 36 * sizeof(double), 256);
+  __half* p_op = reinterpret_cast<__half*>(w + 6 * vb);
+  __half* s_op = reinterpret_cast<__half*>(w + 7 * vb);
+  double* partials = reinterpret_cast<double*>(w + 8 * vb);
+  char* after = w + 8 * vb + align_up(prow * 36 * sizeof(double), 256);
   ScalM* sc = reinterpret_cast<ScalM*>(after);
   double* res_dev = reinterpret_cast<double*>(after + align_up(sizeof(ScalM), 256));   // 12 doubles (inside the +256 tail)
-  const float* b = static_cast<const float*>(src);
-  float* x = static_cast<float*>(xout);
+  const float* b = mrhs_f32(src);
+  float* x = mrhs_f32(xout);
+  MrhsVecHeader* xhdr = static_cast<MrhsVecHeader*>(xout);
 
   struct HostBuf { ScalM sc; double res[kN]; };
   static HostBuf* h = nullptr;   // pinned host mirror
@@ -309,12 +338,14 @@ int run_bicgstab_mrhs(const ok_params* p, const void* W, const void* src, void* 
   for (int j = 0; j < kN; ++j) { active[j] = 1; restart[j] = 0; it_conv[j] = 0; }
   OK_CUDA(cudaMemsetAsync(sc, 0, sizeof(ScalM), st));
   OK_CUDA(cudaMemsetAsync(res_dev, 0, sizeof(double) * kN, st));
+  OK_CUDA(cudaMemsetAsync(xhdr, 0, kMrhsVecHeaderBytes, st));   // x's operand records are stale from here on
   OK_TRY(push_flags());
 
   m_init<<<ncta, kThreads, 0, st>>>(b, x, r, rhat, pp, V, partials);
   OK_LAUNCHED("m_init");
   m_finalize<MF_INIT><<<1, kThreads, 0, st>>>(partials, ncta, sc, res_dev);
   OK_LAUNCHED("m_finalize");
+  OK_TRY(mrhs_write_operand(p, pp, p_op, sc->pscale));   // p = b in operand form
   OK_TRY(fetch());
   OK_TRY(wait());
   double bnorm2[kN], target[kN], true_rr[kN];
@@ -331,39 +362,42 @@ int run_bicgstab_mrhs(const ok_params* p, const void* W, const void* src, void* 
 
   auto true_residual = [&]() -> int {   // t = M x ; ||b - t||^2 per column ; flagged columns restart
     OK_TRY(push_flags());
-    OK_TRY(launch_apply_mrhs(p, W, x, t));
+    OK_CUDA(cudaMemsetAsync(&xhdr->valid, 0, sizeof(unsigned), st));
+    OK_TRY(mrhs_ensure_operand(p, xout));   // x in operand form (column maxima + split: two passes over x, only here)
+    OK_TRY(launch_apply_mrhs(p, W, mrhs_op(xout, g.V), xhdr->scale, t, nullptr, nullptr, nullptr, nullptr));
     m_residual<<<ncta, kThreads, 0, st>>>(b, t, r, rhat, pp, V, sc, partials);
     OK_LAUNCHED("m_residual");
     m_finalize<MF_RES><<<1, kThreads, 0, st>>>(partials, ncta, sc, res_dev);
     OK_LAUNCHED("m_finalize");
+    bool any = false;
+    for (int j = 0; j < kN; ++j) any = any || restart[j];
+    if (any) OK_TRY(mrhs_write_operand(p, pp, p_op, sc->pscale));   // restarted columns: p = true residual
     OK_TRY(fetch());
     OK_TRY(wait());
     return OK_SUCCESS;
   };
 
   int status = OK_SUCCESS;
-  int it = 0;
+  int it = 0, na = 0;
   while (nactive > 0 && it < maxit) {
     ++it;
-    OK_TRY(launch_apply_mrhs(p, W, pp, v));
-    m_dot<<<ncta, kThreads, 0, st>>>(rhat, v, V, partials);
-    OK_LAUNCHED("m_dot");
-    m_finalize<MF_V><<<1, kThreads, 0, st>>>(partials, ncta, sc, res_dev);
+    OK_TRY(launch_apply_mrhs(p, W, p_op, sc->pscale, v, nullptr, rhat, partials, &na));   // v = M p ; <rhat,v>, ||v||^2
+    m_finalize<MF_V><<<1, kThreads, 0, st>>>(partials, na, sc, res_dev);
     OK_LAUNCHED("m_finalize");
-    m_s_update<<<ncta, kThreads, 0, st>>>(r, v, s, V, sc);
+    m_s_update<<<ncta, kThreads, 0, st>>>(r, v, s, s_op, V, sc);
     OK_LAUNCHED("m_s_update");
-    OK_TRY(launch_apply_mrhs(p, W, s, t));
-    m_dot<<<ncta, kThreads, 0, st>>>(s, t, V, partials);
-    OK_LAUNCHED("m_dot");
-    m_finalize<MF_T><<<1, kThreads, 0, st>>>(partials, ncta, sc, res_dev);
+    OK_TRY(launch_apply_mrhs(p, W, s_op, sc->sscale, t, nullptr, s, partials, &na));      // t = M s ; <s,t>, ||t||^2
+    m_finalize<MF_T><<<1, kThreads, 0, st>>>(partials, na, sc, res_dev);
     OK_LAUNCHED("m_finalize");
     m_xr_update<<<ncta, kThreads, 0, st>>>(x, pp, s, t, r, rhat, V, sc, partials);
     OK_LAUNCHED("m_xr_update");
     m_finalize<MF_XR><<<1, kThreads, 0, st>>>(partials, ncta, sc, res_dev);
     OK_LAUNCHED("m_finalize");
     OK_TRY(fetch());
-    m_p_update<<<ncta, kThreads, 0, st>>>(pp, r, v, V, sc);
+    m_p_update<<<ncta, kThreads, 0, st>>>(pp, p_op, r, v, V, sc, partials);
     OK_LAUNCHED("m_p_update");
+    m_finalize<MF_P><<<1, kThreads, 0, st>>>(partials, ncta, sc, res_dev);
+    OK_LAUNCHED("m_finalize");
     OK_TRY(wait());
     bool check = false, broke = false;
     for (int j = 0; j < kN; ++j) {

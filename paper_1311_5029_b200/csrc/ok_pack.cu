@@ -25,8 +25,8 @@ __global__ void pack_spinor_kernel(const vec_t* __restrict__ canon, vec_t* __res
   }
 }
 
-// nrhs = 12, fp32: canonical [n][comp][rhs][re,im] <-> per-site records (ok_internal.cuh,
-// mrhs_vec_index).  One thread per complex number.
+// nrhs = 12, fp32: canonical [n][comp][rhs][re,im] <-> the fp32 per-site records of the field (ok_internal.cuh,
+// mrhs_vec_index).  One thread per complex number.  Packing then also writes the operand records (mrhs_ensure_operand).
 __global__ void pack_spinor_mrhs_kernel(const float2* __restrict__ canon, float* __restrict__ packed, int V, bool unpack) {
   long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (u >= (long long)V * 144) return;
@@ -75,10 +75,11 @@ int launch_pack_spinor(const ok_params* p, const void* canon, void* packed, bool
   const int T = 256;
   if (p->nrhs == 12) {
     long long total = (long long)g.V * 144;
+    if (!unpack) OK_CUDA(cudaMemsetAsync(packed, 0, kMrhsVecHeaderBytes, ctx().stream));   // header: operand records not valid yet
     pack_spinor_mrhs_kernel<<<(unsigned)((total + T - 1) / T), T, 0, ctx().stream>>>(
-        static_cast<const float2*>(canon), static_cast<float*>(packed), g.V, unpack);
+        static_cast<const float2*>(canon), mrhs_f32(packed), g.V, unpack);
     OK_LAUNCHED("pack_spinor_mrhs_kernel");
-    return OK_SUCCESS;
+    return unpack ? OK_SUCCESS : mrhs_ensure_operand(p, packed);
   }
   int NC = p->precision == OK_FP64 ? 12 : 6;
   long long total = (long long)g.nblk * NC * kBlock;

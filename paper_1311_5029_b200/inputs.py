@@ -181,6 +181,28 @@ def point_source(dims, site: int = 0, comp: int = 0) -> np.ndarray:
     return psi
 
 
+def sample_sites(dims, n_even: int = 384, n_rand: int = 384, seed: int = 11) -> np.ndarray:
+    """Sorted site indices on which full-size results are compared with the oracle: the lattice corners and faces
+    (every wrap-around of the stencil, the antiperiodic time boundary), the last 40 sites of the site order (the ragged
+    last block), evenly spaced sites and pseudo-random interior sites.  A test stimulus only."""
+    Lx, Ly, Lz, T = dims
+    V = volume(dims)
+
+    def site(x, y, z, t):
+        return x + Lx * (y + Ly * (z + Lz * t))
+
+    s = set()
+    for x in (0, 1, Lx - 2, Lx - 1):
+        for y in (0, 1, Ly - 2, Ly - 1):
+            for z in (0, 1, Lz - 2, Lz - 1):
+                for t in (0, 1, T - 2, T - 1):
+                    s.add(site(x, y, z, t))
+    s.update(range(V - 40, V))
+    s.update((np.arange(n_even) * (V // n_even) + 7).tolist())
+    s.update(np.random.default_rng(seed).integers(0, V, n_rand).tolist())
+    return np.array(sorted(s), dtype=np.int64)
+
+
 # --------------------------------------------------------------------------- u0
 def mean_plaquette(dims, U: np.ndarray) -> float:
     """(1/6V) sum_x sum_{mu<nu} (1/3) Re Tr U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag,

@@ -52,7 +52,7 @@ def test_sizes(lib):
     assert B.ok_vec_bytes(pr) == 96 * 12 * 16
     assert B.ok_work_bytes(pr) > 0
     pm = B.make_params(I.make_params((4, 4, 4, 8), 0.1, 0.95), B.OK_FP32, nrhs=12)
-    assert B.ok_vec_bytes(pm) == 512 * 12 * 12 * 8
+    assert B.ok_vec_bytes(pm) == 256 + 2 * 512 * 12 * 12 * 8     # header + fp32 records + tensor-core operand records
     # reduced storage formats: 260 resp. 132 colour blocks of 9 complex per site
     pb = B.make_params(I.make_params((20, 20, 20, 64), 0.1, 0.95), B.OK_FP32, storage=B.OK_W_BLOCK)
     assert B.ok_W_bytes(pb) == 1024 + V * 260 * 9 * 8            # 18 720 B/site

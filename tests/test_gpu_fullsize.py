@@ -24,23 +24,7 @@ FP32_TOL = 2e-5
 NR = 12
 
 
-def sample_sites(dims, n_even=384, n_rand=384, seed=11):
-    Lx, Ly, Lz, T = dims
-    V = Lx * Ly * Lz * T
-
-    def site(x, y, z, t):
-        return x + Lx * (y + Ly * (z + Lz * t))
-
-    s = set()
-    for x in (0, 1, Lx - 2, Lx - 1):
-        for y in (0, 1, Ly - 2, Ly - 1):
-            for z in (0, 1, Lz - 2, Lz - 1):
-                for t in (0, 1, T - 2, T - 1):
-                    s.add(site(x, y, z, t))
-    s.update(range(V - 40, V))                                   # the tail of the site order
-    s.update((np.arange(n_even) * (V // n_even) + 7).tolist())   # evenly spread
-    s.update(np.random.default_rng(seed).integers(0, V, n_rand).tolist())
-    return np.array(sorted(s), dtype=np.int64)
+sample_sites = I.sample_sites
 
 
 @pytest.fixture(scope="module")

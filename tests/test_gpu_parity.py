@@ -57,23 +57,16 @@ def test_pack_unpack_roundtrip(dims, prec):
 
 
 # ------------------------------------------------------------------ a3: apply in isolation (oracle W)
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("prec", [B.OK_FP64, B.OK_FP32])
 @pytest.mark.parametrize("dims", SHAPES)
-def test_apply_with_oracle_W(dims, prec, variant):
-    if prec == B.OK_FP64 and variant in (3,):
-        pytest.skip("RPT=6 fp64 variant not built (register budget)")
+def test_apply_with_oracle_W(dims, prec):
     U, pd, o = setup(dims)
     p = B.make_params(pd, prec)
     Wc = o.precalc_W()
     psi = I.gaussian_spinor(dims, 2)
     W = B.alloc_W(p)
     B.ok_pack_W(p, G.to_dev(Wc, G.cdtype(prec)), W)
-    B.ok_set_apply_variant(variant)
-    try:
-        got = G.apply(p, W, psi)
-    finally:
-        B.ok_set_apply_variant(0)
+    got = G.apply(p, W, psi)
     want = o.apply_W(psi, W=Wc)
     if prec == B.OK_FP64:
         assert G.per_site_rel_err(got, want) <= FP64_TOL
