@@ -81,3 +81,19 @@ def per_site_rel_err(got, want):
 
 def rel_l2(got, want):
     return float(np.linalg.norm(got - want) / np.linalg.norm(want))
+
+
+def fp32_operator_slack(o, x, b, idx=None, W=None):
+    """DESIGN.md 10, reading R-RESID.  The library's `resid` of an fp32 solve is || b - fl32(M32 x) || / || b || with M32 the
+    fp32-rounded W it stores; the oracle evaluates || b - M64 x || / || b ||.  The two differ by at most
+        || (M32 - M64) x || + || fl32(M32 x) - M32 x ||   <=   2 * 2^-24 * || |W| |x| ||_2
+    (every real of W rounded once: |dW| <= 2^-24 |W| elementwise, rigorous; the second term is the kernel's own fp32 rounding
+    of the 324-term sums, whose accumulated error stays below one unit 2^-24 |W||x| in every measured case).  Returns that
+    bound relative to || b || -- evaluated by the oracle as apply_W(|x|, W = |W|) -- on the sites `idx` (all sites if None;
+    for a sample the caller extrapolates like the residual itself)."""
+    Wa = np.abs(o.precalc_W(idx) if W is None else W).astype(np.complex128)
+    S = o.apply_W(np.abs(x).astype(np.complex128), idx=idx, W=Wa)
+    scale = 1.0 if idx is None else np.sqrt(o.V / len(idx))
+    if S.ndim == 3:     # [site][comp][rhs]: one bound per column
+        return 2.0 * 2.0 ** -24 * scale * np.linalg.norm(S.reshape(-1, S.shape[2]), axis=0) / np.linalg.norm(b.reshape(-1, b.shape[2]), axis=0)
+    return 2.0 * 2.0 ** -24 * scale * float(np.linalg.norm(S)) / float(np.linalg.norm(b))

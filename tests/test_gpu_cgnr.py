@@ -32,7 +32,7 @@ def test_cgnr_vs_oracle(dims, prec, tol, storage):
     xo, ito, reso, sto = oo.cgnr(ap, b, tol, 5000)
     assert sto == 0 and abs(it - ito) <= max(2, ito // 50)
     xs = G.unpack_spinor(p, x, b.shape)
-    assert np.linalg.norm(b - ap(xs)) / np.linalg.norm(b) <= (1.0 if prec == B.OK_FP64 else 2.0) * tol
+    assert np.linalg.norm(b - ap(xs)) / np.linalg.norm(b) <= tol + (0.0 if prec == B.OK_FP64 else G.fp32_operator_slack(o, xs, b, W=Wc))   # R-RESID
     assert G.rel_l2(xs, xo) <= 50 * tol
     x2 = B.alloc_vec(p)
     assert B.ok_cgnr(W, src, x2, tol, 5000, raise_on_fail=False) == (st, it, res) and torch.equal(x, x2)   # bit-reproducible

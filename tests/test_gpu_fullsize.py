@@ -8,6 +8,9 @@ boundary, the last ragged 32-site block) plus evenly spaced and pseudo-random in
 BiCGStab is checked through a property that holds at any size: the residual b - M x,
 evaluated by the ORACLE on the sampled sites, extrapolates to a relative residual of the order of tol.
 """
+import json
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -26,6 +29,32 @@ NR = 12
 
 sample_sites = I.sample_sites
 
+# The oracle's own BiCGStab runs at these sizes (iteration count, true residual, solution on sample sites), written by
+# tests/golden/make_fullsize_golden.py from oracle/ and the seeded input generators only (hours of CPU time; not rerun here).
+_GDIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+GOLD = json.load(open(os.path.join(_GDIR, "fullsize_bicgstab.json")))
+GOLD_X = np.load(os.path.join(_GDIR, "fullsize_x_samples.npz"))
+
+
+def check_against_golden(case, dims, it, tol, xs, ncol=1):
+    """north_star: "BiCGStab iteration counts must agree within +-2" (solver: PAPER.md:114) -- here against the oracle's run
+    on the same seeds at the full size; and the solution on the golden's sample sites.  Two iterates that both satisfy
+    || b - M x || <= tol || b || differ by at most cond(M) 2 tol relative to || x ||; cond(M) of these fields is O(10)
+    (34 BiCGStab iterations to 1e-6), the measured difference is recorded by the assert message."""
+    g = GOLD[case]
+    assert g["dims"] == list(dims) and g["tol"] == tol and len(g["columns"]) == ncol
+    its = [c["iters"] for c in g["columns"]]
+    assert all(c["status"] == 0 and c["true_resid"] <= tol for c in g["columns"])
+    assert abs(it - max(its)) <= 2, (it, its)                 # the library reports the slowest column
+    idx = sample_sites(dims, n_even=g["sample"]["n_even"], n_rand=g["sample"]["n_rand"])
+    want = GOLD_X[case]                                        # [sites, columns, 12]
+    assert want.shape == (len(idx), ncol, 12)
+    got = xs[idx] if ncol == 1 else np.moveaxis(xs[idx], 2, 1)
+    got = got.reshape(want.shape)
+    for j in range(ncol):
+        d = np.linalg.norm(got[:, j] - want[:, j]) / np.linalg.norm(want[:, j])
+        assert d <= 30 * tol, (case, j, d)
+
 
 @pytest.fixture(scope="module")
 def big():
@@ -39,6 +68,14 @@ def big():
 
 def sampled_rel_l2(got, want):
     return float(np.linalg.norm(got - want) / np.linalg.norm(want))
+
+
+def sampled_resid_bound(tol, o, xs, b, idx, W):
+    """Bound on the oracle-evaluated residual of an fp32 solution, extrapolated from the sites idx (R-RESID):
+    tol (asserted on the library's own `resid`) widened by the sampling error of the extrapolation -- the residual's 12 n
+    complex components are a sample of an approximately Gaussian field, so the estimate of its norm scatters by 1/sqrt(24 n)
+    (3 sigma taken) -- plus the fp32-operator slack of G.fp32_operator_slack on the same sites."""
+    return tol * (1.0 + 3.0 / np.sqrt(24.0 * len(idx))) + G.fp32_operator_slack(o, xs, b, idx=idx, W=W)
 
 
 def test_fullsize_single_rhs_apply_and_solve(big):
@@ -65,11 +102,12 @@ def test_fullsize_single_rhs_apply_and_solve(big):
     x = B.alloc_vec(p)
     tol = 1e-6
     st, it, res = B.ok_bicgstab(W, src, x, tol, 2000, raise_on_fail=False)
-    assert st == 0 and res <= tol and 10 <= it <= 200
+    assert st == 0 and res <= tol
     xs = G.unpack_spinor(p, x, psi.shape)
+    check_against_golden("cfg2", DIMS, it, tol, xs)
     r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
     est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
-    assert est <= 5 * tol, est
+    assert est <= sampled_resid_bound(tol, o, xs, psi, idx, want_W), est
 
 
 def test_fullsize_12rhs_apply_and_solve(big):
@@ -93,8 +131,9 @@ def test_fullsize_12rhs_apply_and_solve(big):
     x = B.alloc_vec(p)
     tol = 1e-6
     st, it, res = B.ok_bicgstab(W, src, x, tol, 2000, raise_on_fail=False)
-    assert st == 0 and res <= tol and 10 <= it <= 200
+    assert st == 0 and res <= tol
     xs = G.unpack_spinor(p, x, b.shape)
+    check_against_golden("cfg3", DIMS, it, tol, xs, ncol=NR)
     # residual by the oracle: exactly on the origin's neighbourhood (where b lives and r is largest), and on a uniform
     # random sample of the remaining sites, extrapolated to the whole lattice
     rng = range(-3, 4)
@@ -106,7 +145,12 @@ def test_fullsize_12rhs_apply_and_solve(big):
     n2 = np.linalg.norm(rn.reshape(-1, NR), axis=0) ** 2
     f2 = (o.V - len(near)) / len(far) * np.linalg.norm(rf.reshape(-1, NR), axis=0) ** 2
     est = np.sqrt(n2 + f2)                                                   # ||b_j|| = 1
-    assert est.max() <= 3 * tol, est
+    # R-RESID for the split-fp16 operands (9 units of 2^-24 |W||x| against the 2 of the fp32 path, tests/test_gpu_mrhs.py);
+    # the near part is exact, the far part (a minor share of the norm) carries the sampling error
+    sl_n = G.fp32_operator_slack(o, xs, b, idx=near) / np.sqrt(o.V / len(near))
+    sl_f = G.fp32_operator_slack(o, xs, b, idx=far) * np.sqrt((o.V - len(near)) / o.V)
+    bound = tol * (1.0 + 3.0 / np.sqrt(24.0 * len(far))) + 4.5 * np.sqrt(sl_n ** 2 + sl_f ** 2)
+    assert np.all(est <= bound), (est, bound)
 
 
 @pytest.mark.parametrize("fmt", [B.OK_W_DS, B.OK_W_CONJ])
@@ -138,7 +182,7 @@ def test_fullsize_reduced_formats_apply_and_mixed_solve(big, fmt):
     xs = G.unpack_spinor(p64, x, psi.shape)
     r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
     est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
-    assert est <= 3 * tol, est
+    assert est <= tol * (1.0 + 3.0 / np.sqrt(24.0 * len(idx))), est       # fp64 operator on both sides: sampling error only
     B.ok_set_workspace(None)
 
 
@@ -166,8 +210,9 @@ def test_fullsize_config5_haar_32x32x32x64():
     x = B.alloc_vec(p)
     tol = 1e-6
     st, it, res = B.ok_bicgstab(W, src, x, tol, 2000, raise_on_fail=False)
-    assert st == 0 and res <= tol and 3 <= it <= 40           # strongly diagonally dominant at kappa = 0.08 (bench: 9 iterations)
+    assert st == 0 and res <= tol                             # strongly diagonally dominant at kappa = 0.08
     xs = G.unpack_spinor(p, x, psi.shape)
+    check_against_golden("cfg4", dims, it, tol, xs)
     r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
     est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
-    assert est <= 5 * tol, est
+    assert est <= sampled_resid_bound(tol, o, xs, psi, idx, want_W), est

@@ -127,7 +127,9 @@ def test_mrhs_bicgstab_vs_oracle(kind):
         assert sto == 0
         its.append(ito)
         r = bj - o.apply_W(np.ascontiguousarray(x[:, :, j]), W=Wc)
-        assert np.linalg.norm(r) / np.linalg.norm(bj) <= 2 * tol
+        # R-RESID with the split-fp16 operands of this mode: W and Psi each carry 2^-22 (2 x 4 units of 2^-24 |W||x|) + 1 unit of
+        # fp32 accumulation = 9 units against the 2 of the fp32 path
+        assert np.linalg.norm(r) / np.linalg.norm(bj) <= tol + 4.5 * G.fp32_operator_slack(o, np.ascontiguousarray(x[:, :, j]), bj, W=Wc)
         assert G.rel_l2(x[:, :, j], xo) <= 20 * tol
     assert abs(it - max(its)) <= 2          # `iters` reports the slowest column
 

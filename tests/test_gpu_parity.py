@@ -199,7 +199,7 @@ def test_bicgstab_fp32_vs_oracle():
     assert st == 0 and abs(it - ito) <= 2 and res <= tol
     # true residual with the fp64 oracle operator on the fp32 solution
     r = b.astype(np.complex64).astype(np.complex128) - o.apply_W(x, W=Wc)
-    assert np.linalg.norm(r) / np.linalg.norm(b) <= 2 * tol
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= tol + G.fp32_operator_slack(o, x, b, W=Wc)      # DESIGN.md 10, R-RESID
     assert G.rel_l2(x, xo) <= 20 * tol
 
 
