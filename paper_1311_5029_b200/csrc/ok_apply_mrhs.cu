@@ -18,15 +18,20 @@
 //       contiguous bytes per warp load, 2-3 L1 wavefronts) straight into tensor memory with tcgen05.st.32x32b --
 //       no conversion arithmetic, no column-maximum pass in the apply.
 //
-// One persistent CTA per SM, 18 warps; sites are dealt in runs of consecutive x (L1 reuse of the gathered records),
-// runs round-robin over the CTAs (all CTAs sweep the lattice together, so the records stay in L2).  Per site 7
-// K-stages of 4 stencil terms (48 k = 24 TMEM columns):
+// One persistent CTA per SM, 12 warps; sites are dealt in runs of consecutive x, runs round-robin over the CTAs (all CTAs
+// sweep the lattice together, so the gathered records stay in L2).  Per site 7 K-stages of 4 stencil terms (48 k = 24
+// TMEM columns):
 //   W loader    1 thread: one 31 488-B bulk copy (cp.async.bulk, L2 evict-first) per site into a 4-slot smem ring.
-//   A producers 8 warps, 4 per TMEM lane quarter (quarter q holds the rows of n = 12q .. 12q+11): gather the 4
-//               neighbour records of a stage (12 LDG.64 per lane), three stages in flight, 3 x tcgen05.st.32x32b.x8
-//               into a 16-slot ring of 24 TMEM columns.
+//   Psi gather  3 warps: each of 9 lanes issues one 1152-B bulk copy of the operand record of neighbour t into a 3-slot smem ring
+//               (a slot = the 27 records of a site).  No register ever waits on a gathered byte: the gathers of site k + 2
+//               are in flight while the tensor core works on site k, however long L2 takes.
+//   A movers    4 warps, (TMEM lane quarter q) x (A slot k % 2): when the records have landed AND the tensor core has
+//               released the slot: 12 LDS.64 (lane <-> A row, conflict-free) + 3 tcgen05.st.32x32b.x8 per stage.  (The first
+//               version of this kernel gathered straight into registers; its fourth stage could only be loaded after the slot
+//               was free, which put one L2 round trip per site on the tensor core's critical path: ncu showed the MMA thread
+//               waiting 40 % of the time for A.)
 //   MMA         1 thread: 3 tcgen05.mma (M = 128: A rows = TMEM lanes; A from tensor memory, B from smem) per stage
-//               into one of two 48-column fp32 accumulators; tcgen05.commit frees the stage / the W slot.
+//               into one of two 48-column fp32 accumulators; tcgen05.commit frees the A slot / the W slot.
 //   epilogue    2 warps (one per lane quarter): tcgen05.ld.16x256b (hi and lo row of an n in one thread), fold the
 //               pieces, combine Re/Im with one shuffle, coalesced 128-B stores; optionally the per-column reductions
 //               <a, out>, ||out||^2 of BiCGStab in fp64 with a fixed order.
@@ -41,11 +46,12 @@ static int g_sm_count = 0;
 
 namespace {
 
-constexpr int kG = 4;                               // producer warps per lane quarter: (site slot 0/1) x (stages 0-3 / 4-6)
-constexpr int kASites = 2;                          // A ring: two whole sites
+constexpr int kASites = 2;                          // A ring (tensor memory): two whole sites
 constexpr int kACols = 24;                          // TMEM columns per stage (48 fp16 k)
 constexpr int kASiteCols = kMrhsStages * kACols;    // 168
 constexpr int kWSlots = 4;                          // W ring (sites)
+constexpr int kPsiSlots = 3;                        // ring of gathered operand records (sites)
+constexpr int kPsiSlotBytes = kTerms * kMrhsOpSiteHalves * 2;     // 31 104
 constexpr int kWSlotBytes = kMrhsStages * kMrhsStageHalves * 2;   // 32 256 (the last 768 B stay zero)
 constexpr int kDCol0 = 384;                         // accumulator 0; accumulator 1 at +64 (A uses columns 0..335)
 constexpr int kTmemCols = 512;
@@ -53,13 +59,21 @@ constexpr int kNbrRing = 8;
 constexpr int kSBO = 128, kLBO = 768;
 
 // warp w may touch TMEM lanes 32 (w % 4) ..; the A rows live in quarters 0 and 1
-constexpr int kWarpMma = 2, kWarpTma = 3, kWarpIdx = 6, kWarpEpi = 4 * kG;
-constexpr int kWarps = 4 * kG + 2, kThreads = kWarps * 32;
-static_assert(kG == 2 * kASites && kASites * kASiteCols <= kDCol0, "A ring layout");
+// movers: warps 0, 1 (slot 0) and 4, 5 (slot 1); epilogue: warps 8, 9
+// gather: warps 7, 10, 11 (issuing a bulk copy costs a warp ~55 cycles, 27 of them would take the whole site period)
+constexpr int kWarpMma = 2, kWarpTma = 3, kWarpIdx = 6, kWarpEpi = 8;
+constexpr int kGatherWarps = 3, kGatherTerms = kTerms / kGatherWarps;
+constexpr int kWarps = 12, kThreads = kWarps * 32;
+static_assert(kGatherWarps * kGatherTerms == kTerms, "gather split");
+static_assert(kASites == 2 && kASites * kASiteCols <= kDCol0, "A ring layout");
 
 constexpr int kSmemW = kWSlots * kWSlotBytes;       // 129 024
+constexpr int kSmemPsi = kPsiSlots * kPsiSlotBytes; // 93 312
 constexpr int kSmemNbr = kNbrRing * 32 * 4;
-constexpr int kSmemBytes = kSmemW + kSmemNbr;
+constexpr int kDotRing = 4;                          // DOT: ring of `dot_a` records (1152 B each), filled by the W loader
+constexpr int kDotRecBytes = kMrhsVecSiteFloats * 4;
+constexpr int kSmemDot = kDotRing * kDotRecBytes;
+constexpr int kSmemBytes = kSmemW + kSmemPsi + kSmemNbr + kSmemDot;
 
 // D f32, A f16, B f16, both K-major, N = 48, M = 128: row r of A and D = TMEM lane r (rows 64..127 are never written or read;
 // M = 64 costs the same 24 cycles but uses only the lower 16 lanes of a quarter)
@@ -69,6 +83,8 @@ constexpr uint32_t kIdesc = (1u << 4) | (0u << 7) | (0u << 10) | ((48u >> 3) << 
 // u - 2, so a warp that skipped a phase of a barrier (a slot that other warps fill in between) could pass early.
 struct Bars {
   uint64_t afull[kASites], aempty[kASites], wfull[kWSlots], wempty[kWSlots], dfull[2], dempty[2], nfull[kNbrRing], nempty[kNbrRing];
+  uint64_t vfull[kDotRing], vempty[kDotRing];   // DOT: the other vector of the reductions, one record per site
+  uint64_t pfull[kPsiSlots], pempty[kPsiSlots]; // gathered operand records
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -189,13 +205,17 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
   __shared__ __align__(8) Bars bars;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   uint8_t* sW = smem;
-  int* sNbr = reinterpret_cast<int*>(smem + kSmemW);
+  uint8_t* sPsi = smem + kSmemW;
+  int* sNbr = reinterpret_cast<int*>(smem + kSmemW + kSmemPsi);
+  const float* sDot = reinterpret_cast<const float*>(smem + kSmemW + kSmemPsi + kSmemNbr);
 
   if (tid == 0) {
-    for (int i = 0; i < kASites; ++i) { mbar_init(&bars.aempty[i], 1); mbar_init(&bars.afull[i], 4); }
+    for (int i = 0; i < kASites; ++i) { mbar_init(&bars.aempty[i], 1); mbar_init(&bars.afull[i], 2); }
+    for (int i = 0; i < kPsiSlots; ++i) { mbar_init(&bars.pfull[i], kGatherWarps); mbar_init(&bars.pempty[i], 4); }
     for (int i = 0; i < kWSlots; ++i) { mbar_init(&bars.wfull[i], 1); mbar_init(&bars.wempty[i], 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&bars.dfull[i], 1); mbar_init(&bars.dempty[i], 2); }
-    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], 4); }
+    for (int i = 0; i < kNbrRing; ++i) { mbar_init(&bars.nfull[i], 1); mbar_init(&bars.nempty[i], kGatherWarps); }
+    for (int i = 0; i < kDotRing; ++i) { mbar_init(&bars.vfull[i], 1); mbar_init(&bars.vempty[i], 2); }
     asm volatile("fence.mbarrier_init.release.cluster;");
     if (blockIdx.x == 0 && out_hdr) {   // out's operand records no longer match; leave a clean header behind
       out_hdr->valid = 0u;
@@ -223,7 +243,6 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
     nsite = mine * run;
     if (mine > 0 && (nruns - 1) % G == b) nsite -= nruns * run - g.V;   // this CTA owns the (possibly short) last run
   }
-  const int total = nsite * kMrhsStages;   // stage iterations of this CTA
 
   if (warp == kWarpMma) {
     // ------------------------------------------------------------------ MMA issuer (one elected thread, warp-uniform path)
@@ -278,6 +297,15 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
                 smem_u32(sW + ws * kWSlotBytes)),
             "l"(src), "r"(kMrhsWSiteBytes), "r"(smem_u32(&bars.wfull[ws])), "l"(policy)
             : "memory");
+        if (DOT) {   // the site's record of the other vector of the fused reductions -> smem (the epilogue never waits on HBM)
+          const int vs = k & (kDotRing - 1);
+          mbar_wait(&bars.vempty[vs], ((uint32_t)(k / kDotRing) & 1u) ^ 1u);
+          mbar_expect_tx(&bars.vfull[vs], kDotRecBytes);
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                           smem_u32(sDot + vs * kMrhsVecSiteFloats)),
+                       "l"(dot_a + (size_t)si.n * kMrhsVecSiteFloats), "r"(kDotRecBytes), "r"(smem_u32(&bars.vfull[vs]))
+                       : "memory");
+        }
         if (++ws == kWSlots) { ws = 0; eph ^= 1u; }
       }
     }
@@ -307,7 +335,7 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
       if (lane == 0) mbar_arrive(&bars.nfull[slot]);
       if (++slot == kNbrRing) { slot = 0; eph ^= 1u; }
     }
-  } else if (warp >= kWarpEpi) {
+  } else if (warp == kWarpEpi || warp == kWarpEpi + 1) {
     // ------------------------------------------------------------------ epilogue: TMEM -> out (+ fused reductions)
     // thread (gq, cp) of half h: rows n%12 = gq + 8h (hi in TMEM lane 16h + gq, lo 8 lanes further), D columns 8i + 2cp + e
     const int q = warp & 3;
@@ -325,15 +353,19 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
     for (int k = 0; k < nsite; ++k, si.next()) {
       const int d = k & 1;
       float a_own[2][3], a_par[2][3];
-      if (DOT) {   // prefetch the other vector of the reductions while the MMAs of this site finish
-        const float* ar = dot_a + (size_t)si.n * kMrhsVecSiteFloats;
+      if (DOT) {   // the other vector of the reductions: staged in smem by the W loader several sites ahead
+        const int vs = k & (kDotRing - 1);
+        mbar_wait(&bars.vfull[vs], (uint32_t)(k / kDotRing) & 1u);
+        const float* ar = sDot + vs * kMrhsVecSiteFloats;
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-          a_own[0][j] = __ldg(ar + j * 96 + off0);
-          a_par[0][j] = __ldg(ar + j * 96 + pof0);
-          a_own[1][j] = on1 ? __ldg(ar + j * 96 + off1) : 0.f;
-          a_par[1][j] = on1 ? __ldg(ar + j * 96 + pof1) : 0.f;
+          a_own[0][j] = ar[j * 96 + off0];
+          a_par[0][j] = ar[j * 96 + pof0];
+          a_own[1][j] = on1 ? ar[j * 96 + off1] : 0.f;
+          a_par[1][j] = on1 ? ar[j * 96 + pof1] : 0.f;
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars.vempty[vs]);
       }
       mbar_wait(&bars.dfull[d], fph);
       fph ^= (uint32_t)d;
@@ -409,45 +441,59 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
         }
       }
     }
-  } else if ((warp & 3) < 2) {
-    // ------------------------------------------------------------------ A producers: operand records (L1/L2) -> TMEM
-    // warp (q, as, h): A rows of lane quarter q, sites k = as, as + 2, ... of this CTA (A ring slot as), stages 0-3 (h = 0) or
-    // 4-6 (h = 1).  Per stage one LDS.128 (4 neighbour indices), 12 LDG.64, 3 tcgen05.st; all loads of the warp's stages are
-    // issued before it waits for the ring slot, so the gathers of site k + 2 fly while the tensor core works on site k.
-    // Lanes 20-23 and 28-31 own no A row: they re-read a neighbouring lane's row (any finite numbers do; their TMEM lanes are
-    // never read), so no lane is predicated off.
-    const int q = warp & 3, as = (warp >> 2) & 1, h = warp >> 3;
-    const int slot = lane < 20 ? lane : (lane < 28 ? lane - 4 : lane - 8);
-    const uint2* pbase = psi_op + q * 72 + slot;               // + 144 site + 24 g   (8-byte units)
-    const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16) + as * kASiteCols;
-    for (int k = as; k < nsite; k += kASites) {
+  } else if (warp == 7 || warp >= 10) {
+    // ------------------------------------------------------------------ Psi gather: 27 neighbour operand records -> smem slot
+    const int gw = warp == 7 ? 0 : warp - 9;      // this warp issues the copies of terms 9 gw .. 9 gw + 8
+    int ps = 0;
+    uint32_t eph = 1;
+    for (int k = 0; k < nsite; ++k) {
       const int ns = k & (kNbrRing - 1);
       mbar_wait(&bars.nfull[ns], (uint32_t)(k / kNbrRing) & 1u);
-      const int* nb = sNbr + ns * 32;
+      mbar_wait(&bars.pempty[ps], eph);
+      if (lane == 0) mbar_expect_tx(&bars.pfull[ps], kGatherTerms * kMrhsOpSiteHalves * 2);
+      __syncwarp();
+      if (lane < kGatherTerms) {
+        const int term = gw * kGatherTerms + lane;
+        const int nb = sNbr[ns * 32 + term];
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                         smem_u32(sPsi + ps * kPsiSlotBytes + term * (kMrhsOpSiteHalves * 2))),
+                     "l"(psi_op + (size_t)nb * (kMrhsOpSiteHalves / 4)), "r"(kMrhsOpSiteHalves * 2), "r"(smem_u32(&bars.pfull[ps]))
+                     : "memory");
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.nempty[ns]);
+      if (++ps == kPsiSlots) { ps = 0; eph ^= 1u; }
+    }
+  } else if (warp < 6) {
+    // ------------------------------------------------------------------ A movers: gathered records (smem) -> tensor memory
+    // warp (q, as): A rows of lane quarter q, sites k = as, as + 2, ... of this CTA (A ring slot as).  Per stage 12 LDS.64 (lane
+    // <-> A row: 24 consecutive 8-byte words, conflict-free) and 3 tcgen05.st.  Lanes 20-23 and 28-31 own no A row: they
+    // re-read a neighbouring lane's row (any finite numbers do; their TMEM lanes are never read), so no lane is predicated off.
+    const int q = warp & 3, as = warp >> 2;
+    const int slot = lane < 20 ? lane : (lane < 28 ? lane - 4 : lane - 8);
+    const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16) + as * kASiteCols;
+    int ps = 0;
+    uint32_t pph = 0;
+    for (int k = 0; k < nsite; ++k, ps = (ps + 1 == kPsiSlots ? 0 : ps + 1), pph ^= (ps == 0 ? 1u : 0u)) {
+      // every mover observes EVERY phase of the record ring and releases every slot (a wait by parity cannot tell phase u from
+      // u - 2), also for the sites the other A slot's movers handle
+      mbar_wait(&bars.pfull[ps], pph);
+      if ((k & 1) != as) {
+        if (lane == 0) mbar_arrive(&bars.pempty[ps]);
+        continue;
+      }
+      const uint2* rec = reinterpret_cast<const uint2*>(sPsi + ps * kPsiSlotBytes) + q * 72 + slot;   // + 144 term + 24 g (8-byte units)
       auto load = [&](int c, uint2 (&w)[12]) {   // w[pair]: TMEM columns 2 pair, 2 pair + 1 of stage c
-        const int4 t = *reinterpret_cast<const int4*>(nb + 4 * c);
         if (c < 6) {       // pair = 4 g + t4: term 4 c + t4, components 4 g .. 4 g + 3
-          const uint2* r0 = pbase + (size_t)t.x * 144;
-          const uint2* r1 = pbase + (size_t)t.y * 144;
-          const uint2* r2 = pbase + (size_t)t.z * 144;
-          const uint2* r3 = pbase + (size_t)t.w * 144;
 #pragma unroll
-          for (int gg = 0; gg < 3; ++gg) {
-            w[4 * gg + 0] = __ldg(r0 + 24 * gg);
-            w[4 * gg + 1] = __ldg(r1 + 24 * gg);
-            w[4 * gg + 2] = __ldg(r2 + 24 * gg);
-            w[4 * gg + 3] = __ldg(r3 + 24 * gg);
-          }
+          for (int gg = 0; gg < 3; ++gg)
+#pragma unroll
+            for (int t4 = 0; t4 < 4; ++t4) w[4 * gg + t4] = rec[(4 * c + t4) * 144 + 24 * gg];
         } else {           // terms 24..26: pair = s = 3 (term - 24) + g, s < 9; pairs 9..11 are the zero pad (W's pad is zero too)
-          const uint2* r0 = pbase + (size_t)t.x * 144;
-          const uint2* r1 = pbase + (size_t)t.y * 144;
-          const uint2* r2 = pbase + (size_t)t.z * 144;
 #pragma unroll
-          for (int gg = 0; gg < 3; ++gg) {
-            w[gg] = __ldg(r0 + 24 * gg);
-            w[3 + gg] = __ldg(r1 + 24 * gg);
-            w[6 + gg] = __ldg(r2 + 24 * gg);
-          }
+          for (int t3 = 0; t3 < 3; ++t3)
+#pragma unroll
+            for (int gg = 0; gg < 3; ++gg) w[3 * t3 + gg] = rec[(24 + t3) * 144 + 24 * gg];
           w[9] = w[10] = w[11] = make_uint2(0u, 0u);
         }
       };
@@ -459,28 +505,18 @@ apply_mrhs_kernel(const uint8_t* __restrict__ W, const uint2* __restrict__ psi_o
                        "r"(w[4 * j + 1].x), "r"(w[4 * j + 1].y), "r"(w[4 * j + 2].x), "r"(w[4 * j + 2].y), "r"(w[4 * j + 3].x), "r"(w[4 * j + 3].y)
                        : "memory");
       };
-      auto indices_read = [&]() {     // this warp is done with the index slot
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bars.nempty[ns]);
-      };
-      auto slot_free = [&]() {        // the tensor core has finished the site that used this ring slot
-        mbar_wait(&bars.aempty[as], ((uint32_t)(k / kASites) & 1u) ^ 1u);
-        tc_fence_after();
-      };
       uint2 v[3][12];
-      if (h == 0) {
-        load(0, v[0]); load(1, v[1]); load(2, v[2]);
-        slot_free();
-        store(0, v[0]);
-        load(3, v[0]);
-        indices_read();
-        store(1, v[1]); store(2, v[2]); store(3, v[0]);
-      } else {
-        load(4, v[0]); load(5, v[1]); load(6, v[2]);
-        indices_read();
-        slot_free();
-        store(4, v[0]); store(5, v[1]); store(6, v[2]);
-      }
+      load(0, v[0]); load(1, v[1]); load(2, v[2]);
+      // the tensor core has finished the site that used this A slot
+      mbar_wait(&bars.aempty[as], ((uint32_t)(k / kASites) & 1u) ^ 1u);
+      tc_fence_after();
+      store(0, v[0]); load(3, v[0]);
+      store(1, v[1]); load(4, v[1]);
+      store(2, v[2]); load(5, v[2]);
+      store(3, v[0]); load(6, v[0]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars.pempty[ps]);     // every record byte this warp needs is in registers
+      store(4, v[1]); store(5, v[2]); store(6, v[0]);
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       tc_fence_before();
       __syncwarp();
