@@ -95,7 +95,8 @@ typedef enum ok_status {
   OK_ECUDA = -2,       /* CUDA runtime or launch error; text via ok_strerror(OK_ECUDA)           */
   OK_EBREAKDOWN = -3,  /* BiCGStab breakdown: |rho|, |<rhat,v>|, <t,t> or |omega| < 1e-300 / NaN */
   OK_EMAXIT = -4,      /* BiCGStab did not converge in maxit iterations (x, iters, resid valid)   */
-  OK_EWORKSPACE = -5   /* workspace missing or smaller than ok_work_bytes                        */
+  OK_EWORKSPACE = -5,  /* workspace missing or smaller than ok_work_bytes                        */
+  OK_ECOMM = -6        /* a caller-supplied ok_comm callback returned non-zero                   */
 } ok_status;
 
 typedef struct ok_params {
@@ -107,7 +108,8 @@ typedef struct ok_params {
   double zeta, rs;    /* Eqs. (2.6)-(2.8)                                                      */
   double cB, cE, cEE, c1, c2, c3, c4, c5;
   int32_t storage;    /* OK_W_DENSE / OK_W_BLOCK / OK_W_DS: how W is held in device memory            */
-  int32_t reserved_;  /* 0                                                                            */
+  int32_t reserved_;  /* 0; OK_SLAB (1) in the parameters of a t-slab (see ok_slab_*): dims[3] is then the slab's    */
+                      /* own extent Tloc and the lattice is open in t (its t-neighbours arrive as halo slices)       */
 } ok_params;
 
 /* ---- sizes (pure host arithmetic; 0 on invalid params) ---------------------------------- */
@@ -173,6 +175,59 @@ int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x
  * device-resident across calls (the paper keeps the precalculation matrices on the GPU and
  * copies the fermion field every call).  Needs the workspace. */
 int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host);
+
+/* ---- t-slab decomposition ------------------------------------------------------------------
+ * The path shards along T: "In the temporal direction, only the nearest neighbors are involved", "off-node
+ * communications are necessary only for the outermost boundary surfaces" (the paper itself runs on 4 nodes,
+ * PAPER.md:120).  The lattice (Lx, Ly, Lz, T) is cut into slabs of Tloc consecutive time slices, slab s owning global
+ * t = t0 .. t0 + Tloc - 1.  W is slab-local and never communicated; per apply one time slice of the spinor (Lx Ly Lz * 96 B
+ * in fp32: 768 KB at 20^3) travels each way between t-neighbours, and a BiCGStab iteration adds four all-gathers of three
+ * doubles per slab.  One process may hold several slabs (that is also how the decomposition is verified on one GPU).
+ *
+ * Slab parameters: an ok_params with dims = {Lx, Ly, Lz, Tloc}, reserved_ = OK_SLAB, nrhs = 1, storage = OK_W_DENSE,
+ * Lx*Ly*Lz a multiple of 32 (a time slice is then a whole number of 32-site blocks), Tloc >= 2, Tloc + 4 <= T.
+ * Slab fields ("extended" internal layout, ok_slab_vec_bytes): [lower halo slice][Tloc slices][upper halo slice], each slice
+ * ok_slab_slice_bytes long; the middle part IS an ordinary internal-layout field of the (Lx, Ly, Lz, Tloc) lattice, so
+ * ok_pack_spinor / ok_unpack_spinor with (base + ok_slab_slice_bytes) convert it.  The library fills the halos itself inside
+ * ok_slab_bicgstab; for ok_slab_dirac_apply the caller puts the neighbours' boundary slices there. */
+#define OK_SLAB 1
+#define OK_SLAB_LINK_HALO 2   /* time slices of links a slab's W needs beyond its own, below and above */
+
+/* Communication between processes, supplied by the caller (torch.distributed in the Python binding: plumbing only).
+ * Both callbacks receive DEVICE pointers, must order their transfers after the work already enqueued on the library's
+ * stream and before work enqueued on it afterwards, and return 0 on success.  NULL callbacks / NULL ok_comm: the process
+ * holds the whole T extent. */
+typedef struct ok_comm {
+  int32_t rank, nranks;     /* consecutive groups of slabs live on consecutive ranks; every rank holds the same number */
+  /* send_lo (this process's first time slice) goes to rank - 1, which receives it in ITS recv_hi; send_hi (the last
+   * slice) goes to rank + 1's recv_lo; ranks are cyclic.  `bytes` each. */
+  int (*exchange)(void* user, const void* send_lo, const void* send_hi, void* recv_lo, void* recv_hi, size_t bytes);
+  /* recv[r * n + i] = send[i] of rank r, for all ranks, n doubles each */
+  int (*allgather)(void* user, const double* send, double* recv, int n);
+  void* user;
+} ok_comm;
+
+size_t ok_slab_slice_bytes(const ok_params* slab);   /* bytes of one time slice of a field, internal layout            */
+size_t ok_slab_vec_bytes(const ok_params* slab);     /* (Tloc + 2) slices                                              */
+/* workspace: ok_slab_precalc_W needs ok_slab_work_bytes(slab, 1, 1); ok_slab_bicgstab over nslab equal slabs in one process
+ * of nranks needs ok_slab_work_bytes(slab, nslab, nranks) */
+size_t ok_slab_work_bytes(const ok_params* slab, int nslab, int nranks);
+
+/* Precalculation of one slab's W (same matrices, Eqs. 2.6-2.12, as ok_precalc_W gives for these sites on the whole lattice).
+ * links_ext: canonical fp64 links [n][mu][3][3] of the Tloc + 2*OK_SLAB_LINK_HALO global time slices
+ * t0 - 2 .. t0 + Tloc + 1 (modulo T), n = x + Lx (y + Ly (z + Lz k)), k = 0 .. Tloc + 3.  The antiperiodic sign of
+ * slab->bc[3] is applied to U_4 of global slice T - 1 wherever it falls in that window.  W: ok_W_bytes(slab). */
+int ok_slab_precalc_W(const void* links_ext, const ok_params* slab, int T_global, int t0, void* W);
+
+/* Eq. (2.2) on one slab: out(x) for the slab's sites; psi_ext must hold the two halo slices.  out_ext's halos are not written. */
+int ok_slab_dirac_apply(const void* W, const void* psi_ext, void* out_ext);
+
+/* BiCGStab (as ok_bicgstab) over the nslab slabs this process holds, in t order (W[s], src_ext[s], x_ext[s] of slab s);
+ * with comm, over nslab * comm->nranks slabs in all.  Every reduction is summed per slab and then over the slabs in global
+ * order, so the iteration is bit-reproducible and independent of how the slabs are dealt to processes.  *iters, *resid as
+ * ok_bicgstab, identical on every process.  Pointer arrays, iters, resid: HOST. */
+int ok_slab_bicgstab(int nslab, const void* const* W, const void* const* src_ext, void* const* x_ext, double tol, int maxit,
+                     const ok_comm* comm, int* iters, double* resid);
 
 /* ---- diagnostics -------------------------------------------------------------------------- */
 /* Read the parameters stored in W's header back into *p (HOST).  Always reads the 1 KiB device header (synchronises the

@@ -243,6 +243,7 @@ int ok_dirac_apply(const void* W, const void* psi, void* out) {
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
+  if (p.reserved_ == OK_SLAB) return OK_EINVAL;   // a t-slab is open in t: ok_slab_dirac_apply
   if (p.nrhs == 12) return mrhs_apply_vec(&p, W_payload(W), const_cast<void*>(psi), out);
   return launch_apply(&p, W_payload(W), psi, out, nullptr, nullptr, nullptr);
 }
@@ -252,6 +253,7 @@ int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host) {
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
+  if (p.reserved_ == OK_SLAB) return OK_EINVAL;
   size_t vb = ok_vec_bytes(&p);
   Geom g = make_geom(&p);
   size_t cb = (size_t)g.V * 12 * 2 * real_bytes(&p) * p.nrhs;   // canonical bytes (no padding)
@@ -274,6 +276,7 @@ int ok_bicgstab(const void* W, const void* src, void* x, double tol, int maxit, 
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
+  if (p.reserved_ == OK_SLAB) return OK_EINVAL;   // ok_slab_bicgstab
   if (p.nrhs == 12) {
     if (!ctx().work || ctx().work_bytes < bicgstab_mrhs_work_bytes(&p)) return OK_EWORKSPACE;
     return run_bicgstab_mrhs(&p, W_payload(W), src, x, tol, maxit, iters, resid);
@@ -287,7 +290,7 @@ int ok_cgnr(const void* W, const void* src, void* x, double tol, int maxit, int*
   ok_params p;
   int st = lookup_W(W, &p);
   if (st) return st;
-  if (p.nrhs != 1) return OK_EINVAL;
+  if (p.nrhs != 1 || p.reserved_ == OK_SLAB) return OK_EINVAL;
   if (!ctx().work || ctx().work_bytes < bicgstab_work_bytes(&p)) return OK_EWORKSPACE;
   return run_cgnr(&p, W_payload(W), src, x, tol, maxit, iters, resid);
 }
@@ -306,11 +309,82 @@ int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x
   int st = lookup_W(W64, &p64);
   if (st) return st;
   if ((st = lookup_W(W32, &p32))) return st;
-  if (p64.precision != OK_FP64 || p32.precision != OK_FP32 || p64.nrhs != 1 || p32.nrhs != 1) return OK_EINVAL;
+  if (p64.precision != OK_FP64 || p32.precision != OK_FP32 || p64.nrhs != 1 || p32.nrhs != 1 || p64.reserved_ || p32.reserved_) return OK_EINVAL;
   for (int d = 0; d < 4; ++d)
     if (p64.dims[d] != p32.dims[d]) return OK_EINVAL;
   if (!ctx().work || ctx().work_bytes < mixed_work_bytes(&p64)) return OK_EWORKSPACE;
   return run_bicgstab_mixed(&p64, W_payload(W64), &p32, W_payload(W32), src, x, tol, inner_tol, maxit, max_outer, iters, outer, resid);
+}
+
+// ---- t-slab decomposition ---------------------------------------------------------------------------------------
+static bool valid_slab(const ok_params* p) {
+  return valid_params(p) && p->reserved_ == OK_SLAB && p->nrhs == 1 && p->storage == OK_W_DENSE &&
+         ((long long)p->dims[0] * p->dims[1] * p->dims[2]) % kBlock == 0;
+}
+
+size_t ok_slab_slice_bytes(const ok_params* p) {
+  if (!valid_slab(p)) return 0;
+  return (size_t)p->dims[0] * p->dims[1] * p->dims[2] * 12 * 2 * real_bytes(p);
+}
+
+size_t ok_slab_vec_bytes(const ok_params* p) { return valid_slab(p) ? (size_t)(p->dims[3] + 2) * ok_slab_slice_bytes(p) : 0; }
+
+static ok_params slab_link_lattice(const ok_params* p) {   // the lattice the slab's link window lives on
+  ok_params e = *p;
+  e.dims[3] = p->dims[3] + 2 * OK_SLAB_LINK_HALO;
+  e.reserved_ = 0;
+  return e;
+}
+
+size_t ok_slab_work_bytes(const ok_params* p, int nslab, int nranks) {
+  if (!valid_slab(p) || nslab < 1 || nranks < 1) return 0;
+  const ok_params e = slab_link_lattice(p);
+  const size_t a = precalc_work_bytes(&e), b = (size_t)nslab * bicgstab_slab_work_bytes(p) + bicgstab_slab_shared_bytes(nslab, nranks);
+  return (a > b ? a : b) + 4096;
+}
+
+int ok_slab_precalc_W(const void* links_ext, const ok_params* p, int T, int t0, void* W) {
+  if (!valid_slab(p) || !aligned16(links_ext) || !aligned16(W)) return OK_EINVAL;
+  const int Tloc = p->dims[3], H = OK_SLAB_LINK_HALO;
+  if (T < Tloc + 2 * H || t0 < 0 || t0 >= T) return OK_EINVAL;
+  const ok_params e = slab_link_lattice(p);
+  if (!ctx().work || ctx().work_bytes < precalc_work_bytes(&e)) return OK_EWORKSPACE;
+  int st = bind_device();
+  if (st) return st;
+  if ((st = write_header(W, p))) return st;
+  // window slice k holds global t = t0 - H + k (mod T): where is T - 1 ?
+  int k = ((T - 1) - (t0 - H)) % T;
+  if (k < 0) k += T;
+  const int tfold = k < Tloc + 2 * H ? k : -1;
+  const int slice_blocks = p->dims[0] * p->dims[1] * p->dims[2] / kBlock;
+  return launch_precalc_window(&e, links_ext, W_payload(W), ctx().work, tfold, H * slice_blocks, Tloc * slice_blocks);
+}
+
+int ok_slab_dirac_apply(const void* W, const void* psi, void* out) {
+  if (!aligned16(psi) || !aligned16(out) || psi == out) return OK_EINVAL;
+  ok_params p;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  if (!valid_slab(&p)) return OK_EINVAL;
+  return launch_apply_slab(&p, W_payload(W), psi, out, nullptr, nullptr);
+}
+
+int ok_slab_bicgstab(int nslab, const void* const* W, const void* const* src, void* const* x, double tol, int maxit, const ok_comm* comm,
+                     int* iters, double* resid) {
+  if (nslab < 1 || nslab > 64 || !W || !src || !x || !iters || !resid || !(tol > 0.0) || maxit < 1) return OK_EINVAL;
+  if (comm && (comm->nranks < 1 || comm->rank < 0 || comm->rank >= comm->nranks)) return OK_EINVAL;
+  static ok_params ps[64];
+  const ok_params* pp[64];
+  const void* payload[64];
+  for (int i = 0; i < nslab; ++i) {
+    if (!aligned16(src[i]) || !aligned16(x[i]) || src[i] == x[i]) return OK_EINVAL;
+    int st = lookup_W(W[i], &ps[i]);
+    if (st) return st;
+    if (!valid_slab(&ps[i]) || ps[i].precision != ps[0].precision) return OK_EINVAL;
+    pp[i] = &ps[i];
+    payload[i] = W_payload(W[i]);
+  }
+  return run_bicgstab_slabs(nslab, pp, payload, src, x, tol, maxit, comm, iters, resid);
 }
 
 int ok_W_unit_index(int storage, int term, int row, int col, int* info) {
@@ -328,6 +402,7 @@ const char* ok_strerror(int status) {
     case OK_EBREAKDOWN: return "BiCGStab breakdown";
     case OK_EMAXIT: return "BiCGStab: maximum iterations reached without convergence";
     case OK_EWORKSPACE: return "workspace missing or too small (see ok_work_bytes / ok_set_workspace)";
+    case OK_ECOMM: return "an ok_comm callback reported a failure";
     default: return "unknown status";
   }
 }

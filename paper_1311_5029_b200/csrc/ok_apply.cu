@@ -48,15 +48,18 @@ __device__ __forceinline__ int wrap(int x, int L) {
 template <typename real, int RPT, bool DOT>
 __global__ void __launch_bounds__(32 * (12 / RPT))
 apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typename Vec<real>::type* __restrict__ psi,
-                    typename Vec<real>::type* __restrict__ out, Geom g,
+                    typename Vec<real>::type* __restrict__ out, Geom g, int vblk0,
                     const typename Vec<real>::type* __restrict__ dot_a, double* __restrict__ partials) {
   using vec_t = typename Vec<real>::type;
   constexpr int NC = Vec<real>::NC;
   constexpr int NW = 12 / RPT;
   const int lane = threadIdx.x & 31;
   const int rg = threadIdx.x >> 5;
-  const int blk = blockIdx.x;
-  int n = blk * kBlock + lane;
+  // blk: 32-site block of W (and of the partial sums); vblk: the same sites' block in the spinor fields, whose lattice is g.
+  // Whole lattice: vblk0 = 0.  t-slab (ok_slab_dirac_apply): the fields carry one halo time slice below and above the slab,
+  // g is that extended lattice and vblk0 the blocks of one slice, so the +-t neighbours of the boundary slices are the halos.
+  const int blk = blockIdx.x, vblk = blk + vblk0;
+  int n = vblk * kBlock + lane;
   if (n >= g.V) n = 0;   // padded lane: W is zero there, the result is zero
   const int x = n % g.L[0];
   int q = n / g.L[0];
@@ -94,7 +97,7 @@ apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typena
   }
 
   // store: row -> (unit c, sub) of the internal spinor layout
-  real* ob = reinterpret_cast<real*>(out + (size_t)blk * NC * kBlock);
+  real* ob = reinterpret_cast<real*>(out + (size_t)vblk * NC * kBlock);
   constexpr int RPU = 12 / NC;   // rows (components) per 16-byte unit: 2 (fp32) or 1 (fp64)
 #pragma unroll
   for (int r = 0; r < RPT; ++r) {
@@ -109,7 +112,7 @@ apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typena
 
   if constexpr (DOT) {
     // partials[blk] = ( Re<a,out>, Im<a,out>, ||out||^2 ), fp64, fixed summation order
-    const real* ab = reinterpret_cast<const real*>(dot_a + (size_t)blk * NC * kBlock);
+    const real* ab = reinterpret_cast<const real*>(dot_a + (size_t)vblk * NC * kBlock);
     double d0 = 0.0, d1 = 0.0, d2 = 0.0;
 #pragma unroll
     for (int r = 0; r < RPT; ++r) {
@@ -144,16 +147,16 @@ apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typena
 
 template <typename real, int RPT>
 static int launch_direct(const Geom& g, const void* W, const void* psi, void* out, double* partials,
-                         const void* dot_a) {
+                         const void* dot_a, int nblk = -1, int vblk0 = 0) {
   using vec_t = typename Vec<real>::type;
-  dim3 grid(g.nblk), block(32 * (12 / RPT));
+  dim3 grid(nblk < 0 ? g.nblk : nblk), block(32 * (12 / RPT));
   if (partials)
     apply_direct_kernel<real, RPT, true><<<grid, block, 0, ctx().stream>>>(
-        static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g,
+        static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g, vblk0,
         static_cast<const vec_t*>(dot_a), partials);
   else
     apply_direct_kernel<real, RPT, false><<<grid, block, 0, ctx().stream>>>(
-        static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g, nullptr, nullptr);
+        static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g, vblk0, nullptr, nullptr);
   OK_LAUNCHED("apply_direct_kernel");
   return OK_SUCCESS;
 }
@@ -169,6 +172,23 @@ int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, 
   Geom g = make_geom(p);
   if (p->precision == OK_FP64) return launch_direct<double, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
   return launch_direct<float, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
+}
+
+// t-slab apply (ok_slab.cu): p = the slab's own lattice (Lx, Ly, Lz, Tloc) whose W this is; psi, out, dot_a are fields of the
+// extended lattice (Lx, Ly, Lz, Tloc + 2) in the internal layout, i.e. [lower halo slice][Tloc slices][upper halo slice].
+int launch_apply_slab(const ok_params* p, const void* W, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext) {
+  if (p->nrhs != 1 || p->storage != OK_W_DENSE) return OK_EINVAL;
+  int st = upload_offsets();
+  if (st) return st;
+  const Geom g = make_geom(p);
+  const int slice = p->dims[0] * p->dims[1] * p->dims[2];
+  if (slice % kBlock) return OK_EINVAL;
+  Geom ge = g;
+  ge.L[3] = g.L[3] + 2;
+  ge.V = g.V + 2 * slice;
+  ge.nblk = ge.V / kBlock;
+  if (p->precision == OK_FP64) return launch_direct<double, kRowsPerWarp>(ge, W, psi_ext, out_ext, partials, dot_a_ext, g.nblk, slice / kBlock);
+  return launch_direct<float, kRowsPerWarp>(ge, W, psi_ext, out_ext, partials, dot_a_ext, g.nblk, slice / kBlock);
 }
 
 }  // namespace okd

@@ -164,34 +164,9 @@ k_residual(const typename C2<real>::type* __restrict__ b, const typename C2<real
 // ---- single-CTA finalisers: sum `count` partial triples in fixed order, update the scalars ---
 enum Stage { FIN_INIT = 0, FIN_V = 1, FIN_T = 2, FIN_XR = 3, FIN_RES = 4 };
 
+// the BiCGStab scalars from the three totals of a reduction stage (one thread)
 template <int STAGE>
-__global__ void __launch_bounds__(kVecThreads) k_finalize(const double* __restrict__ partials, int count, Scal* sc) {
-  // thread-serial sum in a fixed order; the loads of 8 consecutive strides are issued together (latency, not order, changes)
-  constexpr bool kThree = STAGE == FIN_V || STAGE == FIN_T || STAGE == FIN_XR;
-  double d[3] = {0.0, 0.0, 0.0};
-  int i = threadIdx.x;
-  for (; i + 7 * kVecThreads < count; i += 8 * kVecThreads) {
-    double v[8][3];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      const double* q = partials + (size_t)(i + u * kVecThreads) * 3;
-      v[u][0] = q[0];
-      v[u][1] = kThree ? q[1] : 0.0;
-      v[u][2] = kThree ? q[2] : 0.0;
-    }
-#pragma unroll
-    for (int u = 0; u < 8; ++u) { d[0] += v[u][0]; d[1] += v[u][1]; d[2] += v[u][2]; }
-  }
-  for (; i < count; i += kVecThreads) {
-    d[0] += partials[(size_t)i * 3 + 0];
-    if (kThree) {
-      d[1] += partials[(size_t)i * 3 + 1];
-      d[2] += partials[(size_t)i * 3 + 2];
-    }
-  }
-  __shared__ double tot[3];
-  block_reduce<3>(d, tot);
-  if (threadIdx.x != 0) return;
+__device__ __forceinline__ void update_scalars(const double (&tot)[3], Scal* sc) {
   if (STAGE == FIN_INIT) {
     sc->bnorm2 = tot[0]; sc->rr = tot[0];
     sc->rho[0] = tot[0]; sc->rho[1] = 0.0;
@@ -228,6 +203,37 @@ __global__ void __launch_bounds__(kVecThreads) k_finalize(const double* __restri
     sc->beta[1] = q0 * a1 + q1 * a0;
     sc->rho[0] = nr; sc->rho[1] = ni;
   }
+}
+
+template <int STAGE>
+__global__ void __launch_bounds__(kVecThreads) k_finalize(const double* __restrict__ partials, int count, Scal* sc) {
+  // thread-serial sum in a fixed order; the loads of 8 consecutive strides are issued together (latency, not order, changes)
+  constexpr bool kThree = STAGE == FIN_V || STAGE == FIN_T || STAGE == FIN_XR;
+  double d[3] = {0.0, 0.0, 0.0};
+  int i = threadIdx.x;
+  for (; i + 7 * kVecThreads < count; i += 8 * kVecThreads) {
+    double v[8][3];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const double* q = partials + (size_t)(i + u * kVecThreads) * 3;
+      v[u][0] = q[0];
+      v[u][1] = kThree ? q[1] : 0.0;
+      v[u][2] = kThree ? q[2] : 0.0;
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { d[0] += v[u][0]; d[1] += v[u][1]; d[2] += v[u][2]; }
+  }
+  for (; i < count; i += kVecThreads) {
+    d[0] += partials[(size_t)i * 3 + 0];
+    if (kThree) {
+      d[1] += partials[(size_t)i * 3 + 1];
+      d[2] += partials[(size_t)i * 3 + 2];
+    }
+  }
+  __shared__ double tot[3];
+  block_reduce<3>(d, tot);
+  if (threadIdx.x != 0) return;
+  update_scalars<STAGE>(tot, sc);
 }
 
 // -------------------------------------------------------------------------------------------
@@ -345,6 +351,265 @@ int run_bicgstab(const ok_params* p, const void* W, const void* src, void* x, do
   if (p->nrhs != 1) return OK_EINVAL;
   if (p->precision == OK_FP64) return solve<double>(p, W, src, x, tol, maxit, iters, resid);
   return solve<float>(p, W, src, x, tol, maxit, iters, resid);
+}
+
+// =====================================================================================================
+// t-slab decomposition: the same BiCGStab over a lattice cut along T into slabs.
+// "In the temporal direction, only the nearest neighbors are involved" and "off-node communications are
+// necessary only for the outermost boundary surfaces": W is slab-local, a slab's fields carry one halo
+// time slice below and above (ok.h), and before every apply each slab's halos are refreshed from its t-neighbours --
+// device copies between the slabs of this process, the caller's `exchange` for the two outer faces.  Reductions:
+// per-CTA partials (as above) -> one fixed-order total per SLAB -> (all-gather over processes) -> sum over all slabs in
+// global slab order -> scalars.  The result therefore depends on the number of slabs, not on how they are dealt to
+// processes; every process computes identical scalars.
+template <bool THREE>
+__global__ void __launch_bounds__(kVecThreads)
+k_slab_sum(const double* __restrict__ partials, const int* __restrict__ first, const int* __restrict__ count, double* __restrict__ slabtot) {
+  const double* q = partials + (size_t)first[blockIdx.x] * 3;
+  const int n = count[blockIdx.x];
+  double d[3] = {0.0, 0.0, 0.0};
+  for (int i = threadIdx.x; i < n; i += kVecThreads) {
+    d[0] += q[(size_t)i * 3 + 0];
+    if (THREE) {
+      d[1] += q[(size_t)i * 3 + 1];
+      d[2] += q[(size_t)i * 3 + 2];
+    }
+  }
+  block_reduce<3>(d, slabtot + (size_t)blockIdx.x * 3);
+}
+
+template <int STAGE>
+__global__ void k_slab_scalars(const double* __restrict__ slabtot, int nslab_all, Scal* sc) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double tot[3] = {0.0, 0.0, 0.0};
+  for (int i = 0; i < nslab_all; ++i) {   // global slab order
+    tot[0] += slabtot[(size_t)i * 3 + 0];
+    tot[1] += slabtot[(size_t)i * 3 + 1];
+    tot[2] += slabtot[(size_t)i * 3 + 2];
+  }
+  update_scalars<STAGE>(tot, sc);
+}
+
+size_t bicgstab_slab_work_bytes(const ok_params* p) {   // per slab; p: the slab's own lattice
+  if (p->nrhs != 1) return 0;
+  Geom g = make_geom(p);
+  const size_t slice = (size_t)p->dims[0] * p->dims[1] * p->dims[2];
+  const size_t vb = align_up(((size_t)g.V + 2 * slice) * 24 * real_bytes(p), 256);
+  return 6 * vb + align_up((size_t)g.nblk * 3 * sizeof(double), 256);
+}
+size_t bicgstab_slab_shared_bytes(int nslab, int nranks) {   // once per solve
+  return align_up((size_t)nslab * 3 * sizeof(int), 256) + align_up((size_t)nslab * 3 * sizeof(double), 256) +
+         align_up((size_t)nslab * (size_t)nranks * 3 * sizeof(double), 256) + 256;
+}
+
+template <typename real>
+static int solve_slabs(int nslab, const ok_params* const* ps, const void* const* Ws, const void* const* srcs, void* const* xs, double tol,
+                       int maxit, const ok_comm* comm, int* iters, double* resid) {
+  using c2 = typename C2<real>::type;
+  cudaStream_t st = ctx().stream;
+  const int nranks = comm ? comm->nranks : 1;
+  struct Slab {
+    const ok_params* p;
+    const void* W;
+    Geom g;
+    long long halo, ncomplex;   // complex elements of one time slice; of the interior
+    size_t slice_bytes;
+    int ngrp, pfirst;
+    c2 *r, *rhat, *pp, *v, *s, *t, *x;   // extended fields (base pointers)
+    const c2* b;
+  };
+  Slab sl[64];
+  if (nslab < 1 || nslab > 64) return OK_EINVAL;
+  char* w = static_cast<char*>(ctx().work);
+  size_t need = 0;
+  int nblk_all = 0;
+  for (int i = 0; i < nslab; ++i) {
+    Slab& a = sl[i];
+    a.p = ps[i];
+    a.W = Ws[i];
+    a.g = make_geom(ps[i]);
+    a.halo = (long long)ps[i]->dims[0] * ps[i]->dims[1] * ps[i]->dims[2] * 12;
+    a.ncomplex = (long long)a.g.V * 12;
+    a.slice_bytes = (size_t)a.halo * 2 * sizeof(real);
+    a.ngrp = (a.g.nblk + kBlocksPerCta - 1) / kBlocksPerCta;
+    a.pfirst = nblk_all;
+    nblk_all += a.g.nblk;
+    const size_t vb = align_up((size_t)(a.ncomplex + 2 * a.halo) * 2 * sizeof(real), 256);
+    c2** f[6] = {&a.r, &a.rhat, &a.pp, &a.v, &a.s, &a.t};
+    for (int k = 0; k < 6; ++k) {
+      *f[k] = reinterpret_cast<c2*>(w + need);
+      need += vb;
+    }
+    a.x = static_cast<c2*>(xs[i]);
+    a.b = static_cast<const c2*>(srcs[i]);
+    if (i > 0 && (ps[i]->dims[0] != ps[0]->dims[0] || ps[i]->dims[1] != ps[0]->dims[1] || ps[i]->dims[2] != ps[0]->dims[2])) return OK_EINVAL;
+  }
+  double* partials = reinterpret_cast<double*>(w + need);
+  need += align_up((size_t)nblk_all * 3 * sizeof(double), 256);
+  int* d_first = reinterpret_cast<int*>(w + need);          // [nslab] first partial triple of a slab
+  int* d_cnt_apply = d_first + nslab;                       // [nslab] triples written by the apply (one per 32-site block)
+  int* d_cnt_vec = d_first + 2 * nslab;                     // [nslab] triples written by a vector kernel (one per CTA)
+  need += align_up((size_t)nslab * 3 * sizeof(int), 256);
+  double* slabtot = reinterpret_cast<double*>(w + need);    // [nslab][3]
+  need += align_up((size_t)nslab * 3 * sizeof(double), 256);
+  double* gathered = reinterpret_cast<double*>(w + need);   // [nranks][nslab][3]
+  need += align_up((size_t)nslab * nranks * 3 * sizeof(double), 256);
+  Scal* sc = reinterpret_cast<Scal*>(w + need);
+  need += 256;
+  if (!ctx().work || ctx().work_bytes < need) return OK_EWORKSPACE;
+  {
+    int hbuf[3 * 64];
+    for (int i = 0; i < nslab; ++i) {
+      hbuf[i] = sl[i].pfirst;
+      hbuf[nslab + i] = sl[i].g.nblk;
+      hbuf[2 * nslab + i] = sl[i].ngrp;
+    }
+    OK_CUDA(cudaMemcpyAsync(d_first, hbuf, (size_t)nslab * 3 * sizeof(int), cudaMemcpyHostToDevice, st));   // pageable source: copied before return
+  }
+
+  static Scal* h = nullptr;
+  static cudaEvent_t ev = nullptr;
+  if (!h) OK_CUDA(cudaHostAlloc(reinterpret_cast<void**>(&h), sizeof(Scal), cudaHostAllocDefault));
+  if (!ev) OK_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+  int rc;
+#define OK_TRY(e) do { if ((rc = (e))) return rc; } while (0)
+  auto fetch = [&]() -> int {
+    OK_CUDA(cudaMemcpyAsync(h, sc, sizeof(Scal), cudaMemcpyDeviceToHost, st));
+    OK_CUDA(cudaEventRecord(ev, st));
+    return OK_SUCCESS;
+  };
+  auto wait = [&]() -> int {
+    OK_CUDA(cudaEventSynchronize(ev));
+    return OK_SUCCESS;
+  };
+  // one reduction stage: slab totals -> all slabs of all processes in global order -> scalars
+  auto finalize = [&](int stage, bool from_apply) -> int {
+    const bool three = stage == FIN_V || stage == FIN_T || stage == FIN_XR;
+    const int* cnt = from_apply ? d_cnt_apply : d_cnt_vec;
+    if (three) k_slab_sum<true><<<nslab, kVecThreads, 0, st>>>(partials, d_first, cnt, slabtot);
+    else k_slab_sum<false><<<nslab, kVecThreads, 0, st>>>(partials, d_first, cnt, slabtot);
+    OK_LAUNCHED("k_slab_sum");
+    const double* all = slabtot;
+    if (comm && comm->allgather) {
+      if (comm->allgather(comm->user, slabtot, gathered, 3 * nslab)) return OK_ECOMM;
+      all = gathered;
+    }
+    const int n = nslab * nranks;
+    switch (stage) {
+      case FIN_INIT: k_slab_scalars<FIN_INIT><<<1, 32, 0, st>>>(all, n, sc); break;
+      case FIN_V: k_slab_scalars<FIN_V><<<1, 32, 0, st>>>(all, n, sc); break;
+      case FIN_T: k_slab_scalars<FIN_T><<<1, 32, 0, st>>>(all, n, sc); break;
+      case FIN_XR: k_slab_scalars<FIN_XR><<<1, 32, 0, st>>>(all, n, sc); break;
+      default: k_slab_scalars<FIN_RES><<<1, 32, 0, st>>>(all, n, sc); break;
+    }
+    OK_LAUNCHED("k_slab_scalars");
+    return OK_SUCCESS;
+  };
+  // halo refresh of one field of every slab; sel picks the field
+  auto halos = [&](c2* Slab::*field) -> int {
+    auto lo_halo = [&](Slab& a) { return reinterpret_cast<char*>(a.*field); };
+    auto first_slice = [&](Slab& a) { return reinterpret_cast<char*>(a.*field) + a.slice_bytes; };
+    auto last_slice = [&](Slab& a) { return reinterpret_cast<char*>(a.*field) + (size_t)a.p->dims[3] * a.slice_bytes; };
+    auto hi_halo = [&](Slab& a) { return reinterpret_cast<char*>(a.*field) + (size_t)(a.p->dims[3] + 1) * a.slice_bytes; };
+    const size_t nb = sl[0].slice_bytes;
+    for (int i = 0; i + 1 < nslab; ++i) {
+      OK_CUDA(cudaMemcpyAsync(hi_halo(sl[i]), first_slice(sl[i + 1]), nb, cudaMemcpyDeviceToDevice, st));
+      OK_CUDA(cudaMemcpyAsync(lo_halo(sl[i + 1]), last_slice(sl[i]), nb, cudaMemcpyDeviceToDevice, st));
+    }
+    Slab &a0 = sl[0], &a1 = sl[nslab - 1];
+    if (comm && comm->exchange) {
+      if (comm->exchange(comm->user, first_slice(a0), last_slice(a1), lo_halo(a0), hi_halo(a1), nb)) return OK_ECOMM;
+    } else {   // this process holds the whole T extent: periodic closure (the boundary condition sits in W)
+      OK_CUDA(cudaMemcpyAsync(lo_halo(a0), last_slice(a1), nb, cudaMemcpyDeviceToDevice, st));
+      OK_CUDA(cudaMemcpyAsync(hi_halo(a1), first_slice(a0), nb, cudaMemcpyDeviceToDevice, st));
+    }
+    return OK_SUCCESS;
+  };
+#define OK_INT(a, f) ((a).f + (a).halo)   /* interior of an extended field */
+  for (int i = 0; i < nslab; ++i) {
+    Slab& a = sl[i];
+    k_init<real><<<a.ngrp, kVecThreads, 0, st>>>(OK_INT(a, b), OK_INT(a, x), OK_INT(a, r), OK_INT(a, rhat), OK_INT(a, pp), a.ncomplex,
+                                               partials + (size_t)a.pfirst * 3);
+    OK_LAUNCHED("k_init");
+  }
+  OK_TRY(finalize(FIN_INIT, false));
+  OK_TRY(fetch());
+  OK_TRY(wait());
+  const double bnorm2 = h->bnorm2;
+  *iters = 0;
+  if (!(bnorm2 > 0.0)) {
+    *resid = 0.0;
+    return isnan(bnorm2) ? OK_EBREAKDOWN : OK_SUCCESS;
+  }
+  const double target = tol * tol * bnorm2;
+  auto apply_all = [&](c2* Slab::*in, c2* Slab::*out, c2* Slab::*dot) -> int {
+    OK_TRY(halos(in));
+    for (int i = 0; i < nslab; ++i) {
+      Slab& a = sl[i];
+      OK_TRY(launch_apply_slab(a.p, a.W, a.*in, a.*out, dot ? partials + (size_t)a.pfirst * 3 : nullptr, dot ? a.*dot : nullptr));
+    }
+    return OK_SUCCESS;
+  };
+  auto true_residual = [&]() -> int {
+    OK_TRY(apply_all(&Slab::x, &Slab::t, nullptr));
+    for (int i = 0; i < nslab; ++i) {
+      Slab& a = sl[i];
+      k_residual<real><<<a.ngrp, kVecThreads, 0, st>>>(OK_INT(a, b), OK_INT(a, t), OK_INT(a, r), OK_INT(a, rhat), OK_INT(a, pp), a.ncomplex,
+                                                     partials + (size_t)a.pfirst * 3);
+      OK_LAUNCHED("k_residual");
+    }
+    OK_TRY(finalize(FIN_RES, false));
+    OK_TRY(fetch());
+    OK_TRY(wait());
+    return OK_SUCCESS;
+  };
+  int status = OK_EMAXIT;
+  int it = 0;
+  while (it < maxit) {
+    ++it;
+    OK_TRY(apply_all(&Slab::pp, &Slab::v, &Slab::rhat));   // v = M p, <rhat,v>
+    OK_TRY(finalize(FIN_V, true));
+    for (int i = 0; i < nslab; ++i) {
+      Slab& a = sl[i];
+      k_s_update<real><<<a.ngrp, kVecThreads, 0, st>>>(OK_INT(a, r), OK_INT(a, v), OK_INT(a, s), a.ncomplex, sc);
+      OK_LAUNCHED("k_s_update");
+    }
+    OK_TRY(apply_all(&Slab::s, &Slab::t, &Slab::s));       // t = M s, <s,t>, <t,t>
+    OK_TRY(finalize(FIN_T, true));
+    for (int i = 0; i < nslab; ++i) {
+      Slab& a = sl[i];
+      k_xr_update<real><<<a.ngrp, kVecThreads, 0, st>>>(OK_INT(a, x), OK_INT(a, pp), OK_INT(a, s), OK_INT(a, t), OK_INT(a, r), OK_INT(a, rhat),
+                                                      a.ncomplex, sc, partials + (size_t)a.pfirst * 3);
+      OK_LAUNCHED("k_xr_update");
+    }
+    OK_TRY(finalize(FIN_XR, false));
+    OK_TRY(fetch());
+    for (int i = 0; i < nslab; ++i) {
+      Slab& a = sl[i];
+      k_p_update<real><<<a.ngrp, kVecThreads, 0, st>>>(OK_INT(a, pp), OK_INT(a, r), OK_INT(a, v), a.ncomplex, sc);
+      OK_LAUNCHED("k_p_update");
+    }
+    OK_TRY(wait());
+    if (h->breakdown & 3) { status = OK_EBREAKDOWN; break; }
+    if (h->rr <= target) {
+      OK_TRY(true_residual());
+      if (h->rr <= target) { status = OK_SUCCESS; break; }
+      continue;
+    }
+    if ((h->breakdown & 4) || isnan(h->rr)) { status = OK_EBREAKDOWN; break; }
+  }
+  if (status != OK_SUCCESS) OK_TRY(true_residual());
+  *iters = it;
+  *resid = sqrt(h->rr / bnorm2);
+#undef OK_INT
+#undef OK_TRY
+  return status;
+}
+
+int run_bicgstab_slabs(int nslab, const ok_params* const* ps, const void* const* Ws, const void* const* srcs, void* const* xs, double tol,
+                       int maxit, const ok_comm* comm, int* iters, double* resid) {
+  if (ps[0]->precision == OK_FP64) return solve_slabs<double>(nslab, ps, Ws, srcs, xs, tol, maxit, comm, iters, resid);
+  return solve_slabs<float>(nslab, ps, Ws, srcs, xs, tol, maxit, comm, iters, resid);
 }
 
 }  // namespace okd

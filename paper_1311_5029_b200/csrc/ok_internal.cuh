@@ -211,6 +211,13 @@ int launch_pack_W(const ok_params* p, const void* canon, void* Wpayload, bool un
 int launch_apply(const ok_params* p, const void* Wpayload, const void* psi, void* out,
                  double* dot_partials /* nullable */, const void* dot_a, const void* dot_b);
 int launch_precalc(const ok_params* p, const void* links, void* Wpayload, void* work);
+int launch_precalc_window(const ok_params* p, const void* links, void* Wpayload, void* work, int tfold, int win_blk0, int win_nblk);
+// t-slab decomposition (ok.h): p = the slab's own lattice
+int launch_apply_slab(const ok_params* p, const void* Wpayload, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext);
+size_t bicgstab_slab_work_bytes(const ok_params* p);
+size_t bicgstab_slab_shared_bytes(int nslab, int nranks);
+int run_bicgstab_slabs(int nslab, const ok_params* const* ps, const void* const* Wpayloads, const void* const* srcs, void* const* xs,
+                       double tol, int maxit, const ok_comm* comm, int* iters, double* resid);
 int launch_apply_sparse(const ok_params* p, const void* Wpayload, const void* psi, void* out, double* dot_partials, const void* dot_a);
 size_t precalc_work_bytes(const ok_params* p);
 int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,

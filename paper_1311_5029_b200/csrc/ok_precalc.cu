@@ -36,7 +36,9 @@ struct PrecalcArgs {
   int storage;                 // OK_W_DENSE / OK_W_BLOCK / OK_W_DS (ok_sparse.cuh)
   int pair;                    // 1: the thread of a positive-direction term also writes the opposite term of the neighbour site
   int posonly;                 // 1: grid over W^0 and the 13 positive-direction terms only (pair, or OK_W_CONJ)
-  int blk0;                    // first 32-site block of this launch (12-RHS: the dense W of a chunk goes to a bounce buffer)
+  int blk0;                    // first 32-site block of this launch (12-RHS: the dense W of a chunk goes to a bounce buffer;
+                               // t-slab: the first interior block of the extended link window)
+  int tfold;                   // time slice whose U_4 carries bc[3] (L[3] - 1 on a whole lattice; t-slab: where global T - 1 sits, or -1)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
   double s4;                   // c_EE / (2 u0^4)      (Eq. 2.7)
@@ -142,7 +144,7 @@ __device__ __forceinline__ Site shift(Site s, int mu, int d, const Geom& g) {   
 // U_mu(x) with the boundary-condition sign folded in.
 __device__ __forceinline__ cm3 ldU(const double2* __restrict__ links, const Site& s, int mu, const PrecalcArgs& a) {
   const double2* p = links + ((size_t)index_of(s, a.g) * 4 + mu) * 9;
-  const double sg = (a.bc[mu] < 0 && s.c[mu] == a.g.L[mu] - 1) ? -1.0 : 1.0;
+  const double sg = (a.bc[mu] < 0 && s.c[mu] == (mu == 3 ? a.tfold : a.g.L[mu] - 1)) ? -1.0 : 1.0;
   cm3 r;
 #pragma unroll
   for (int i = 0; i < 9; ++i) {
@@ -530,6 +532,13 @@ size_t precalc_work_bytes(const ok_params* p) {
 }
 
 int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) {
+  return launch_precalc_window(p, links, Wp, work, p->dims[3] - 1, 0, -1);
+}
+
+// p: the lattice the LINKS live on.  win_nblk < 0: W of the whole lattice.  Otherwise (t-slab, ok_slab.cu): W of the
+// 32-site blocks [win_blk0, win_blk0 + win_nblk) only, written compactly to Wp, every term assembled by its own thread
+// (the partner site of the pairing trick may lie outside the window); nrhs = 1, OK_W_DENSE.
+int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void* work, int tfold, int win_blk0, int win_nblk) {
   if (!g_poff_uploaded) {
     OK_CUDA(cudaMemcpyToSymbol(c_poff, kOffsets, sizeof(kOffsets)));
     static int h[3][kTerms][2][4];
@@ -543,7 +552,8 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
   a.Vpad = a.g.nblk * kBlock;
   a.mrhs = p->nrhs == 12;
   a.storage = p->storage;
-  a.pair = (p->nrhs == 1 && p->storage != OK_W_CONJ) ? 1 : 0;   // 12-RHS assembles chunk by chunk: the partner site may be outside
+  a.pair = (p->nrhs == 1 && p->storage != OK_W_CONJ && win_nblk < 0) ? 1 : 0;   // chunks / windows: the partner site may be outside
+  a.tfold = tfold;
   a.posonly = (a.pair || p->storage == OK_W_CONJ) ? 1 : 0;
   const double u0 = p->u0, u2 = u0 * u0, u3 = u2 * u0, u4 = u2 * u2;
   a.mass = u0 / (2.0 * p->kappa);
@@ -592,10 +602,12 @@ int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) 
     }
     return OK_SUCCESS;
   }
-  OK_ASM_LAUNCH(1, (a.posonly ? 1 : 2), a.g.nblk, Wp);   // the heavy class first
-  OK_ASM_LAUNCH(0, 1, a.g.nblk, Wp);
-  OK_ASM_LAUNCH(2, (a.posonly ? 1 : 2), a.g.nblk, Wp);
-  OK_ASM_LAUNCH(3, (a.posonly ? 2 : 4), a.g.nblk, Wp);
+  const int nb = win_nblk < 0 ? a.g.nblk : win_nblk;
+  a.blk0 = win_nblk < 0 ? 0 : win_blk0;
+  OK_ASM_LAUNCH(1, (a.posonly ? 1 : 2), nb, Wp);   // the heavy class first
+  OK_ASM_LAUNCH(0, 1, nb, Wp);
+  OK_ASM_LAUNCH(2, (a.posonly ? 1 : 2), nb, Wp);
+  OK_ASM_LAUNCH(3, (a.posonly ? 2 : 4), nb, Wp);
 #undef OK_ASM_LAUNCH
   return OK_SUCCESS;
 }
