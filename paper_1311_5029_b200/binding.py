@@ -13,6 +13,7 @@ OK_FP32, OK_FP64 = 0, 1
 OK_W_DENSE, OK_W_BLOCK, OK_W_DS, OK_W_CONJ = 0, 1, 2, 3
 OK_NTERMS = 27
 OK_W_HEADER_BYTES = 1024
+OK_SLAB, OK_SLAB_LINK_HALO = 1, 2
 
 _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libokdirac.so")
 _lib = None
@@ -30,6 +31,14 @@ class ok_params(C.Structure):
                 ("cB", C.c_double), ("cE", C.c_double), ("cEE", C.c_double), ("c1", C.c_double),
                 ("c2", C.c_double), ("c3", C.c_double), ("c4", C.c_double), ("c5", C.c_double),
                 ("storage", C.c_int32), ("reserved_", C.c_int32)]
+
+
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t)
+ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int)
+
+
+class ok_comm(C.Structure):
+    _fields_ = [("rank", C.c_int32), ("nranks", C.c_int32), ("exchange", EXCHANGE_FN), ("allgather", ALLGATHER_FN), ("user", C.c_void_p)]
 
 
 EXPORTS = {
@@ -53,6 +62,13 @@ EXPORTS = {
     "ok_mixed_work_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
     "ok_bicgstab_mixed": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int,
                                     C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
+    "ok_slab_slice_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
+    "ok_slab_vec_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
+    "ok_slab_work_bytes": (C.c_size_t, [C.POINTER(ok_params), C.c_int, C.c_int]),
+    "ok_slab_precalc_W": (C.c_int, [C.c_void_p, C.POINTER(ok_params), C.c_int, C.c_int, C.c_void_p]),
+    "ok_slab_dirac_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_slab_bicgstab": (C.c_int, [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.c_int,
+                                   C.POINTER(ok_comm), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_W_params": (C.c_int, [C.c_void_p, C.POINTER(ok_params)]),
     "ok_forget_W": (C.c_int, [C.c_void_p]),
     "ok_launch_count": (C.c_uint64, []),
@@ -204,6 +220,47 @@ def ok_bicgstab_mixed(W64, W32, src, x, tol, inner_tol, maxit, max_outer=50, rai
     if st != 0 and raise_on_fail:
         raise OkError(st, "ok_bicgstab_mixed")
     return st, it.value, outer.value, res.value
+
+
+def make_slab_params(p: ok_params, Tloc: int) -> ok_params:
+    """The parameters of a t-slab of Tloc time slices of the lattice p (ok.h: reserved_ = OK_SLAB, dims[3] = Tloc)."""
+    q = ok_params.from_buffer_copy(bytes(p))
+    q.dims[3] = int(Tloc)
+    q.reserved_ = OK_SLAB
+    return q
+
+
+def ok_slab_slice_bytes(slab):
+    return lib().ok_slab_slice_bytes(C.byref(slab))
+
+
+def ok_slab_vec_bytes(slab):
+    return lib().ok_slab_vec_bytes(C.byref(slab))
+
+
+def ok_slab_work_bytes(slab, nslab=1, nranks=1):
+    return lib().ok_slab_work_bytes(C.byref(slab), int(nslab), int(nranks))
+
+
+def ok_slab_precalc_W(links_ext, slab, T_global, t0, W):
+    _check(lib().ok_slab_precalc_W(_ptr(links_ext), C.byref(slab), int(T_global), int(t0), _ptr(W)), "ok_slab_precalc_W")
+
+
+def ok_slab_dirac_apply(W, psi_ext, out_ext):
+    _check(lib().ok_slab_dirac_apply(_ptr(W), _ptr(psi_ext), _ptr(out_ext)), "ok_slab_dirac_apply")
+
+
+def ok_slab_bicgstab(W, src_ext, x_ext, tol, maxit, comm=None, raise_on_fail=True):
+    """W, src_ext, x_ext: lists (one entry per slab this process holds, in t order).  comm: ok_comm or None.
+    Returns (status, iters, true_relative_residual)."""
+    n = len(W)
+    arr = lambda ts: (C.c_void_p * n)(*[_ptr(t) for t in ts])
+    it, res = C.c_int(0), C.c_double(0.0)
+    st = lib().ok_slab_bicgstab(n, arr(W), arr(src_ext), arr(x_ext), float(tol), int(maxit), C.byref(comm) if comm is not None else None,
+                                C.byref(it), C.byref(res))
+    if st != 0 and raise_on_fail:
+        raise OkError(st, "ok_slab_bicgstab")
+    return st, it.value, res.value
 
 
 def ok_W_params(W):
