@@ -174,6 +174,19 @@ int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, 
   return launch_direct<float, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
 }
 
+// Eq. (2.2) for the 32-site blocks [blk0, blk0 + nblk) of the whole lattice only (ok_dirac_apply_host pipelines the apply over
+// chunks of time slices behind the host -> device copy); Wp = W's payload of the whole lattice.
+int launch_apply_range(const ok_params* p, const void* Wp, const void* psi, void* out, int blk0, int nblk) {
+  if (p->nrhs != 1 || p->storage != OK_W_DENSE) return OK_EINVAL;
+  int st = upload_offsets();
+  if (st) return st;
+  const Geom g = make_geom(p);
+  const size_t wblock = (size_t)kTerms * 144 * 2 * real_bytes(p) * kBlock;   // bytes of W per 32-site block
+  const char* Wb = static_cast<const char*>(Wp) + (size_t)blk0 * wblock;
+  if (p->precision == OK_FP64) return launch_direct<double, kRowsPerWarp>(g, Wb, psi, out, nullptr, nullptr, nblk, blk0);
+  return launch_direct<float, kRowsPerWarp>(g, Wb, psi, out, nullptr, nullptr, nblk, blk0);
+}
+
 // t-slab apply (ok_slab.cu): p = the slab's own lattice (Lx, Ly, Lz, Tloc) whose W this is; psi, out, dot_a are fields of the
 // extended lattice (Lx, Ly, Lz, Tloc + 2) in the internal layout, i.e. [lower halo slice][Tloc slices][upper halo slice].
 int launch_apply_slab(const ok_params* p, const void* W, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext) {

@@ -213,6 +213,7 @@ int launch_apply(const ok_params* p, const void* Wpayload, const void* psi, void
 int launch_precalc(const ok_params* p, const void* links, void* Wpayload, void* work);
 int launch_precalc_window(const ok_params* p, const void* links, void* Wpayload, void* work, int tfold, int win_blk0, int win_nblk);
 // t-slab decomposition (ok.h): p = the slab's own lattice
+int launch_apply_range(const ok_params* p, const void* Wpayload, const void* psi, void* out, int blk0, int nblk);
 int launch_apply_slab(const ok_params* p, const void* Wpayload, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext);
 size_t bicgstab_slab_work_bytes(const ok_params* p);
 size_t bicgstab_slab_shared_bytes(int nslab, int nranks);
