@@ -205,6 +205,55 @@ __global__ void __launch_bounds__(128) field_strength_kernel(const double2* __re
   FS[(size_t)k * a.Vpad + n] = F;
 }
 
+// ------------------------------------------------------------------------- step a1b: colour matrices of the one-link hops
+// The Pauli components of W^+_i that need link-times-field products or staples (Eq. 2.8, see the header comment), computed
+// once per (site, direction) by three threads -- one per B component entering the products -- instead of inside the thread
+// that later writes the 2 x 144 entries of W^+_i(x) and W^-_i(x + i).  HB[(5 i + q)][n], cyclic (i, k, l):
+//   q = 0: S.C_0 =  i cs (U B_i(x+i) + B_i(x) U)
+//   q = 1: S.C_k =    cs (U B_l(x+i) - B_l(x) U)            q = 3: D.C_k = i c5/u0^4 (U B_k(x+i) + B_k(x) U) + i cg G_l
+//   q = 2: S.C_l =   -cs (U B_k(x+i) - B_k(x) U)            q = 4: D.C_l = i c5/u0^4 (U B_l(x+i) + B_l(x) U) - i cg G_k
+// role 0 writes q = 0; role 1 (products with B_k, staples along l) q = 2, 3; role 2 (B_l, staples along k) q = 1, 4.
+constexpr int kHopMats = 15;
+__global__ void __launch_bounds__(128) hop_blocks_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS, cm3* __restrict__ HB,
+                                                         PrecalcArgs a) {
+  const int n = blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= a.g.V) return;
+  const int i = blockIdx.y / 3, role = blockIdx.y % 3;
+  const int k = (i + 1) % 3, l = (i + 2) % 3;
+  const int m = role == 0 ? i : (role == 1 ? k : l);       // the B component of this thread's products
+  const Site x = site_of(n, a.g);
+  const Site xp = shift(x, i, 1, a.g);
+  const cm3 U = ldU(links, x, i, a);
+  const cm3 P = mul(U, ldF(FS, m, xp, a)), Q = mul(ldF(FS, m, x, a), U);
+  cm3* out = HB + (size_t)(5 * i) * a.Vpad + n;
+  if (role == 0) {
+    cm3 R = zero3();
+    axpy(R, 0.0, a.cs, P);
+    axpy(R, 0.0, a.cs, Q);
+    out[0] = R;
+    return;
+  }
+  cm3 Sd = zero3(), Dd = zero3();
+  const double sg = role == 1 ? -1.0 : 1.0;                 // role 1: S.C_l = -cs Dif_k ; role 2: S.C_k = +cs Dif_l
+  axpy(Sd, sg * a.cs, 0.0, P);
+  axpy(Sd, -sg * a.cs, 0.0, Q);
+  axpy(Dd, 0.0, a.c5u, P);
+  axpy(Dd, 0.0, a.c5u, Q);
+  if (a.cg != 0.0) {
+    const int sd = role == 1 ? l : k;                       // staple direction; role 1: + i cg G_l, role 2: - i cg G_k
+    const double gs = role == 1 ? 1.0 : -1.0;
+    cm3 G = mul(ldU(links, x, sd, a), ldU(links, shift(x, sd, 1, a.g), i, a));   // up: U_m(x) U_i(x+m) U_m(x+i)^dag
+    G = mul_nd(G, ldU(links, xp, sd, a));
+    axpy(Dd, 0.0, gs * a.cg, G);
+    const Site xm = shift(x, sd, -1, a.g);                                        // down: U_m(x-m)^dag U_i(x-m) U_m(x-m+i)
+    G = mul_dn(ldU(links, xm, sd, a), ldU(links, xm, i, a));
+    G = mul(G, ldU(links, shift(xm, i, 1, a.g), sd, a));
+    axpy(Dd, 0.0, -gs * a.cg, G);
+  }
+  out[(size_t)(role == 1 ? 2 : 1) * a.Vpad] = Sd;
+  out[(size_t)(role == 1 ? 3 : 4) * a.Vpad] = Dd;
+}
+
 // ------------------------------------------------------------------------- step a2: W assembly
 struct P4 {
   cm3 c[4];
@@ -236,41 +285,14 @@ __device__ __forceinline__ void positive_blocks(const Site& x, const double2* __
   } else if constexpr (fam == 2) {
     constexpr int k = (i + 1) % 3, l = (i + 2) % 3;
     const cm3 U = ldU(links, x, i, a);
-    const Site xp = shift(x, i, 1, a.g);
+    const cm3* HB = FS + (size_t)(6 + 5 * i) * a.Vpad;      // hop_blocks_kernel (the scratch follows the six clover fields)
     axpy(B.c[i + 1], a.a1, 0.0, U);
     axpy(A.c[0], a.d1, 0.0, U);
-    {   // m = i : only the sum enters (S, C0)
-      cm3 P = mul(U, ldF(FS, i, xp, a));
-      axpy(P, 1.0, 0.0, mul(ldF(FS, i, x, a), U));
-      axpy(B.c[0], 0.0, a.cs, P);
-    }
-    {   // m = k : Dif_k -> S.C_l (minus), Sum_k -> D.C_k
-      const cm3 P = mul(U, ldF(FS, k, xp, a)), Q = mul(ldF(FS, k, x, a), U);
-      axpy(B.c[l + 1], -a.cs, 0.0, P); axpy(B.c[l + 1], a.cs, 0.0, Q);
-      axpy(A.c[k + 1], 0.0, a.c5u, P); axpy(A.c[k + 1], 0.0, a.c5u, Q);
-    }
-    {   // m = l : Dif_l -> S.C_k (plus), Sum_l -> D.C_l
-      const cm3 P = mul(U, ldF(FS, l, xp, a)), Q = mul(ldF(FS, l, x, a), U);
-      axpy(B.c[k + 1], a.cs, 0.0, P); axpy(B.c[k + 1], -a.cs, 0.0, Q);
-      axpy(A.c[l + 1], 0.0, a.c5u, P); axpy(A.c[l + 1], 0.0, a.c5u, Q);
-    }
-    if (a.cg != 0.0) {
-#pragma unroll
-      for (int q = 0; q < 2; ++q) {
-        const int m = q ? l : k;           // staple direction
-        const int tgt = q ? k : l;         // sigma index receiving G_m:  +i cg G_l -> C_k ; -i cg G_k -> C_l
-        const double sgn = q ? 1.0 : -1.0;
-        // up: U_m(x) U_i(x+m) U_m(x+i)^dag
-        cm3 G = mul(ldU(links, x, m, a), ldU(links, shift(x, m, 1, a.g), i, a));
-        G = mul_nd(G, ldU(links, xp, m, a));
-        axpy(A.c[tgt + 1], 0.0, sgn * a.cg, G);
-        // down: U_m(x-m)^dag U_i(x-m) U_m(x-m+i)
-        const Site xm = shift(x, m, -1, a.g);
-        G = mul_dn(ldU(links, xm, m, a), ldU(links, xm, i, a));
-        G = mul(G, ldU(links, shift(xm, i, 1, a.g), m, a));
-        axpy(A.c[tgt + 1], 0.0, -sgn * a.cg, G);
-      }
-    }
+    B.c[0] = ldF(HB, 0, x, a);
+    B.c[k + 1] = ldF(HB, 1, x, a);
+    B.c[l + 1] = ldF(HB, 2, x, a);
+    A.c[k + 1] = ldF(HB, 3, x, a);
+    A.c[l + 1] = ldF(HB, 4, x, a);
   } else if constexpr (fam == 3) {
     const cm3 P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), i, a));
     axpy(A.c[0], a.dii, 0.0, P);
@@ -408,7 +430,10 @@ __device__ __noinline__ void assemble_term(const double2* __restrict__ links, co
 // CLS splits the 27 terms into four launches so that every launch carries only the registers its families need:
 //   0: W^0, W^+-_4 (terms 0, 7, 8)   1: W^+-_i (1..6, the heavy one)   2: W^{++/--}_ii (9..14)   3: the 12 pair terms (15..26)
 template <typename real, int CLS>
-__global__ void __launch_bounds__(32 * 3, 4) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+#ifndef OK_CLS1_MINB
+#define OK_CLS1_MINB 4
+#endif
+__global__ void __launch_bounds__(32 * 3, CLS == 1 ? OK_CLS1_MINB : 4) assemble_W_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
                                                                            typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
   using unit_t = typename WUnit<real>::type;
   constexpr int NC = WUnit<real>::NC;
@@ -527,7 +552,7 @@ static int mrhs_bounce_blocks(const Geom& g) { return g.nblk < kBounceBlocksMax 
 
 size_t precalc_work_bytes(const ok_params* p) {
   Geom g = make_geom(p);
-  const size_t fs = (size_t)6 * g.nblk * kBlock * sizeof(cm3);
+  const size_t fs = (size_t)(6 + kHopMats) * g.nblk * kBlock * sizeof(cm3);
   return p->nrhs == 12 ? fs + 256 + (size_t)mrhs_bounce_blocks(g) * kBounceBlockBytes : fs;
 }
 
@@ -572,6 +597,8 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
   cudaStream_t st = ctx().stream;
   field_strength_kernel<<<dim3((a.g.V + 127) / 128, 6), 128, 0, st>>>(static_cast<const double2*>(links), FS, a);
   OK_LAUNCHED("field_strength_kernel");
+  hop_blocks_kernel<<<dim3((a.g.V + 127) / 128, 9), 128, 0, st>>>(static_cast<const double2*>(links), FS, FS + (size_t)6 * a.Vpad, a);
+  OK_LAUNCHED("hop_blocks_kernel");
   const dim3 block(32, 3);
   const double2* lk = static_cast<const double2*>(links);
 #define OK_ASM_LAUNCH(CLS, NY, NB, OUT)                                                                                     \
@@ -587,7 +614,7 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
       OK_CUDA(cudaFuncSetAttribute(mrhs_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSmem));
       attr_set = true;
     }
-    const size_t fs = ((size_t)6 * a.g.nblk * kBlock * sizeof(cm3) + 255) / 256 * 256;
+    const size_t fs = ((size_t)(6 + kHopMats) * a.g.nblk * kBlock * sizeof(cm3) + 255) / 256 * 256;
     void* bounce = static_cast<char*>(work) + fs;
     const int cap = mrhs_bounce_blocks(a.g);
     for (int b0 = 0; b0 < a.g.nblk; b0 += cap) {
