@@ -162,6 +162,7 @@ static int launch_direct(const Geom& g, const void* W, const void* psi, void* ou
 }
 
 constexpr int kRowsPerWarp = 3;   // 4 warps per CTA, 40 registers: the measured optimum (profiles/r01_apply.md)
+constexpr int kSmallLatticeBlocks = 4 * 148;   // below four CTAs per SM: 12 warps per CTA
 
 int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, double* partials,
                  const void* dot_a, const void* /*unused*/) {
@@ -170,6 +171,13 @@ int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, 
   int st = upload_offsets();
   if (st) return st;
   Geom g = make_geom(p);
+  // Small lattices (BASELINE configs[0], [1]): one CTA per 32-site block leaves most SMs with one or two CTAs, too few W
+  // loads in flight to fill the HBM pipe.  There a CTA uses 12 warps of one output row each instead of 4 warps of three
+  // (same arithmetic and summation order per row, hence the same bits).
+  if (g.nblk < kSmallLatticeBlocks) {
+    if (p->precision == OK_FP64) return launch_direct<double, 1>(g, W, psi, out, partials, dot_a);
+    return launch_direct<float, 1>(g, W, psi, out, partials, dot_a);
+  }
   if (p->precision == OK_FP64) return launch_direct<double, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
   return launch_direct<float, kRowsPerWarp>(g, W, psi, out, partials, dot_a);
 }
