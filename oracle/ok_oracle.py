@@ -22,9 +22,13 @@ Pins (tests/test_oracle_*.py, all -m "not gpu"): direct == W form (P1); free-fie
 form and plane-wave eigen-relation (P2); gauge covariance (P3); gamma5-hermiticity and
 Eqs. (2.3)/(2.10) (P4); hand-coded Wilson / Wilson-clover special cases (P5); zero-block
 structure (P6); dense LU vs BiCGStab (P7); staple content of the c5 hop term (Eq. 2.8's 1/4);
-mixed-precision defect correction vs dense LU (P8); CG on the normal equations and Gamma_5 M Gamma_5 = M^dag (P9).
+mixed-precision defect correction vs dense LU (P8); CG on the normal equations and Gamma_5 M Gamma_5 = M^dag (P9);
+cubic-group covariance: 90-degree rotations about the three spatial axes with the matching spinor rotation, and spatial
+parity with gamma_4 (P10: pins the assignment of sigma_i to direction i, the orientation of every B_i and E_i component
+against the links, and the diagonal / off-diagonal placement of the axial and vector terms).
 Parity unpinned (conventions with no printed value to check, shared as input spec):
-trace subtraction in F (none), the Pauli basis, the coefficient values, sign E_i = F_4i.
+trace subtraction in F (none), the choice of Pauli basis as a whole (any basis related by a spin rotation gives an
+equivalent operator), the coefficient values, the overall sign convention E_i = F_4i (a sign of c_E).
 
 Conventions (DESIGN.md R-GAMMA): sigma_k standard Pauli; gamma_i = [[0,s_i],[s_i,0]],
 gamma_4 = diag(1,1,-1,-1); a 12x12 W is W[3*alpha+a, 3*beta+b]; the paper's 2x2 block

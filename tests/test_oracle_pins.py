@@ -439,3 +439,107 @@ def test_P9_cgnr_vs_dense_LU_and_gamma5():
     assert st0 == 0 and it0 == 0 and np.all(x0 == 0)
     x1, it1, res1, st1 = oo.cgnr(ap, b, 1e-10, 3)
     assert st1 == -4 and it1 == 3 and res1 > 1e-10
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P10: cubic-group covariance.  The OK action is built from lattice-covariant objects (an improved
+# Wilson-type action; Eqs. 2.6-2.12 treat the three spatial directions alike), so a rotation of the gauge field by 90
+# degrees about a spatial axis, with the spinor rotated by the matching S, must commute with M; likewise spatial parity
+# with psi -> gamma_4 psi.  This pins what P1-P9 cannot: the assignment of sigma_i to direction i, the orientation of
+# B_i = eps_ijk F_jk / 2 against the links it multiplies, and the placement of the E (vector) and B (axial) terms in the
+# off-diagonal / diagonal spin blocks -- a plausible slip there (a swapped pair of B components, a wrong sign on one of
+# them, E in a diagonal block) leaves every earlier pin green if made consistently in both evaluations of the operator.
+def _coords(dims):
+    return I.site_coords(dims)
+
+
+def _index(dims, c):
+    Lx, Ly, Lz, T = dims
+    return c[:, 0] + Lx * (c[:, 1] + Ly * (c[:, 2] + Lz * c[:, 3]))
+
+
+def _rotated_links(dims, U, a, b):
+    """Image of the gauge field under the rotation by +90 degrees in the (a, b) plane: direction a -> b, b -> -a
+    (L_a = L_b).  The link x -> x + a becomes the link x' -> x' + b; the link x -> x + b becomes x' -> x' - a, i.e.
+    the reversed link U'_a(x' - a); all other links keep their direction."""
+    c = _coords(dims)
+    cp = c.copy()
+    cp[:, a] = (-c[:, b]) % dims[a]
+    cp[:, b] = c[:, a]
+    img = _index(dims, cp)                      # img[n] = index of R x_n
+    Up = np.empty_like(U)
+    Up[img, b] = U[:, a]
+    cm = cp.copy()
+    cm[:, a] = (cm[:, a] - 1) % dims[a]
+    Up[_index(dims, cm), a] = oo.dag(U[:, b])
+    for mu in range(4):
+        if mu not in (a, b):
+            Up[img, mu] = U[:, mu]
+    return Up, img
+
+
+@pytest.mark.parametrize("plane", [(0, 1), (1, 2), (2, 0)])
+def test_P10_rotation_covariance(plane):
+    a, b = plane
+    dims = [3, 3, 3, 2]
+    dims[a] = dims[b] = 4
+    dims = tuple(dims)
+    U = I.near_identity_links(dims, 0.4, 21)
+    pd = I.make_params(dims, 0.11, 0.93)
+    Up, img = _rotated_links(dims, U, a, b)
+    # the spinor representation is DEFINED by S gamma_mu S^-1 = gamma_(R mu): R a = b, R b = -a
+    S = (np.eye(4) - GAMMA[a] @ GAMMA[b]) / np.sqrt(2.0)
+    Si = np.linalg.inv(S)
+    assert np.allclose(S @ GAMMA[a] @ Si, GAMMA[b]) and np.allclose(S @ GAMMA[b] @ Si, -GAMMA[a])
+    for mu in range(4):
+        if mu not in (a, b):
+            assert np.allclose(S @ GAMMA[mu] @ Si, GAMMA[mu])
+    psi = I.gaussian_spinor(dims, 22)
+    V = psi.shape[0]
+
+    def rot(f):                                 # (T f)(R x) = S f(x)
+        g = np.empty_like(f)
+        g[img] = np.einsum("st,ntc->nsc", S, f.reshape(V, 4, 3)).reshape(V, 12)
+        return g
+
+    lhs = Oracle(Up, pd).apply_W(rot(psi))
+    rhs = rot(Oracle(U, pd).apply_W(psi))
+    assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(rhs)
+    # the direct (link-product) evaluation obeys it too
+    lhs_d = Oracle(Up, pd).apply_direct(rot(psi))
+    assert np.linalg.norm(lhs_d - rhs) <= 1e-12 * np.linalg.norm(rhs)
+    # and the check has teeth: the unrotated spinor map fails
+    g = np.empty_like(psi)
+    g[img] = psi
+    assert np.linalg.norm(Oracle(Up, pd).apply_W(g) - rhs) > 1e-2 * np.linalg.norm(rhs)
+
+
+def test_P10_spatial_parity_covariance():
+    dims = (4, 3, 3, 2)
+    U = I.near_identity_links(dims, 0.4, 23)
+    pd = I.make_params(dims, 0.11, 0.93)
+    c = _coords(dims)
+    cp = c.copy()
+    for i in range(3):
+        cp[:, i] = (-c[:, i]) % dims[i]
+    img = _index(dims, cp)
+    Up = np.empty_like(U)
+    for i in range(3):                          # the link x -> x + i becomes x' -> x' - i: the reversed link U'_i(x' - i)
+        cm = cp.copy()
+        cm[:, i] = (cm[:, i] - 1) % dims[i]
+        Up[_index(dims, cm), i] = oo.dag(U[:, i])
+    Up[img, 3] = U[:, 3]
+    psi = I.gaussian_spinor(dims, 24)
+    V = psi.shape[0]
+
+    def par(f):                                 # (P f)(-x, t) = gamma_4 f(x, t); gamma_4 gamma_i gamma_4 = -gamma_i
+        g = np.empty_like(f)
+        g[img] = np.einsum("st,ntc->nsc", GAMMA[3], f.reshape(V, 4, 3)).reshape(V, 12)
+        return g
+
+    lhs = Oracle(Up, pd).apply_W(par(psi))
+    rhs = par(Oracle(U, pd).apply_W(psi))
+    assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(rhs)
+    g = np.empty_like(psi)
+    g[img] = psi                                # without gamma_4 the E terms and the hops come out with the wrong sign
+    assert np.linalg.norm(Oracle(Up, pd).apply_W(g) - rhs) > 1e-2 * np.linalg.norm(rhs)
