@@ -492,6 +492,96 @@ def sub_record(wl, dev, stream, index, peaks, steps=2):
     return out
 
 
+def slab_record(wl, nslab, dev, stream, index, peaks, steps=2):
+    """The t-slab decomposition (ok_slab_* in include/ok.h) on ONE GPU: the lattice of workload wl cut into nslab
+    slabs held by this process (virtual ranks: separate W, fields and halos per slab, halo refresh by device copies), so
+    that the cost of the decomposition itself -- the extra launches, the halo copies, the per-slab reduction stage -- is
+    measured against the unsharded numbers.  No inter-GPU transfer is involved or claimed."""
+    import torch
+    from paper_1311_5029_b200 import binding as B
+    from paper_1311_5029_b200 import slab as S
+    dims, sbytes, eps, lseed, sseed, kappa, tol = WORKLOADS[wl]
+    U = make_links(dims, eps, lseed)
+    plaq = I.mean_plaquette(dims, U)
+    pd = I.make_params(dims, kappa, I.tadpole_u0(plaq))
+    p = B.make_params(pd, B.OK_FP32 if sbytes == 4 else B.OK_FP64)
+    ranges = S.slab_ranges(dims[3], nslab)
+    slab = B.make_slab_params(p, ranges[0][1])
+    plocal = B.make_params(dict(pd, dims=tuple(dims[:3]) + (ranges[0][1],)), p.precision)
+    cdt = torch.complex64 if sbytes == 4 else torch.complex128
+    work = B.alloc_bytes(B.ok_slab_work_bytes(slab, nslab, 1), dev)
+    B.ok_set_stream(stream)
+    B.ok_set_workspace(work, work.numel())
+    psi = I.gaussian_spinor(dims, sseed)
+    Ws, links, src, out, xs = [], [], [], [], []
+    for t0, Tl in ranges:
+        Ws.append(B.alloc_W(slab, dev))
+        links.append(torch.from_numpy(S.link_window(U, dims, t0, Tl)).to(dev))
+        v = torch.zeros(B.ok_slab_vec_bytes(slab), dtype=torch.uint8, device=dev)
+        with torch.cuda.stream(stream):
+            B.ok_pack_spinor(plocal, torch.from_numpy(S.spinor_slab(psi, dims, t0, Tl)).to(cdt).to(dev), S.interior(slab, v))
+        src.append(v)
+        out.append(torch.zeros_like(v))
+        xs.append(torch.zeros_like(v))
+    stream.synchronize()
+    V = int(np.prod(dims))
+    rec = {"pre_ms": [], "apply_ms": [], "solve_s": [], "iters": [], "resid": []}
+
+    def step(record):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        with torch.cuda.stream(stream):
+            ev[0].record(stream)
+            for (t0, Tl), W, lk in zip(ranges, Ws, links):
+                B.ok_slab_precalc_W(lk, slab, dims[3], t0, W)
+            ev[1].record(stream)
+            for _ in range(NAPPLY):
+                for i in range(nslab):       # halo refresh (what ok_slab_bicgstab does internally), then the slab applies
+                    lo, first, last, hi = S.halo_views(slab, src[i])
+                    lo.copy_(S.halo_views(slab, src[(i - 1) % nslab])[2], non_blocking=True)
+                    hi.copy_(S.halo_views(slab, src[(i + 1) % nslab])[1], non_blocking=True)
+                for i in range(nslab):
+                    B.ok_slab_dirac_apply(Ws[i], src[i], out[i])
+            ev[2].record(stream)
+            st, it, res = B.ok_slab_bicgstab(Ws, src, xs, tol, 5000, raise_on_fail=False)
+            ev[3].record(stream)
+        if st != 0:
+            raise RuntimeError(f"ok_slab_bicgstab failed: {B.ok_strerror(st)}")
+        if record:
+            stream.synchronize()
+            rec["pre_ms"].append(ev[0].elapsed_time(ev[1]))
+            rec["apply_ms"].append(ev[1].elapsed_time(ev[2]) / NAPPLY)
+            rec["solve_s"].append(ev[2].elapsed_time(ev[3]) / 1e3)
+            rec["iters"].append(it)
+            rec["resid"].append(res)
+
+    for _ in range(3):
+        step(False)
+    stream.synchronize()
+    l0 = B.ok_launch_count()
+    with ClockSampler(index) as cs:
+        for _ in range(steps):
+            step(True)
+        stream.synchronize()
+    a_ms = float(np.mean(rec["apply_ms"]))
+    alg = V * alg_bytes_per_site(sbytes, 1, 0)
+    ach = alg / (a_ms * 1e-3) / 1e9
+    outrec = {"workload": wl, "slabs": nslab, "Tloc": ranges[0][1], "what": "t-slab decomposition on one GPU (virtual ranks; halo refresh by device copies)",
+              "apply_ms": a_ms, "value": ach, "unit": "GB/s", "halo_bytes_per_apply_per_slab": 2 * B.ok_slab_slice_bytes(slab),
+              "bicgstab_solve_s": float(np.mean(rec["solve_s"])), "bicgstab_iters": int(np.max(rec["iters"])),
+              "bicgstab_true_resid": float(np.max(rec["resid"])), "bicgstab_tol": tol, "oracle_bicgstab": oracle_golden(wl),
+              "precalc_ms": float(np.mean(rec["pre_ms"])),
+              "roofline": {"bound": "hbm", "kernel": "okd::apply_direct_kernel<float,...> over %d slabs" % nslab, "achieved": ach, "peak": peaks["hbm_gbs"],
+                           "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "peak_source": peaks["_source"], "algorithmic_bytes_per_launch": alg // nslab,
+                           "traffic": None},
+              "gpu_launches": int(B.ok_launch_count() - l0), "clocks": cs.summary(), "steps": steps, "warmup": 3}
+    B.ok_set_workspace(None)
+    for W in Ws:
+        B.ok_forget_W(W)
+    del Ws, links, src, out, xs, work
+    torch.cuda.empty_cache()
+    return outrec
+
+
 def run_ours(args, wl):
     import torch
     from paper_1311_5029_b200 import binding as B
@@ -614,6 +704,10 @@ def run_ours(args, wl):
                     line["configs"][name] = sub_record(sub, dev, stream, local, peaks)
                 except Exception as e:      # a sub-record must not take the contract line down with it
                     line["configs"][name] = {"workload": sub, "error": repr(e)[:300]}
+            try:
+                line["configs"]["configs[2] as 4 t-slabs (one GPU)"] = slab_record("20x20x20x64-fp32", 4, dev, stream, local, peaks)
+            except Exception as e:
+                line["configs"]["configs[2] as 4 t-slabs (one GPU)"] = {"error": repr(e)[:300]}
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
@@ -674,9 +768,16 @@ def main():
     ap.add_argument("--workload", default="20x20x20x64-fp32", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the 1000-apply series and the sub-records of the other BASELINE configs")
+    ap.add_argument("--slabs", type=int, default=0, help="time the t-slab decomposition of the workload with this many slabs on one GPU")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: apply throughput over lattice sizes (not the driver's contract line)")
     args = ap.parse_args()
-    if args.sweep:
+    if args.slabs:
+        import torch
+        from paper_1311_5029_b200 import binding as B
+        torch.cuda.set_device(0)
+        B.lib()
+        print(json.dumps(slab_record(args.workload, args.slabs, "cuda:0", torch.cuda.Stream(device="cuda:0"), 0, measured_peaks(), steps=args.steps)))
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args, args.workload)

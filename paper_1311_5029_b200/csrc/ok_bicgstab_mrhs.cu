@@ -423,16 +423,19 @@ int run_bicgstab_mrhs(const ok_params* p, const void* W, const void* src, void* 
     }
   }
   if (status == OK_SUCCESS && nactive > 0) status = OK_EMAXIT;
-  // report the true residual of every column at exit
-  for (int j = 0; j < kN; ++j) restart[j] = 0;
-  OK_TRY(true_residual());
+  // Report the true residual of every column at exit.  After a clean finish every column was frozen right after its own
+  // true-residual check and has not changed since, so those values stand; otherwise recompute them all.
+  if (status != OK_SUCCESS) {
+    for (int j = 0; j < kN; ++j) restart[j] = 0;
+    OK_TRY(true_residual());
+    for (int j = 0; j < kN; ++j) true_rr[j] = h->res[j];
+  }
   double worst = 0.0;
   int itmax = 0;
   for (int j = 0; j < kN; ++j) {
-    if (bnorm2[j] > 0.0) worst = fmax(worst, sqrt(h->res[j] / bnorm2[j]));
+    if (bnorm2[j] > 0.0) worst = fmax(worst, sqrt(true_rr[j] / bnorm2[j]));
     if (it_conv[j] > itmax) itmax = it_conv[j];
   }
-  (void)true_rr;
   *iters = itmax;
   *resid = worst;
 #undef OK_TRY

@@ -216,3 +216,60 @@ def test_fullsize_config5_haar_32x32x32x64():
     r = psi[idx] - o.apply_W(xs, idx=idx, W=want_W)
     est = np.sqrt(o.V / len(idx)) * np.linalg.norm(r) / np.linalg.norm(psi)
     assert est <= sampled_resid_bound(tol, o, xs, psi, idx, want_W), est
+
+
+def test_fullsize_t_slabs_equal_the_whole_lattice(big):
+    """The t-slab decomposition at BASELINE configs[2]'s size, 4 slabs of 16 time slices on one GPU: every slab's W
+    (sampled blocks) and the slab apply equal the unsharded CUDA result bit for bit; ok_slab_bicgstab reproduces the oracle's
+    iteration count (+-2) and solution (golden cfg2)."""
+    from paper_1311_5029_b200 import slab as S
+    U, pd, o = big[5]
+    p = B.make_params(pd, B.OK_FP32)
+    W = G.precalc(p, U)
+    psi = I.gaussian_spinor(DIMS, 6)
+    whole = G.apply(p, W, psi)
+    B.ok_forget_W(W)
+    del W
+    torch.cuda.empty_cache()
+    nslab = 4
+    ranges = S.slab_ranges(DIMS[3], nslab)
+    slab = B.make_slab_params(p, ranges[0][1])
+    plocal = B.make_params(dict(pd, dims=DIMS[:3] + (ranges[0][1],)), B.OK_FP32)
+    work = B.alloc_bytes(B.ok_slab_work_bytes(slab, nslab, 1), G.DEV)
+    B.ok_set_stream(None)
+    B.ok_set_workspace(work, work.numel())
+    Ws, src = [], []
+    for t0, Tl in ranges:
+        Wt = B.alloc_W(slab, G.DEV)
+        B.ok_slab_precalc_W(G.to_dev(S.link_window(U, DIMS, t0, Tl), torch.complex128), slab, DIMS[3], t0, Wt)
+        Ws.append(Wt)
+        v = torch.zeros(B.ok_slab_vec_bytes(slab), dtype=torch.uint8, device=G.DEV)
+        B.ok_pack_spinor(plocal, G.to_dev(S.spinor_slab(psi, DIMS, t0, Tl), torch.complex64), S.interior(slab, v))
+        src.append(v)
+    for i in range(nslab):
+        lo, first, last, hi = S.halo_views(slab, src[i])
+        lo.copy_(S.halo_views(slab, src[(i - 1) % nslab])[2])
+        hi.copy_(S.halo_views(slab, src[(i + 1) % nslab])[1])
+    sites = DIMS[0] * DIMS[1] * DIMS[2]
+    got = []
+    for Wt, v in zip(Ws, src):
+        out = torch.zeros_like(v)
+        B.ok_slab_dirac_apply(Wt, v, out)
+        canon = torch.empty((ranges[0][1] * sites, 12), dtype=torch.complex64, device=G.DEV)
+        B.ok_unpack_spinor(plocal, S.interior(slab, out), canon)
+        got.append(canon)
+    torch.cuda.synchronize()
+    got = torch.cat(got).cpu().numpy().astype(np.complex128)
+    assert np.array_equal(got, whole)
+    xs = [torch.zeros_like(v) for v in src]
+    tol = 1e-6
+    st, it, res = B.ok_slab_bicgstab(Ws, src, xs, tol, 2000, raise_on_fail=False)
+    assert st == 0 and res <= tol
+    xg = []
+    for v in xs:
+        canon = torch.empty((ranges[0][1] * sites, 12), dtype=torch.complex64, device=G.DEV)
+        B.ok_unpack_spinor(plocal, S.interior(slab, v), canon)
+        xg.append(canon)
+    torch.cuda.synchronize()
+    check_against_golden("cfg2", DIMS, it, tol, torch.cat(xg).cpu().numpy().astype(np.complex128))
+    B.ok_set_workspace(None)
