@@ -174,7 +174,8 @@ int ok_bicgstab_mixed(const void* W64, const void* W32, const void* src, void* x
  * device, packs, applies, unpacks and copies back, synchronising the stream.  W stays
  * device-resident across calls (the paper keeps the precalculation matrices on the GPU and
  * copies the fermion field every call).  Needs the workspace.
- * nrhs = 1, OK_W_DENSE, T >= 8 and Lx*Ly*Lz a multiple of 32: the call is pipelined over chunks of time slices on two
+ * nrhs = 1, OK_W_DENSE, T >= 8, Lx*Ly*Lz a multiple of 32 and a field of at least 8 MiB (or OK_HOST_PIPELINE set in the
+ * environment, for tests): the call is pipelined over chunks of time slices on two
  * library-owned copy streams beside the caller's stream (the stencil reaches one slice in t), so the copies
  * hide behind the W stream; pinned host buffers are needed for that overlap (pageable ones still work, serially). */
 int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host);

@@ -333,7 +333,9 @@ int ok_dirac_apply_host(const void* W, const void* psi_host, void* out_host) {
   if (!ctx().work || ctx().work_bytes < 4 * vb) return OK_EWORKSPACE;
   char* w = static_cast<char*>(ctx().work);
   char *canon_in = w, *packed_in = w + vb, *packed_out = w + 2 * vb, *canon_out = w + 3 * vb;
-  if (p.nrhs == 1 && p.storage == OK_W_DENSE && p.dims[3] >= 8 && ((long long)p.dims[0] * p.dims[1] * p.dims[2]) % kBlock == 0)
+  // (small fields: the two dozen extra launches and event waits of the pipeline cost more than the copies it hides)
+  if (p.nrhs == 1 && p.storage == OK_W_DENSE && p.dims[3] >= 8 && ((long long)p.dims[0] * p.dims[1] * p.dims[2]) % kBlock == 0 &&
+      (cb >= ((size_t)8 << 20) || getenv("OK_HOST_PIPELINE")))
     return apply_host_pipelined(p, W, static_cast<const char*>(psi_host), static_cast<char*>(out_host), canon_in, packed_in, packed_out,
                                 canon_out);
   OK_CUDA(cudaMemcpyAsync(canon_in, psi_host, cb, cudaMemcpyHostToDevice, ctx().stream));

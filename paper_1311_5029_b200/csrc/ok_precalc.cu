@@ -493,6 +493,107 @@ __global__ void __launch_bounds__(32 * 3, CLS == 1 ? OK_CLS1_MINB : 4) assemble_
 #undef OK_ASM
 }
 
+// ------------------------------------------------------------------------- step a2, the 18 two-link terms (dense layout)
+// W^{++}_ii, W^{++}_ij, W^{+-}_ij and their conjugates (Eqs. 2.9-2.12; terms 9..26, two thirds of W's bytes) are Kronecker
+// products  W = K (x) P  of a 4x4 spin matrix K and ONE 3x3 colour matrix:
+//   P_ii = U_i(x) U_i(x+i)                                    D = (c4/u0) 1 (x) P ,       S = ((c1+2c2)/2u0) sigma_i (x) P      (2.9)
+//   P_ij = U_i(x) U_j(x+i) + U_j(x) U_i(x+j)                  D = 0 ,                     S = (c2/2u0) (sigma_i + sigma_j) (x) P  (2.11)
+//   P_i-j = U_i(x) U_j(x-j+i)^dag + U_j(x-j)^dag U_i(x-j)     D = 0 ,                     S = (c2/2u0) (sigma_i - sigma_j) (x) P  (2.12)
+// W = [[D, S], [S, D]]; the opposite-direction matrix is [[D^dag, -S^dag], [-S^dag, D^dag]] of the blocks at x + offset (2.3, 2.10):
+// same K with the sign of S flipped, P -> P^dag.  One thread per (site, term) writes its own site only (coalesced, sector
+// aligned), one rolled loop over the spin row keeps the code small: the templated assembly path spends most of its time waiting
+// for instructions (profiles/r02_precalc.md).  fp64 throughout, rounded once.
+template <typename real>
+__global__ void __launch_bounds__(32 * 3) kron_terms_kernel(const double2* __restrict__ links, typename WUnit<real>::type* __restrict__ W,
+                                                            PrecalcArgs a) {
+  using unit_t = typename WUnit<real>::type;
+  constexpr int NC = WUnit<real>::NC;
+  const int lane = threadIdx.x;
+  const int term = 9 + blockIdx.y * 3 + threadIdx.y;
+  const int blk = blockIdx.x;
+  const int n = (blk + a.blk0) * kBlock + lane;
+  unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
+  if (n >= a.g.V) {   // padded site: zeros
+    unit_t z = {};
+    for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
+    return;
+  }
+  // term -> family, directions, sign (term order of ok.h)
+  int fam, i, j = 0;
+  bool neg;
+  if (term < 15) {
+    fam = 3; i = (term - 9) >> 1; neg = ((term - 9) & 1) != 0;
+  } else {
+    const int q = (term - 15) >> 2, w = (term - 15) & 3;
+    i = q == 2 ? 1 : 0;
+    j = q == 0 ? 1 : 2;
+    fam = w < 2 ? 4 : 5;
+    neg = (w & 1) != 0;
+  }
+  Site x = site_of(n, a.g);
+  if (neg)   // the positive blocks live at x + offset(term)
+    for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
+  cm3 P;
+  if (fam == 3) {
+    P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), i, a));
+  } else if (fam == 4) {
+    P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), j, a));
+    axpy(P, 1.0, 0.0, mul(ldU(links, x, j, a), ldU(links, shift(x, j, 1, a.g), i, a)));
+  } else {
+    const Site xmj = shift(x, j, -1, a.g);
+    P = mul_nd(ldU(links, x, i, a), ldU(links, shift(xmj, i, 1, a.g), j, a));
+    axpy(P, 1.0, 0.0, mul_dn(ldU(links, xmj, j, a), ldU(links, xmj, i, a)));
+  }
+  if (neg) P = adj(P);
+  // spin structure: D = kD 1 ; S = s1 sigma_1 + s2 sigma_2 + s3 sigma_3 (real coefficients)
+  const double kD = fam == 3 ? a.dii : 0.0;
+  double sk[3] = {0.0, 0.0, 0.0};
+  const double sgn = neg ? -1.0 : 1.0;
+  if (fam == 3) {
+    sk[i] = sgn * a.sii;
+  } else {
+    sk[i] = sgn * a.sij;
+    sk[j] = sgn * (fam == 4 ? a.sij : -a.sij);
+  }
+  // S2[al][be]: [[s3, s1 - i s2], [s1 + i s2, -s3]]
+#pragma unroll 1
+  for (int alpha = 0; alpha < 4; ++alpha) {
+    const int bi = alpha >> 1, al = alpha & 1;
+    // this spin row's four coefficients K[alpha][beta], beta = 2 bj + be
+    double2 K[4];
+#pragma unroll
+    for (int beta = 0; beta < 4; ++beta) {
+      const int bj = beta >> 1, be = beta & 1;
+      double2 v;
+      if (bi == bj) {
+        v = make_double2(al == be ? kD : 0.0, 0.0);
+      } else if (al == be) {
+        v = make_double2(al == 0 ? sk[2] : -sk[2], 0.0);
+      } else {
+        v = make_double2(sk[0], al == 0 ? -sk[1] : sk[1]);
+      }
+      K[beta] = v;
+    }
+#pragma unroll
+    for (int ca = 0; ca < 3; ++ca) {
+      double2 row[12];
+#pragma unroll
+      for (int beta = 0; beta < 4; ++beta)
+#pragma unroll
+        for (int cb = 0; cb < 3; ++cb) row[3 * beta + cb] = cmul(K[beta], P.e[3 * ca + cb]);
+      unit_t* dst = Wt + (size_t)(3 * alpha + ca) * NC * kBlock;
+      if constexpr (sizeof(real) == 4) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c)
+          dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
+      } else {
+#pragma unroll
+        for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------- 12-RHS tile writer
 // The 12-RHS W tile of a site (ok_internal.cuh) interleaves the four terms of a K stage inside 16-byte core-matrix rows,
 // so a (site, term) thread would write 8-byte pieces 31 KB apart.  Instead the dense fp32 W of a chunk of blocks is
@@ -607,6 +708,12 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
     else assemble_W_kernel<float, CLS><<<dim3(NB, NY), block, 0, st>>>(lk, FS, static_cast<float4*>(OUT), a);               \
     OK_LAUNCHED("assemble_W_kernel");                                                                                       \
   } while (0)
+#define OK_KRON_LAUNCH(NB, OUT)                                                                                             \
+  do {                                                                                                                      \
+    if (p->precision == OK_FP64) kron_terms_kernel<double><<<dim3(NB, 6), block, 0, st>>>(lk, static_cast<double2*>(OUT), a); \
+    else kron_terms_kernel<float><<<dim3(NB, 6), block, 0, st>>>(lk, static_cast<float4*>(OUT), a);                         \
+    OK_LAUNCHED("kron_terms_kernel");                                                                                       \
+  } while (0)
   a.blk0 = 0;
   if (a.mrhs) {   // dense fp32 W of a chunk of blocks -> bounce buffer -> split-fp16 tiles (mrhs_tile_kernel)
     static bool attr_set = false;
@@ -622,8 +729,7 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
       a.blk0 = b0;
       OK_ASM_LAUNCH(1, 2, nb, bounce);
       OK_ASM_LAUNCH(0, 1, nb, bounce);
-      OK_ASM_LAUNCH(2, 2, nb, bounce);
-      OK_ASM_LAUNCH(3, 4, nb, bounce);
+      OK_KRON_LAUNCH(nb, bounce);
       mrhs_tile_kernel<<<dim3(2 * nb, kMrhsStages), kTileThreads, kTileSmem, st>>>(static_cast<const float4*>(bounce), static_cast<__half*>(Wp), b0, a.g.V);
       OK_LAUNCHED("mrhs_tile_kernel");
     }
@@ -633,9 +739,14 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
   a.blk0 = win_nblk < 0 ? 0 : win_blk0;
   OK_ASM_LAUNCH(1, (a.posonly ? 1 : 2), nb, Wp);   // the heavy class first
   OK_ASM_LAUNCH(0, 1, nb, Wp);
-  OK_ASM_LAUNCH(2, (a.posonly ? 1 : 2), nb, Wp);
-  OK_ASM_LAUNCH(3, (a.posonly ? 2 : 4), nb, Wp);
+  if (p->storage == OK_W_DENSE) {
+    OK_KRON_LAUNCH(nb, Wp);
+  } else {
+    OK_ASM_LAUNCH(2, (a.posonly ? 1 : 2), nb, Wp);
+    OK_ASM_LAUNCH(3, (a.posonly ? 2 : 4), nb, Wp);
+  }
 #undef OK_ASM_LAUNCH
+#undef OK_KRON_LAUNCH
   return OK_SUCCESS;
 }
 

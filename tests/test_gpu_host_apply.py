@@ -17,7 +17,13 @@ pytestmark = pytest.mark.gpu
 @pytest.mark.parametrize("prec", [B.OK_FP64, B.OK_FP32])
 @pytest.mark.parametrize("dims", [(4, 4, 4, 8), (4, 4, 2, 16), (4, 4, 2, 36), (4, 4, 2, 9), (4, 3, 3, 2), (3, 3, 3, 8)])
 @pytest.mark.parametrize("pinned", [True, False])
-def test_host_apply_equals_device_apply_and_oracle(dims, prec, pinned):
+@pytest.mark.parametrize("pipeline", [True, False])
+def test_host_apply_equals_device_apply_and_oracle(dims, prec, pinned, pipeline, monkeypatch):
+    # fields below 8 MiB take the sequential path unless OK_HOST_PIPELINE is set (include/ok.h); both are exercised here
+    if pipeline:
+        monkeypatch.setenv("OK_HOST_PIPELINE", "1")
+    else:
+        monkeypatch.delenv("OK_HOST_PIPELINE", raising=False)
     U = I.near_identity_links(dims, 0.3, 1)
     pd = I.make_params(dims, 0.10, I.tadpole_u0(I.mean_plaquette(dims, U)))
     o = oo.Oracle(U, pd)
