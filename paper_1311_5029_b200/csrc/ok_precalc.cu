@@ -142,23 +142,39 @@ __device__ __forceinline__ Site shift(Site s, int mu, int d, const Geom& g) {   
 }
 
 // U_mu(x) with the boundary-condition sign folded in.
+// `links` inside the kernels is the TRANSPOSED copy made by transpose_links_kernel: element e of U_mu(n) at
+// [(9 mu + e) Vpad + n], so that with lane <-> site a warp-wide load is one contiguous 512-byte line (the canonical
+// [n][mu][3][3] layout has 576 bytes between lanes: ncu showed the field-strength and hop kernels L1-throughput bound on it).
 __device__ __forceinline__ cm3 ldU(const double2* __restrict__ links, const Site& s, int mu, const PrecalcArgs& a) {
-  const double2* p = links + ((size_t)index_of(s, a.g) * 4 + mu) * 9;
+  const double2* p = links + (size_t)(9 * mu) * a.Vpad + index_of(s, a.g);
   const double sg = (a.bc[mu] < 0 && s.c[mu] == (mu == 3 ? a.tfold : a.g.L[mu] - 1)) ? -1.0 : 1.0;
   cm3 r;
 #pragma unroll
   for (int i = 0; i < 9; ++i) {
-    double2 v = __ldg(p + i);
+    double2 v = __ldg(p + (size_t)i * a.Vpad);
     r.e[i] = make_double2(sg * v.x, sg * v.y);
   }
   return r;
 }
+// Scratch colour-matrix fields (clover fields, hop blocks) are kept the same way: matrix k, element e of site n at
+// [(9 k + e) Vpad + n] double2 (a `cm3*` advanced by k Vpad still points at matrix k).
 __device__ __forceinline__ cm3 ldF(const cm3* __restrict__ FS, int k, const Site& s, const PrecalcArgs& a) {
-  const double2* p = reinterpret_cast<const double2*>(FS + (size_t)k * a.Vpad + index_of(s, a.g));
+  const double2* p = reinterpret_cast<const double2*>(FS) + (size_t)(9 * k) * a.Vpad + index_of(s, a.g);
   cm3 r;
 #pragma unroll
-  for (int i = 0; i < 9; ++i) r.e[i] = __ldg(p + i);
+  for (int i = 0; i < 9; ++i) r.e[i] = __ldg(p + (size_t)i * a.Vpad);
   return r;
+}
+__device__ __forceinline__ void stF(cm3* __restrict__ FS, int k, int n, const cm3& F, const PrecalcArgs& a) {
+  double2* p = reinterpret_cast<double2*>(FS) + (size_t)(9 * k) * a.Vpad + n;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) p[(size_t)i * a.Vpad] = F.e[i];
+}
+__global__ void __launch_bounds__(256) transpose_links_kernel(const double2* __restrict__ canon, double2* __restrict__ T, PrecalcArgs a) {
+  const long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // one 16-byte element; the transposed side is coalesced
+  if (u >= (long long)36 * a.g.V) return;
+  const int n = (int)(u % a.g.V), q = (int)(u / a.g.V);
+  T[(size_t)q * a.Vpad + n] = __ldg(canon + (size_t)n * 36 + q);
 }
 
 // ------------------------------------------------------------------------- step a1: clover F
@@ -202,7 +218,7 @@ __global__ void __launch_bounds__(128) field_strength_kernel(const double2* __re
       F.e[3 * i + j].x = (Q.e[3 * i + j].x - Q.e[3 * j + i].x) * 0.125;
       F.e[3 * i + j].y = (Q.e[3 * i + j].y + Q.e[3 * j + i].y) * 0.125;
     }
-  FS[(size_t)k * a.Vpad + n] = F;
+  stF(FS, k, n, F, a);
 }
 
 // ------------------------------------------------------------------------- step a1b: colour matrices of the one-link hops
@@ -225,12 +241,11 @@ __global__ void __launch_bounds__(128) hop_blocks_kernel(const double2* __restri
   const Site xp = shift(x, i, 1, a.g);
   const cm3 U = ldU(links, x, i, a);
   const cm3 P = mul(U, ldF(FS, m, xp, a)), Q = mul(ldF(FS, m, x, a), U);
-  cm3* out = HB + (size_t)(5 * i) * a.Vpad + n;
   if (role == 0) {
     cm3 R = zero3();
     axpy(R, 0.0, a.cs, P);
     axpy(R, 0.0, a.cs, Q);
-    out[0] = R;
+    stF(HB, 5 * i, n, R, a);
     return;
   }
   cm3 Sd = zero3(), Dd = zero3();
@@ -250,8 +265,8 @@ __global__ void __launch_bounds__(128) hop_blocks_kernel(const double2* __restri
     G = mul(G, ldU(links, shift(xm, i, 1, a.g), sd, a));
     axpy(Dd, 0.0, -gs * a.cg, G);
   }
-  out[(size_t)(role == 1 ? 2 : 1) * a.Vpad] = Sd;
-  out[(size_t)(role == 1 ? 3 : 4) * a.Vpad] = Dd;
+  stF(HB, 5 * i + (role == 1 ? 2 : 1), n, Sd, a);
+  stF(HB, 5 * i + (role == 1 ? 3 : 4), n, Dd, a);
 }
 
 // ------------------------------------------------------------------------- step a2: W assembly
@@ -653,7 +668,7 @@ static int mrhs_bounce_blocks(const Geom& g) { return g.nblk < kBounceBlocksMax 
 
 size_t precalc_work_bytes(const ok_params* p) {
   Geom g = make_geom(p);
-  const size_t fs = (size_t)(6 + kHopMats) * g.nblk * kBlock * sizeof(cm3);
+  const size_t fs = (size_t)(6 + kHopMats + 4) * g.nblk * kBlock * sizeof(cm3);
   return p->nrhs == 12 ? fs + 256 + (size_t)mrhs_bounce_blocks(g) * kBounceBlockBytes : fs;
 }
 
@@ -696,6 +711,11 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
   a.sij = p->c2 / (2.0 * u0);
   cm3* FS = static_cast<cm3*>(work);
   cudaStream_t st = ctx().stream;
+  // scratch: [6 clover fields][15 hop blocks][the 4 links, transposed]
+  double2* linksT = reinterpret_cast<double2*>(FS + (size_t)(6 + kHopMats) * a.Vpad);
+  transpose_links_kernel<<<(unsigned)(((long long)36 * a.g.V + 255) / 256), 256, 0, st>>>(static_cast<const double2*>(links), linksT, a);
+  OK_LAUNCHED("transpose_links_kernel");
+  links = linksT;
   field_strength_kernel<<<dim3((a.g.V + 127) / 128, 6), 128, 0, st>>>(static_cast<const double2*>(links), FS, a);
   OK_LAUNCHED("field_strength_kernel");
   hop_blocks_kernel<<<dim3((a.g.V + 127) / 128, 9), 128, 0, st>>>(static_cast<const double2*>(links), FS, FS + (size_t)6 * a.Vpad, a);
@@ -721,7 +741,7 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
       OK_CUDA(cudaFuncSetAttribute(mrhs_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSmem));
       attr_set = true;
     }
-    const size_t fs = ((size_t)(6 + kHopMats) * a.g.nblk * kBlock * sizeof(cm3) + 255) / 256 * 256;
+    const size_t fs = ((size_t)(6 + kHopMats + 4) * a.g.nblk * kBlock * sizeof(cm3) + 255) / 256 * 256;
     void* bounce = static_cast<char*>(work) + fs;
     const int cap = mrhs_bounce_blocks(a.g);
     for (int b0 = 0; b0 < a.g.nblk; b0 += cap) {
