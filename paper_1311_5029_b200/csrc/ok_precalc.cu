@@ -229,11 +229,21 @@ __global__ void __launch_bounds__(128) field_strength_kernel(const double2* __re
 //   q = 1: S.C_k =    cs (U B_l(x+i) - B_l(x) U)            q = 3: D.C_k = i c5/u0^4 (U B_k(x+i) + B_k(x) U) + i cg G_l
 //   q = 2: S.C_l =   -cs (U B_k(x+i) - B_k(x) U)            q = 4: D.C_l = i c5/u0^4 (U B_l(x+i) + B_l(x) U) - i cg G_k
 // role 0 writes q = 0; role 1 (products with B_k, staples along l) q = 2, 3; role 2 (B_l, staples along k) q = 1, 4.
-constexpr int kHopMats = 15;
+constexpr int kHopMats = 18;   // 15 of the spatial hops + T_m = (cEE/2u0^4) (U_4 E_m(x+t) - E_m(x) U_4), m = 0..2 (Eq. 2.7)
 __global__ void __launch_bounds__(128) hop_blocks_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS, cm3* __restrict__ HB,
                                                          PrecalcArgs a) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n >= a.g.V) return;
+  if (blockIdx.y >= 9) {   // the temporal hop: S^+_4 components
+    const int m = blockIdx.y - 9;
+    const Site x = site_of(n, a.g);
+    const cm3 U = ldU(links, x, 3, a);
+    cm3 T = zero3();
+    axpy(T, a.s4, 0.0, mul(U, ldF(FS, 3 + m, shift(x, 3, 1, a.g), a)));
+    axpy(T, -a.s4, 0.0, mul(ldF(FS, 3 + m, x, a), U));
+    stF(HB, 15 + m, n, T, a);
+    return;
+  }
   const int i = blockIdx.y / 3, role = blockIdx.y % 3;
   const int k = (i + 1) % 3, l = (i + 2) % 3;
   const int m = role == 0 ? i : (role == 1 ? k : l);       // the B component of this thread's products
@@ -508,6 +518,117 @@ __global__ void __launch_bounds__(32 * 3, CLS == 1 ? OK_CLS1_MINB : 4) assemble_
 #undef OK_ASM
 }
 
+// ------------------------------------------------------------------------- step a2, W^0, W^+-_i, W^+-_4 (dense layout)
+// Terms 0..8: every 6x6 block is a Pauli sum  sum_k sigma_k (x) C_k  whose colour matrices C_k are, up to a constant, one of the
+// scratch fields (clover fields, hop blocks) or a link.  One thread per (site, term); a rolled loop over the colour row reads
+// row ca of each C_k (for the opposite-direction terms: column ca of the matrices at x + offset, conjugated, Eqs. 2.3 / 2.10)
+// straight from the transposed scratch -- 3 contiguous-line loads per matrix -- and writes the four spin rows (alpha, ca) of
+// W.  No matrix is held in registers across rows (the templated path spilled 2.5-3 KB per thread on the seven matrices of a
+// one-link hop), every thread writes its own site only.  fp64 throughout, rounded once.
+template <typename real>
+__global__ void __launch_bounds__(32 * 3) pauli_terms_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                                             typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
+  using unit_t = typename WUnit<real>::type;
+  constexpr int NC = WUnit<real>::NC;
+  const int lane = threadIdx.x;
+  const int term = blockIdx.y * 3 + threadIdx.y;          // 0..8
+  const int blk = blockIdx.x;
+  const int n = (blk + a.blk0) * kBlock + lane;
+  unit_t* Wt = W + ((size_t)blk * kTerms + term) * 12 * NC * kBlock + lane;
+  if (n >= a.g.V) {
+    unit_t z = {};
+    for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
+    return;
+  }
+  const int fam = term == 0 ? 0 : (term >= 7 ? 1 : 2);
+  const int i = fam == 2 ? (term - 1) >> 1 : 3;           // hop direction
+  const bool neg = fam == 0 ? false : (fam == 1 ? term == 8 : ((term - 1) & 1) != 0);
+  Site x = site_of(n, a.g);
+  if (neg)
+    for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
+  const int ns = index_of(x, a.g);
+  const double2* F = reinterpret_cast<const double2*>(FS) + ns;                                   // matrix k, element e: F[(9k+e) Vpad]
+  const double usg = (fam != 0 && a.bc[i] < 0 && x.c[i] == (i == 3 ? a.tfold : a.g.L[i] - 1)) ? -1.0 : 1.0;
+  const double2* Ul = links + (size_t)(9 * (fam == 0 ? 0 : i)) * a.Vpad + ns;                       // the hop's link
+  const int k = fam == 2 ? (i + 1) % 3 : 1, l = fam == 2 ? (i + 2) % 3 : 2;
+  const bool ulA = fam == 1 ? neg : true, lrA = fam == 1 ? !neg : true;
+  const double llsgn = fam == 0 ? -1.0 : 1.0, mass = fam == 0 ? a.mass : 0.0;
+  auto at = [&](const double2* base, int kmat, int e) { return __ldg(base + (size_t)(9 * kmat + e) * a.Vpad); };
+#pragma unroll 1
+  for (int ca = 0; ca < 3; ++ca) {
+    // Pauli components of this colour row: A (diagonal blocks) and B (off-diagonal blocks), index 0 = 1, 1..3 = sigma_x,y,z
+    double2 A[4][3], Bm[4][3];
+#pragma unroll
+    for (int cb = 0; cb < 3; ++cb) {
+      const int e = neg ? 3 * cb + ca : 3 * ca + cb;       // the adjoint reads the transposed element
+      const double2 z = make_double2(0.0, 0.0);
+      double2 a0 = z, a1 = z, a2 = z, a3 = z, b0 = z, b1 = z, b2 = z, b3 = z;
+      if (fam == 0) {          // D^0 = i d0 sum sigma_m B_m ; S^0 = s0 sum sigma_m E_m     (Eq. 2.6)
+        const double2 f0 = at(F, 0, e), f1 = at(F, 1, e), f2 = at(F, 2, e);
+        a1 = make_double2(-a.d0 * f0.y, a.d0 * f0.x); a2 = make_double2(-a.d0 * f1.y, a.d0 * f1.x); a3 = make_double2(-a.d0 * f2.y, a.d0 * f2.x);
+        const double2 g0 = at(F, 3, e), g1 = at(F, 4, e), g2 = at(F, 5, e);
+        b1 = make_double2(a.s0 * g0.x, a.s0 * g0.y); b2 = make_double2(a.s0 * g1.x, a.s0 * g1.y); b3 = make_double2(a.s0 * g2.x, a.s0 * g2.y);
+      } else if (fam == 1) {   // D^+_4 = -U_4 ; S^+_4 = sum sigma_m T_m                        (Eq. 2.7)
+        const double2 u = __ldg(Ul + (size_t)e * a.Vpad);
+        a0 = make_double2(-usg * u.x, -usg * u.y);
+        b1 = at(F, 6 + 15, e); b2 = at(F, 6 + 16, e); b3 = at(F, 6 + 17, e);
+      } else {                 // Eq. (2.8): hop_blocks_kernel's q = 0..4 of direction i, and U_i itself
+        const double2 u = __ldg(Ul + (size_t)e * a.Vpad);
+        const int hb = 6 + 5 * i;
+        const double2 vi_b = make_double2(a.a1 * usg * u.x, a.a1 * usg * u.y);                     // S.C_i = a1 U
+        const double2 vk_b = at(F, hb + 1, e), vl_b = at(F, hb + 2, e), vk_a = at(F, hb + 3, e), vl_a = at(F, hb + 4, e);
+        a0 = make_double2(a.d1 * usg * u.x, a.d1 * usg * u.y);                                     // D.C_0 = d1 U
+        b0 = at(F, hb, e);
+        // direction d carries the i-, k- or l-component
+        a1 = i == 0 ? z : (k == 0 ? vk_a : vl_a); b1 = i == 0 ? vi_b : (k == 0 ? vk_b : vl_b);
+        a2 = i == 1 ? z : (k == 1 ? vk_a : vl_a); b2 = i == 1 ? vi_b : (k == 1 ? vk_b : vl_b);
+        a3 = i == 2 ? z : (k == 2 ? vk_a : vl_a); b3 = i == 2 ? vi_b : (k == 2 ? vk_b : vl_b);
+      }
+      if (neg) {               // A -> A^dag, B -> -B^dag (the element was read transposed)
+        a0.y = -a0.y; a1.y = -a1.y; a2.y = -a2.y; a3.y = -a3.y;
+        b0.x = -b0.x; b1.x = -b1.x; b2.x = -b2.x; b3.x = -b3.x;
+      }
+      A[0][cb] = a0; A[1][cb] = a1; A[2][cb] = a2; A[3][cb] = a3;
+      Bm[0][cb] = b0; Bm[1][cb] = b1; Bm[2][cb] = b2; Bm[3][cb] = b3;
+    }
+#pragma unroll
+    for (int alpha = 0; alpha < 4; ++alpha) {
+      const int bi = alpha >> 1, al = alpha & 1;
+      double2 row[12];
+#pragma unroll
+      for (int beta = 0; beta < 4; ++beta) {
+        const int bj = beta >> 1, be = beta & 1;
+        const bool diag = bi == bj;
+        const bool useA = diag && (bi == 0 ? ulA : lrA);
+#pragma unroll
+        for (int cb = 0; cb < 3; ++cb) {
+          const double2 c0 = diag ? A[0][cb] : Bm[0][cb], c1 = diag ? A[1][cb] : Bm[1][cb], c2 = diag ? A[2][cb] : Bm[2][cb],
+                        c3 = diag ? A[3][cb] : Bm[3][cb];
+          double2 v;
+          if (al == be) v = al == 0 ? make_double2(c0.x + c3.x, c0.y + c3.y) : make_double2(c0.x - c3.x, c0.y - c3.y);
+          else v = al == 0 ? make_double2(c1.x + c2.y, c1.y - c2.x) : make_double2(c1.x - c2.y, c1.y + c2.x);
+          if (diag) {
+            if (!useA) v = make_double2(0.0, 0.0);
+            if (alpha == beta && ca == cb) v.x += mass;
+          } else if (bi == 1) {
+            v.x *= llsgn; v.y *= llsgn;
+          }
+          row[3 * beta + cb] = v;
+        }
+      }
+      unit_t* dst = Wt + (size_t)(3 * alpha + ca) * NC * kBlock;
+      if constexpr (sizeof(real) == 4) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c)
+          dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
+      } else {
+#pragma unroll
+        for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------- step a2, the 18 two-link terms (dense layout)
 // W^{++}_ii, W^{++}_ij, W^{+-}_ij and their conjugates (Eqs. 2.9-2.12; terms 9..26, two thirds of W's bytes) are Kronecker
 // products  W = K (x) P  of a 4x4 spin matrix K and ONE 3x3 colour matrix:
@@ -718,7 +839,7 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
   links = linksT;
   field_strength_kernel<<<dim3((a.g.V + 127) / 128, 6), 128, 0, st>>>(static_cast<const double2*>(links), FS, a);
   OK_LAUNCHED("field_strength_kernel");
-  hop_blocks_kernel<<<dim3((a.g.V + 127) / 128, 9), 128, 0, st>>>(static_cast<const double2*>(links), FS, FS + (size_t)6 * a.Vpad, a);
+  hop_blocks_kernel<<<dim3((a.g.V + 127) / 128, 12), 128, 0, st>>>(static_cast<const double2*>(links), FS, FS + (size_t)6 * a.Vpad, a);
   OK_LAUNCHED("hop_blocks_kernel");
   const dim3 block(32, 3);
   const double2* lk = static_cast<const double2*>(links);
@@ -727,6 +848,12 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
     if (p->precision == OK_FP64) assemble_W_kernel<double, CLS><<<dim3(NB, NY), block, 0, st>>>(lk, FS, static_cast<double2*>(OUT), a); \
     else assemble_W_kernel<float, CLS><<<dim3(NB, NY), block, 0, st>>>(lk, FS, static_cast<float4*>(OUT), a);               \
     OK_LAUNCHED("assemble_W_kernel");                                                                                       \
+  } while (0)
+#define OK_PAULI_LAUNCH(NB, OUT)                                                                                            \
+  do {                                                                                                                      \
+    if (p->precision == OK_FP64) pauli_terms_kernel<double><<<dim3(NB, 3), block, 0, st>>>(lk, FS, static_cast<double2*>(OUT), a); \
+    else pauli_terms_kernel<float><<<dim3(NB, 3), block, 0, st>>>(lk, FS, static_cast<float4*>(OUT), a);                    \
+    OK_LAUNCHED("pauli_terms_kernel");                                                                                      \
   } while (0)
 #define OK_KRON_LAUNCH(NB, OUT)                                                                                             \
   do {                                                                                                                      \
@@ -747,8 +874,7 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
     for (int b0 = 0; b0 < a.g.nblk; b0 += cap) {
       const int nb = a.g.nblk - b0 < cap ? a.g.nblk - b0 : cap;
       a.blk0 = b0;
-      OK_ASM_LAUNCH(1, 2, nb, bounce);
-      OK_ASM_LAUNCH(0, 1, nb, bounce);
+      OK_PAULI_LAUNCH(nb, bounce);
       OK_KRON_LAUNCH(nb, bounce);
       mrhs_tile_kernel<<<dim3(2 * nb, kMrhsStages), kTileThreads, kTileSmem, st>>>(static_cast<const float4*>(bounce), static_cast<__half*>(Wp), b0, a.g.V);
       OK_LAUNCHED("mrhs_tile_kernel");
@@ -757,16 +883,18 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
   }
   const int nb = win_nblk < 0 ? a.g.nblk : win_nblk;
   a.blk0 = win_nblk < 0 ? 0 : win_blk0;
-  OK_ASM_LAUNCH(1, (a.posonly ? 1 : 2), nb, Wp);   // the heavy class first
-  OK_ASM_LAUNCH(0, 1, nb, Wp);
   if (p->storage == OK_W_DENSE) {
+    OK_PAULI_LAUNCH(nb, Wp);
     OK_KRON_LAUNCH(nb, Wp);
   } else {
+    OK_ASM_LAUNCH(1, (a.posonly ? 1 : 2), nb, Wp);   // the heavy class first
+    OK_ASM_LAUNCH(0, 1, nb, Wp);
     OK_ASM_LAUNCH(2, (a.posonly ? 1 : 2), nb, Wp);
     OK_ASM_LAUNCH(3, (a.posonly ? 2 : 4), nb, Wp);
   }
 #undef OK_ASM_LAUNCH
 #undef OK_KRON_LAUNCH
+#undef OK_PAULI_LAUNCH
   return OK_SUCCESS;
 }
 
