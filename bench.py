@@ -63,8 +63,11 @@ WORKLOADS["20x20x20x64-fp64-ds"] = WORKLOADS["20x20x20x64-fp64"]
 WORKLOADS["32x32x32x64-fp32-ds"] = WORKLOADS["32x32x32x64-fp32"]
 WORKLOADS["20x20x20x64-fp32-conj"] = WORKLOADS["20x20x20x64-fp32"]
 WORKLOADS["20x20x20x64-fp64-conj"] = WORKLOADS["20x20x20x64-fp64"]
-STORAGE = {"20x20x20x64-fp32-conj": 3, "20x20x20x64-fp64-conj": 3, "20x20x20x64-fp32-block": 1, "20x20x20x64-fp32-ds": 2, "20x20x20x64-fp64-ds": 2, "32x32x32x64-fp32-ds": 2}
-W_COMPLEX_PER_SITE = {0: 27 * 144, 1: 260 * 9, 2: 132 * 9, 3: 70 * 9}
+WORKLOADS["20x20x20x64-fp32-pauli"] = WORKLOADS["20x20x20x64-fp32"]
+WORKLOADS["20x20x20x64-fp64-pauli"] = WORKLOADS["20x20x20x64-fp64"]
+WORKLOADS["32x32x32x64-fp32-pauli"] = WORKLOADS["32x32x32x64-fp32"]
+STORAGE = {"20x20x20x64-fp32-pauli": 4, "20x20x20x64-fp64-pauli": 4, "32x32x32x64-fp32-pauli": 4, "20x20x20x64-fp32-conj": 3, "20x20x20x64-fp64-conj": 3, "20x20x20x64-fp32-block": 1, "20x20x20x64-fp32-ds": 2, "20x20x20x64-fp64-ds": 2, "32x32x32x64-fp32-ds": 2}
+W_COMPLEX_PER_SITE = {0: 27 * 144, 1: 260 * 9, 2: 132 * 9, 3: 70 * 9, 4: 37 * 9}
 
 
 def make_links(dims, eps, lseed):
@@ -376,6 +379,7 @@ class Prepared:
         stream.synchronize()
         self.alg = self.V * alg_bytes_per_site(self.sbytes, self.nrhs, self.storage)
         self.kernel = (KERNEL_NAME[(self.sbytes, self.nrhs)] if self.storage == 0 else
+                       ("okd::apply_pauli_kernel<%s>" % ("float" if self.sbytes == 4 else "double")) if self.storage == 4 else
                        "okd::apply_sparse_kernel<%s,%d>" % ("float" if self.sbytes == 4 else "double", self.storage))
 
     def step(self, rec=None):
@@ -450,6 +454,14 @@ class Prepared:
         r = {"bound": "hbm", "kernel": self.kernel, "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
              "frac_of_nominal_8000": ach / 8000.0, "peak_source": peaks["_source"], "algorithmic_bytes_per_launch": self.alg}
         r.update(ncu_record(self.wl))
+        if self.storage == 4:
+            # OK_W_PAULI is bound by the fp32 pipes, not by HBM: 68 matrix uses x 36 complex MACs x 8 flop per site
+            # against 148 SMs x 128 lanes x 2 flop x sm_max_mhz; the HBM figures above stay for comparison with the other formats
+            flops = 68 * 36 * 8 * self.V
+            peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+            r["alu"] = {"bound": "alu", "achieved": flops / (a_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                        "frac": flops / (a_ms * 1e-3) / 1e12 / peak, "flops_per_launch": flops,
+                        "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 flop x sm_max_mhz (DESIGN.md 6.6)"}
         return r
 
     def tensor(self, a_ms, clocks, peaks, ncu):
@@ -670,7 +682,7 @@ def run_ours(args, wl):
             "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if sbytes == 4 else "f64", "data": "synthetic",
-            "config": {"workload": wl, "nrhs": nrhs, "storage": ["dense", "block (260 colour blocks)", "ds (132 colour blocks)", "conj (70 colour blocks)"][P.storage], "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
+            "config": {"workload": wl, "nrhs": nrhs, "storage": ["dense", "block (260 colour blocks)", "ds (132 colour blocks)", "conj (70 colour blocks)", "pauli (49 colour blocks as 37 stored matrices)"][P.storage], "step": f"ok_precalc_W + {NAPPLY} x ok_dirac_apply + ok_bicgstab(tol={tol:g})",
                        "sites": V, "l2_flush": "not needed: W (%.1f GB) >> L2 (126 MB)" % (B.ok_W_bytes(p) / 1e9),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "plaquette": P.plaq, "u0": P.pd["u0"]},
             "pct_of_peak": {"measured_copy": 100 * value / world / peaks["hbm_gbs"], "nominal_8000": 100 * value / world / 8000.0},
@@ -730,7 +742,7 @@ def run_sweep(args):
         links = torch.from_numpy(U).to(dev)
         V = int(np.prod(dims))
         psi = torch.from_numpy(I.gaussian_spinor(dims, 9)).to(torch.complex64).to(dev)
-        for storage in (0, 2, 3):
+        for storage in (0, 2, 3, 4):
             p = B.make_params(pd, B.OK_FP32, storage=storage)
             W, work = B.alloc_W(p, dev), B.alloc_work(p, dev)
             src, out = B.alloc_vec(p, dev), B.alloc_vec(p, dev)
@@ -749,7 +761,7 @@ def run_sweep(args):
             stream.synchronize()
             ms = e0.elapsed_time(e1) / nrep
             alg = V * alg_bytes_per_site(4, 1, storage)
-            rows.append({"dims": "x".join(map(str, dims)), "sites": V, "storage": ["dense", "block", "ds", "conj"][storage],
+            rows.append({"dims": "x".join(map(str, dims)), "sites": V, "storage": ["dense", "block", "ds", "conj", "pauli"][storage],
                          "W_GB": B.ok_W_bytes(p) / 1e9, "apply_ms": ms, "GBps": alg / ms / 1e6, "sites_per_s": V / ms * 1e3,
                          "gflops": V * FLOP_PER_SITE / ms / 1e6})
             B.ok_set_workspace(None)

@@ -85,6 +85,13 @@ extern "C" {
                             /* 5 040 B fp32); the opposite-direction matrices are rebuilt from the          */
                             /* neighbour site by the conjugation relations, Eqs. (2.3), (2.10) */
 
+#define OK_W_PAULI 4        /* the Pauli components of D and S of W^0 and the 13 positive-direction terms: the paper's "50 colour  */
+                            /* blocks" (49 by the structure of Eqs. 2.6-2.12, 37 stored matrices = 2 664 B fp32   */
+                            /* once components that coincide up to a constant of the action are merged; csrc/ok_pauli.cu).        */
+                            /* Written by ok_precalc_W only (ok_pack_W returns OK_EINVAL: a general W has no such form);          */
+                            /* ok_unpack_W rebuilds the 27 dense matrices.  The apply is bound by the fp32 pipes, not by HBM.     */
+#define OK_W_PAULI_MATS 37
+
 #define OK_NTERMS 27
 #define OK_SITE_BLOCK 32
 #define OK_W_HEADER_BYTES 1024
@@ -107,7 +114,7 @@ typedef struct ok_params {
   double kappa, u0;   /* hopping parameter, tadpole factor (Eq. 2.6)                           */
   double zeta, rs;    /* Eqs. (2.6)-(2.8)                                                      */
   double cB, cE, cEE, c1, c2, c3, c4, c5;
-  int32_t storage;    /* OK_W_DENSE / OK_W_BLOCK / OK_W_DS: how W is held in device memory            */
+  int32_t storage;    /* OK_W_DENSE / OK_W_BLOCK / OK_W_DS / OK_W_CONJ / OK_W_PAULI: how W is held in device memory */
   int32_t reserved_;  /* 0; OK_SLAB (1) in the parameters of a t-slab (see ok_slab_*): dims[3] is then the slab's    */
                       /* own extent Tloc and the lattice is open in t (its t-neighbours arrive as halo slices)       */
 } ok_params;

@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 OK_FP32, OK_FP64 = 0, 1
-OK_W_DENSE, OK_W_BLOCK, OK_W_DS, OK_W_CONJ = 0, 1, 2, 3
+OK_W_DENSE, OK_W_BLOCK, OK_W_DS, OK_W_CONJ, OK_W_PAULI = 0, 1, 2, 3, 4
 OK_NTERMS = 27
 OK_W_HEADER_BYTES = 1024
 OK_SLAB, OK_SLAB_LINK_HALO = 1, 2

@@ -49,7 +49,8 @@ int fail_cuda(cudaError_t e, const char* where) {
 
 static uint32_t layout_id(const ok_params* p) {
   if (p->nrhs == 12) return kLayoutMrhs;
-  return p->storage == OK_W_BLOCK ? kLayoutBlock : p->storage == OK_W_DS ? kLayoutDS : p->storage == OK_W_CONJ ? kLayoutConj : kLayoutDense;
+  return p->storage == OK_W_BLOCK ? kLayoutBlock : p->storage == OK_W_DS ? kLayoutDS : p->storage == OK_W_CONJ ? kLayoutConj :
+         p->storage == OK_W_PAULI ? kLayoutPauli : kLayoutDense;
 }
 
 bool valid_params(const ok_params* p) {
@@ -64,7 +65,7 @@ bool valid_params(const ok_params* p) {
   if (p->precision != OK_FP32 && p->precision != OK_FP64) return false;
   if (p->nrhs != 1 && p->nrhs != 12) return false;
   if (p->nrhs == 12 && p->precision != OK_FP32) return false;
-  if (p->storage < OK_W_DENSE || p->storage > OK_W_CONJ) return false;
+  if (p->storage < OK_W_DENSE || p->storage > OK_W_PAULI) return false;
   if (p->nrhs == 12 && p->storage != OK_W_DENSE) return false;
   if (!(p->kappa > 0.0) || !(p->u0 > 0.0)) return false;
   return true;
@@ -159,6 +160,7 @@ size_t ok_W_bytes(const ok_params* p) {
   if (!valid_params(p)) return 0;
   Geom g = make_geom(p);
   if (p->nrhs == 12) return OK_W_HEADER_BYTES + (size_t)g.V * kMrhsWSiteBytes;
+  if (p->storage == OK_W_PAULI) return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * (OK_W_PAULI_MATS * 9) * 2 * real_bytes(p);
   if (p->storage != OK_W_DENSE)
     return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * sparse_site_units_rt(p->storage) * 2 * real_bytes(p);
   return OK_W_HEADER_BYTES + (size_t)g.nblk * kBlock * kTerms * 144 * 2 * real_bytes(p);
@@ -200,6 +202,7 @@ int ok_unpack_spinor(const ok_params* p, const void* packed, void* canon) {
 
 int ok_pack_W(const ok_params* p, const void* canon, void* W) {
   if (!valid_params(p) || !aligned16(canon) || !aligned16(W)) return OK_EINVAL;
+  if (p->storage == OK_W_PAULI) return OK_EINVAL;   // only ok_precalc_W writes this format (ok.h)
   int st = bind_device();
   if (st) return st;
   st = write_header(W, p);
@@ -212,6 +215,7 @@ int ok_unpack_W(const void* W, void* canon) {
   if (!aligned16(canon)) return OK_EINVAL;
   int st = lookup_W(W, &p);
   if (st) return st;
+  if (p.storage == OK_W_PAULI) return launch_unpack_pauli(&p, W_payload(W), canon);
   return launch_pack_W(&p, canon, const_cast<char*>(W_payload(W)), true);
 }
 

@@ -167,6 +167,7 @@ constexpr int kSmallLatticeBlocks = 4 * 148;   // below four CTAs per SM: 12 war
 int launch_apply(const ok_params* p, const void* W, const void* psi, void* out, double* partials,
                  const void* dot_a, const void* /*unused*/) {
   if (p->nrhs != 1) return OK_EINVAL;   // multi-RHS apply: ok_apply_mrhs.cu
+  if (p->storage == OK_W_PAULI) return launch_apply_pauli(p, W, psi, out, partials, dot_a);     // ok_pauli.cu
   if (p->storage != OK_W_DENSE) return launch_apply_sparse(p, W, psi, out, partials, dot_a);   // ok_apply_sparse.cu
   int st = upload_offsets();
   if (st) return st;

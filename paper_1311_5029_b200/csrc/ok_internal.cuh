@@ -18,6 +18,7 @@ constexpr uint32_t kLayoutDense = 1;       // [block][term][row][c][site][16 B]
 constexpr uint32_t kLayoutBlock = 4;       // OK_W_BLOCK: [block][unit 2340][site][complex]   (ok_sparse.cuh)
 constexpr uint32_t kLayoutConj = 6;        // OK_W_CONJ:  [block][unit 630][site][complex]
 constexpr uint32_t kLayoutDS = 5;          // OK_W_DS:    [block][unit 1188][site][complex]
+constexpr uint32_t kLayoutPauli = 7;       // OK_W_PAULI: [block][37 x 9 units][site][complex]   (ok_pauli.cu)
 constexpr uint32_t kLayoutMrhs = 3;        // nrhs = 12: per-site tcgen05 operand tiles, split fp16 (ok_apply_mrhs.cu)
 
 // ---- nrhs = 12 (tensor-core) layouts, fp32 fields (ok_apply_mrhs.cu) -------------------------------
@@ -219,6 +220,8 @@ size_t bicgstab_slab_work_bytes(const ok_params* p);
 size_t bicgstab_slab_shared_bytes(int nslab, int nranks);
 int run_bicgstab_slabs(int nslab, const ok_params* const* ps, const void* const* Wpayloads, const void* const* srcs, void* const* xs,
                        double tol, int maxit, const ok_comm* comm, int* iters, double* resid);
+int launch_apply_pauli(const ok_params* p, const void* Wpayload, const void* psi, void* out, double* dot_partials, const void* dot_a);
+int launch_unpack_pauli(const ok_params* p, const void* Wpayload, void* canon);
 int launch_apply_sparse(const ok_params* p, const void* Wpayload, const void* psi, void* out, double* dot_partials, const void* dot_a);
 size_t precalc_work_bytes(const ok_params* p);
 int run_bicgstab(const ok_params* p, const void* Wpayload, const void* src, void* x, double tol, int maxit,

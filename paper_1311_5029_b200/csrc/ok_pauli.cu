@@ -1,0 +1,494 @@
+// OK_W_PAULI: the paper's strongest compression of the precalculation matrices ("compress the 432 color
+// blocks into 50"), SURVEY.md 8(f) item 2.  Every 6x6 block of Eqs. (2.6)-(2.12) is a Pauli sum  sum_k sigma_k (x) C_k  of 3x3
+// colour matrices; counting the non-vanishing components block by block gives
+//   W^0: 3 + 3    W^+_4: 1 + 3    W^+_i: 3 + 4 (x3)    W^{++}_ii: 1 + 1 (x3)    W^{++}_ij, W^{+-}_ij: 0 + 2 (x6)    = 49
+// colour blocks for W^0 and the 13 positive-direction matrices (the opposite-direction ones follow from Eqs. 2.3, 2.10).
+// Where two components of a term are the same matrix up to a constant of the action (D.C_0 = d1 U and S.C_i = a1 U of a hop;
+// D = (c4/u0) P and S = ((c1+2c2)/2u0) sigma_i P of W_ii; the two sigma components of a pair term) it is stored once, so a
+// site holds 37 colour matrices = 333 complex = 2 664 B in fp32 (dense: 31 104 B; OK_W_CONJ: 5 040 B).
+//
+// Stored matrices, index m (layout [block 32 sites][9 m + element][site][complex]):
+//   0..2  i d0 B_m           3..5  s0 E_m             (Eq. 2.6; D^0, S^0 components sigma_m)
+//   6     U_4                7..9  T_m = (cEE/2u0^4)(U_4 E_m(x+t) - E_m(x) U_4)                              (Eq. 2.7)
+//   10+6i U_i   +1 S.C_0   +2 S.C_k   +3 S.C_l   +4 D.C_k   +5 D.C_l      (Eq. 2.8; i = 0..2, cyclic (i,k,l); hop_blocks_kernel)
+//   28+i  P_ii = U_i(x) U_i(x+i)                                                                             (Eq. 2.9)
+//   31+2q P_ij = U_i(x)U_j(x+i) + U_j(x)U_i(x+j)     32+2q  P_i-j = U_i(x)U_j(x-j+i)^dag + U_j(x-j)^dag U_i(x-j)   (2.11, 2.12)
+// The boundary-condition signs are inside the links, as everywhere.
+//
+// Apply: out(x) = mass psi(x) + sum over 68 "uses" of a stored matrix: (matrix m at the neighbour site of stencil term t, or its
+// adjoint for an opposite-direction term, Eqs. 2.3/2.10) times the four colour vectors of psi(x + offset_t), placed into the
+// output by one or two Pauli placements  coef * sigma_k  in the diagonal (D) or off-diagonal (S) spin blocks.  The uses are a
+// constant table built on the host from the equations (build_uses below); the kernel is one rolled loop over it.
+// 21 kflop per 2 856 B per site: this format is bound by the fp32 pipes, not by HBM.
+#include "ok_internal.cuh"
+
+namespace okd {
+
+namespace {
+
+constexpr int kPauliMats = OK_W_PAULI_MATS;   // 37
+constexpr int kMaxUses = 80;
+enum Coef { C_ONE = 0, C_MINUS, C_D1, C_A1, C_MA1, C_DII, C_SII, C_MSII, C_SIJ, C_MSIJ, C_COUNT };
+
+struct Placement {
+  int8_t kind;    // 0: D (diagonal spin blocks), 1: S (off-diagonal)
+  int8_t sigma;   // 0 = 1, 1..3 = sigma_x, sigma_y, sigma_z
+  int8_t coef;    // Coef
+  int8_t flags;   // D: bit 0 = upper-left block present, bit 1 = lower-right ; S: bit 2 = the lower-left block carries a minus
+};
+struct Use {
+  int8_t m, term, adj, np;
+  Placement pl[2];
+};
+struct UseTable {
+  int n;
+  int first[5];   // warp w of a CTA handles uses first[w] .. first[w+1]-1 (whole terms, so the neighbour spinor is loaded once per term)
+  Use u[kMaxUses];
+};
+
+__constant__ UseTable c_uses;
+__constant__ int8_t c_poff2[kTerms][4];
+static bool g_pauli_ready = false;
+static UseTable h_uses;
+
+Placement Dp(int sigma, int coef, int ul = 1, int lr = 1) { return Placement{0, (int8_t)sigma, (int8_t)coef, (int8_t)(ul | (lr << 1))}; }
+Placement Sp(int sigma, int coef, int llneg = 0) { return Placement{1, (int8_t)sigma, (int8_t)coef, (int8_t)(llneg << 2)}; }
+
+void add_use(UseTable& t, int m, int term, int adj, Placement a, const Placement* b = nullptr) {
+  Use& u = t.u[t.n++];
+  u.m = (int8_t)m; u.term = (int8_t)term; u.adj = (int8_t)adj; u.np = b ? 2 : 1;
+  u.pl[0] = a;
+  u.pl[1] = b ? *b : Placement{0, 0, 0, 0};
+}
+
+// The 68 uses, term by term, from Eqs. (2.6)-(2.12) and the conjugation relations (2.3), (2.10):
+// the opposite-direction matrix is [[D^dag, -S^dag], [-S^dag, D^dag]] of the blocks at the neighbour site.
+void build_uses(UseTable& t) {
+  t.n = 0;
+  int start_of_term[kTerms + 1];
+  auto begin = [&](int term) { start_of_term[term] = t.n; };
+  // term 0: W^0 = [[D0, S0], [-S0, D0]] + mass
+  begin(0);
+  for (int m = 0; m < 3; ++m) add_use(t, m, 0, 0, Dp(m + 1, C_ONE));
+  for (int m = 0; m < 3; ++m) add_use(t, 3 + m, 0, 0, Sp(m + 1, C_ONE, 1));
+  // terms 1..6: one-link hops +-i
+  for (int i = 0; i < 3; ++i) {
+    const int b = 10 + 6 * i, k = (i + 1) % 3, l = (i + 2) % 3;
+    for (int neg = 0; neg < 2; ++neg) {
+      const int term = 1 + 2 * i + neg;
+      begin(term);
+      const Placement su = Sp(i + 1, neg ? C_MA1 : C_A1);
+      add_use(t, b, term, neg, Dp(0, C_D1), &su);
+      add_use(t, b + 1, term, neg, Sp(0, neg ? C_MINUS : C_ONE));
+      add_use(t, b + 2, term, neg, Sp(k + 1, neg ? C_MINUS : C_ONE));
+      add_use(t, b + 3, term, neg, Sp(l + 1, neg ? C_MINUS : C_ONE));
+      add_use(t, b + 4, term, neg, Dp(k + 1, C_ONE));
+      add_use(t, b + 5, term, neg, Dp(l + 1, C_ONE));
+    }
+  }
+  // terms 7, 8: temporal hop; D = -U_4 sits in the lower-right block for +t and in the upper-left one for -t
+  for (int neg = 0; neg < 2; ++neg) {
+    begin(7 + neg);
+    add_use(t, 6, 7 + neg, neg, Dp(0, C_MINUS, neg ? 1 : 0, neg ? 0 : 1));
+    for (int m = 0; m < 3; ++m) add_use(t, 7 + m, 7 + neg, neg, Sp(m + 1, neg ? C_MINUS : C_ONE));
+  }
+  // terms 9..14: +-2i
+  for (int i = 0; i < 3; ++i)
+    for (int neg = 0; neg < 2; ++neg) {
+      begin(9 + 2 * i + neg);
+      const Placement s = Sp(i + 1, neg ? C_MSII : C_SII);
+      add_use(t, 28 + i, 9 + 2 * i + neg, neg, Dp(0, C_DII), &s);
+    }
+  // terms 15..26: pairs (x,y), (x,z), (y,z): +i+j, -i-j, +i-j, -i+j
+  for (int q = 0; q < 3; ++q) {
+    const int i = q == 2 ? 1 : 0, j = q == 0 ? 1 : 2;
+    for (int w = 0; w < 4; ++w) {
+      const int term = 15 + 4 * q + w, neg = w & 1, minus = w >= 2;
+      begin(term);
+      const int ci = neg ? C_MSIJ : C_SIJ, cj = (neg != minus) ? C_MSIJ : C_SIJ;
+      const Placement sj = Sp(j + 1, cj);
+      add_use(t, 31 + 2 * q + (minus ? 1 : 0), term, neg, Sp(i + 1, ci), &sj);
+    }
+  }
+  start_of_term[kTerms] = t.n;
+  // four warps, whole terms each, as even as the term boundaries allow
+  t.first[0] = 0;
+  t.first[4] = t.n;
+  int term = 0;
+  for (int w = 1; w < 4; ++w) {
+    while (term < kTerms && start_of_term[term] < (t.n * w + 2) / 4) ++term;
+    t.first[w] = start_of_term[term];
+  }
+}
+
+template <typename real> struct PV;
+template <> struct PV<float> { using cx = float2; using vec = float4; static constexpr int NC = 6; };
+template <> struct PV<double> { using cx = double2; using vec = double2; static constexpr int NC = 12; };
+
+struct PauliArgs {
+  Geom g;
+  double coef[C_COUNT];
+  double mass;
+};
+
+__device__ __forceinline__ int wrapp(int x, int L) {
+  x += (x < 0) ? L : 0;
+  x -= (x >= L) ? L : 0;
+  return x;
+}
+
+// v * f(sigma, al), f = sigma[al][src]: 1 (sigma_0, sigma_x), -/+ i (sigma_y: al = 0 / 1), +/- 1 (sigma_z)
+template <typename cx, typename real>
+__device__ __forceinline__ cx pauli_factor(cx v, int sigma, int al, real c) {
+  if (sigma == 2) v = al == 0 ? cx{v.y, -v.x} : cx{-v.y, v.x};
+  if (sigma == 3 && al == 1) c = -c;
+  return cx{c * v.x, c * v.y};
+}
+
+constexpr int kPauliWarps = 4;
+
+// acc[BASE + 3 al + ca] += c * sigma[al][be] * tv[be][ca]   (BASE = 0: upper spin half of the output, 6: lower)
+template <int BASE, typename cx, typename real>
+__device__ __forceinline__ void place(cx (&acc)[12], const cx (&tv)[2][3], int sigma, real c) {
+  if (sigma == 0 || sigma == 3) {           // diagonal in spin: +c, +-c
+    const real c1 = sigma == 3 ? -c : c;
+#pragma unroll
+    for (int ca = 0; ca < 3; ++ca) {
+      acc[BASE + ca].x = fma(c, tv[0][ca].x, acc[BASE + ca].x);
+      acc[BASE + ca].y = fma(c, tv[0][ca].y, acc[BASE + ca].y);
+      acc[BASE + 3 + ca].x = fma(c1, tv[1][ca].x, acc[BASE + 3 + ca].x);
+      acc[BASE + 3 + ca].y = fma(c1, tv[1][ca].y, acc[BASE + 3 + ca].y);
+    }
+  } else if (sigma == 1) {                  // sigma_x: swaps the two spins
+#pragma unroll
+    for (int ca = 0; ca < 3; ++ca) {
+      acc[BASE + ca].x = fma(c, tv[1][ca].x, acc[BASE + ca].x);
+      acc[BASE + ca].y = fma(c, tv[1][ca].y, acc[BASE + ca].y);
+      acc[BASE + 3 + ca].x = fma(c, tv[0][ca].x, acc[BASE + 3 + ca].x);
+      acc[BASE + 3 + ca].y = fma(c, tv[0][ca].y, acc[BASE + 3 + ca].y);
+    }
+  } else {                                  // sigma_y: out_0 += -i c t_1 ; out_1 += i c t_0
+#pragma unroll
+    for (int ca = 0; ca < 3; ++ca) {
+      acc[BASE + ca].x = fma(c, tv[1][ca].y, acc[BASE + ca].x);
+      acc[BASE + ca].y = fma(-c, tv[1][ca].x, acc[BASE + ca].y);
+      acc[BASE + 3 + ca].x = fma(-c, tv[0][ca].y, acc[BASE + 3 + ca].x);
+      acc[BASE + 3 + ca].y = fma(c, tv[0][ca].x, acc[BASE + 3 + ca].y);
+    }
+  }
+}
+
+template <typename real, bool DOT>
+__global__ void __launch_bounds__(32 * kPauliWarps)
+apply_pauli_kernel(const typename PV<real>::cx* __restrict__ W, const typename PV<real>::vec* __restrict__ psi,
+                   typename PV<real>::vec* __restrict__ out, PauliArgs a, const typename PV<real>::vec* __restrict__ dot_a,
+                   double* __restrict__ partials) {
+  using cx = typename PV<real>::cx;
+  using vec = typename PV<real>::vec;
+  constexpr int NC = PV<real>::NC;
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  const int blk = blockIdx.x;
+  int n = blk * kBlock + lane;
+  const bool live = n < a.g.V;
+  if (!live) n = 0;
+  const int x = n % a.g.L[0];
+  int q = n / a.g.L[0];
+  const int y = q % a.g.L[1];
+  q /= a.g.L[1];
+  const int z = q % a.g.L[2];
+  const int t = q / a.g.L[2];
+
+  cx acc[12];
+#pragma unroll
+  for (int r = 0; r < 12; ++r) acc[r] = cx{0, 0};
+  cx phi[12];
+  // neighbour site of a stencil term: it holds the spinor and, for an opposite-direction term, the matrices
+  auto site_of_term = [&](int term) {
+    const int xx = wrapp(x + c_poff2[term][0], a.g.L[0]);
+    const int yy = wrapp(y + c_poff2[term][1], a.g.L[1]);
+    const int zz = wrapp(z + c_poff2[term][2], a.g.L[2]);
+    const int tt = wrapp(t + c_poff2[term][3], a.g.L[3]);
+    return xx + a.g.L[0] * (yy + a.g.L[1] * (zz + a.g.L[2] * tt));
+  };
+  auto matrix_of = [&](const Use& u, int nn) {   // a positive term and W^0 use the matrices of THIS site
+    const int nm = u.adj ? nn : n;
+    return W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31) + (size_t)(9 * u.m) * kBlock;
+  };
+  // The loop is rolled (one generic body for the 68 uses) and software-pipelined by hand: the nine loads of the NEXT use are
+  // issued before the arithmetic of the current one (every stored matrix is used by its own site and by one neighbour, so
+  // default-policy loads).
+  const int last = c_uses.first[wp + 1];
+  int ui = c_uses.first[wp];
+  Use u = c_uses.u[ui < last ? ui : 0];
+  int nn = site_of_term(u.term);
+  cx C[9];
+  {
+    const cx* cp = matrix_of(u, nn);
+#pragma unroll
+    for (int e = 0; e < 9; ++e) C[e] = __ldg(cp + (size_t)e * kBlock);
+  }
+  int cur = -1;
+#pragma unroll 1
+  for (; ui < last; ++ui) {
+    Use un = u;
+    int nn_next = nn;
+    cx Cn[9];
+    if (ui + 1 < last) {
+      un = c_uses.u[ui + 1];
+      if (un.term != u.term) nn_next = site_of_term(un.term);
+      const cx* cp = matrix_of(un, nn_next);
+#pragma unroll
+      for (int e = 0; e < 9; ++e) Cn[e] = __ldg(cp + (size_t)e * kBlock);
+    } else {
+#pragma unroll
+      for (int e = 0; e < 9; ++e) Cn[e] = C[e];
+    }
+    if (u.term != cur) {   // new stencil term: load its neighbour spinor
+      cur = u.term;
+      const vec* sp = psi + (size_t)(nn >> 5) * NC * kBlock + (nn & 31);
+      if constexpr (sizeof(real) == 4) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+          const float4 v = __ldg(sp + c * kBlock);
+          phi[2 * c] = cx{v.x, v.y};
+          phi[2 * c + 1] = cx{v.z, v.w};
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < 12; ++c) phi[c] = __ldg(sp + c * kBlock);
+      }
+      if (cur == 0 && wp == 0) {   // the mass term of W^0 (Eq. 2.6)
+        const real ms = (real)a.mass;
+#pragma unroll
+        for (int r = 0; r < 12; ++r) { acc[r].x += ms * phi[r].x; acc[r].y += ms * phi[r].y; }
+      }
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {   // input spin half: upper (spins 0, 1) or lower (2, 3)
+      cx tv[2][3];
+      if (u.adj) {                  // C^dag phi (warp-uniform branch: no per-element selects)
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+          for (int ca = 0; ca < 3; ++ca) {
+            real re = 0, im = 0;
+#pragma unroll
+            for (int cb = 0; cb < 3; ++cb) {
+              const cx w = C[3 * cb + ca], v = phi[3 * (2 * h + s) + cb];
+              re = fma(w.x, v.x, re); re = fma(w.y, v.y, re);
+              im = fma(w.x, v.y, im); im = fma(-w.y, v.x, im);
+            }
+            tv[s][ca] = cx{re, im};
+          }
+      } else {
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+          for (int ca = 0; ca < 3; ++ca) {
+            real re = 0, im = 0;
+#pragma unroll
+            for (int cb = 0; cb < 3; ++cb) {
+              const cx w = C[3 * ca + cb], v = phi[3 * (2 * h + s) + cb];
+              re = fma(w.x, v.x, re); re = fma(-w.y, v.y, re);
+              im = fma(w.x, v.y, im); im = fma(w.y, v.x, im);
+            }
+            tv[s][ca] = cx{re, im};
+          }
+      }
+#pragma unroll
+      for (int pi = 0; pi < 2; ++pi) {
+        if (pi >= u.np) break;
+        const Placement pl = u.pl[pi];
+        real c = (real)a.coef[pl.coef];
+        int th;   // output spin half
+        if (pl.kind == 0) {
+          if (!((pl.flags >> h) & 1)) continue;   // this diagonal block is absent
+          th = h;
+        } else {
+          th = 1 - h;
+          if (th == 1 && (pl.flags & 4)) c = -c;   // lower-left block = -S (W^0)
+        }
+        // out[al] += c sigma[al][be] tv[be]; sigma and th are warp-uniform runtime values: branch, no dynamic register indexing
+        if (th == 0) place<0>(acc, tv, pl.sigma, c);
+        else place<6>(acc, tv, pl.sigma, c);
+      }
+    }
+    u = un;
+    nn = nn_next;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) C[e] = Cn[e];
+  }
+
+  // fixed-order sum of the four warps' partial results, then the store (and the fused BiCGStab reductions)
+  __shared__ cx red[kPauliWarps][12][kBlock];
+#pragma unroll
+  for (int r = 0; r < 12; ++r) red[wp][r][lane] = acc[r];
+  __syncthreads();
+  if (wp != 0) return;
+  cx o[12];
+#pragma unroll
+  for (int r = 0; r < 12; ++r) {
+    cx s = red[0][r][lane];
+#pragma unroll
+    for (int w = 1; w < kPauliWarps; ++w) { s.x += red[w][r][lane].x; s.y += red[w][r][lane].y; }
+    if (!live) s = cx{0, 0};
+    o[r] = s;
+  }
+  vec* ob = out + (size_t)blk * NC * kBlock + lane;
+  if constexpr (sizeof(real) == 4) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) ob[c * kBlock] = make_float4(o[2 * c].x, o[2 * c].y, o[2 * c + 1].x, o[2 * c + 1].y);
+  } else {
+#pragma unroll
+    for (int c = 0; c < 12; ++c) ob[c * kBlock] = o[c];
+  }
+  if constexpr (DOT) {
+    const vec* ab = dot_a + (size_t)blk * NC * kBlock + lane;
+    double d0 = 0.0, d1 = 0.0, d2 = 0.0;
+#pragma unroll
+    for (int r = 0; r < 12; ++r) {
+      double ar, ai;
+      if constexpr (sizeof(real) == 4) {
+        const float4 v = ab[(r >> 1) * kBlock];
+        ar = (r & 1) ? v.z : v.x;
+        ai = (r & 1) ? v.w : v.y;
+      } else {
+        const double2 v = ab[r * kBlock];
+        ar = v.x; ai = v.y;
+      }
+      const double vr = (double)o[r].x, vi = (double)o[r].y;
+      d0 += ar * vr + ai * vi;
+      d1 += ar * vi - ai * vr;
+      d2 += vr * vr + vi * vi;
+    }
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) {
+      d0 += __shfl_xor_sync(0xffffffffu, d0, m);
+      d1 += __shfl_xor_sync(0xffffffffu, d1, m);
+      d2 += __shfl_xor_sync(0xffffffffu, d2, m);
+    }
+    if (lane == 0) {
+      partials[(size_t)blk * 3 + 0] = d0;
+      partials[(size_t)blk * 3 + 1] = d1;
+      partials[(size_t)blk * 3 + 2] = d2;
+    }
+  }
+}
+
+// OK_W_PAULI -> canonical W[n][27][12][12] (ok_unpack_W): the same table, the placements written out as matrix entries
+template <typename real>
+__global__ void __launch_bounds__(128) unpack_pauli_kernel(const typename PV<real>::cx* __restrict__ W, typename PV<real>::cx* __restrict__ canon,
+                                                           PauliArgs a) {
+  using cx = typename PV<real>::cx;
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= (long long)a.g.V * kTerms) return;
+  const int n = (int)(id / kTerms), term = (int)(id % kTerms);
+  cx M[144];
+  for (int e = 0; e < 144; ++e) M[e] = cx{0, 0};
+  if (term == 0)
+    for (int r = 0; r < 12; ++r) M[13 * r].x = (real)a.mass;
+  int q = n / a.g.L[0];
+  const int x = n % a.g.L[0], y = q % a.g.L[1];
+  q /= a.g.L[1];
+  const int z = q % a.g.L[2], t = q / a.g.L[2];
+  for (int ui = 0; ui < c_uses.n; ++ui) {
+    const Use u = c_uses.u[ui];
+    if (u.term != term) continue;
+    int nm = n;
+    if (u.adj) {
+      const int xx = wrapp(x + c_poff2[term][0], a.g.L[0]), yy = wrapp(y + c_poff2[term][1], a.g.L[1]);
+      const int zz = wrapp(z + c_poff2[term][2], a.g.L[2]), tt = wrapp(t + c_poff2[term][3], a.g.L[3]);
+      nm = xx + a.g.L[0] * (yy + a.g.L[1] * (zz + a.g.L[2] * tt));
+    }
+    const cx* cp = W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31) + (size_t)(9 * u.m) * kBlock;
+    cx C[9];
+    for (int ca = 0; ca < 3; ++ca)
+      for (int cb = 0; cb < 3; ++cb) {
+        cx v = cp[(size_t)(u.adj ? 3 * cb + ca : 3 * ca + cb) * kBlock];
+        if (u.adj) v.y = -v.y;
+        C[3 * ca + cb] = v;
+      }
+    for (int pi = 0; pi < u.np; ++pi) {
+      const Placement pl = u.pl[pi];
+      for (int th = 0; th < 2; ++th) {        // output spin half
+        const int h = pl.kind == 0 ? th : 1 - th;   // input spin half
+        real c = (real)a.coef[pl.coef];
+        if (pl.kind == 0 && !((pl.flags >> h) & 1)) continue;
+        if (pl.kind == 1 && th == 1 && (pl.flags & 4)) c = -c;
+        const bool swap = pl.sigma == 1 || pl.sigma == 2;
+        for (int al = 0; al < 2; ++al) {
+          const int be = swap ? 1 - al : al;
+          for (int ca = 0; ca < 3; ++ca)
+            for (int cb = 0; cb < 3; ++cb) {
+              const cx f = pauli_factor<cx, real>(C[3 * ca + cb], pl.sigma, al, c);
+              cx& d = M[(6 * th + 3 * al + ca) * 12 + 6 * h + 3 * be + cb];
+              d.x += f.x; d.y += f.y;
+            }
+        }
+      }
+    }
+  }
+  cx* dst = canon + (size_t)id * 144;
+  for (int e = 0; e < 144; ++e) dst[e] = M[e];
+}
+
+int pauli_init() {
+  if (g_pauli_ready) return OK_SUCCESS;
+  build_uses(h_uses);
+  OK_CUDA(cudaMemcpyToSymbol(c_uses, &h_uses, sizeof(UseTable)));
+  OK_CUDA(cudaMemcpyToSymbol(c_poff2, kOffsets, sizeof(kOffsets)));
+  g_pauli_ready = true;
+  return OK_SUCCESS;
+}
+
+PauliArgs make_args(const ok_params* p) {
+  PauliArgs a;
+  a.g = make_geom(p);
+  const double u0 = p->u0;
+  const double a1 = 0.5 * (p->zeta - 2.0 * p->c1 - 12.0 * p->c2), d1 = -0.5 * (p->rs * p->zeta + 8.0 * p->c4);
+  const double dii = p->c4 / u0, sii = (p->c1 + 2.0 * p->c2) / (2.0 * u0), sij = p->c2 / (2.0 * u0);
+  a.coef[C_ONE] = 1.0; a.coef[C_MINUS] = -1.0;
+  a.coef[C_D1] = d1; a.coef[C_A1] = a1; a.coef[C_MA1] = -a1;
+  a.coef[C_DII] = dii; a.coef[C_SII] = sii; a.coef[C_MSII] = -sii;
+  a.coef[C_SIJ] = sij; a.coef[C_MSIJ] = -sij;
+  a.mass = u0 / (2.0 * p->kappa);
+  return a;
+}
+
+template <typename real>
+int launch_pauli(const ok_params* p, const void* W, const void* psi, void* out, double* partials, const void* dot_a) {
+  using cx = typename PV<real>::cx;
+  using vec = typename PV<real>::vec;
+  const PauliArgs a = make_args(p);
+  if (partials)
+    apply_pauli_kernel<real, true><<<a.g.nblk, 32 * kPauliWarps, 0, ctx().stream>>>(static_cast<const cx*>(W), static_cast<const vec*>(psi),
+                                                                                   static_cast<vec*>(out), a, static_cast<const vec*>(dot_a), partials);
+  else
+    apply_pauli_kernel<real, false><<<a.g.nblk, 32 * kPauliWarps, 0, ctx().stream>>>(static_cast<const cx*>(W), static_cast<const vec*>(psi),
+                                                                                    static_cast<vec*>(out), a, nullptr, nullptr);
+  OK_LAUNCHED("apply_pauli_kernel");
+  return OK_SUCCESS;
+}
+
+}  // namespace
+
+int launch_apply_pauli(const ok_params* p, const void* W, const void* psi, void* out, double* partials, const void* dot_a) {
+  if (p->nrhs != 1 || p->storage != OK_W_PAULI) return OK_EINVAL;
+  if (int st = pauli_init()) return st;
+  return p->precision == OK_FP64 ? launch_pauli<double>(p, W, psi, out, partials, dot_a) : launch_pauli<float>(p, W, psi, out, partials, dot_a);
+}
+
+int launch_unpack_pauli(const ok_params* p, const void* W, void* canon) {
+  if (int st = pauli_init()) return st;
+  const PauliArgs a = make_args(p);
+  const long long total = (long long)a.g.V * kTerms;
+  const unsigned grid = (unsigned)((total + 127) / 128);
+  if (p->precision == OK_FP64)
+    unpack_pauli_kernel<double><<<grid, 128, 0, ctx().stream>>>(static_cast<const double2*>(W), static_cast<double2*>(canon), a);
+  else
+    unpack_pauli_kernel<float><<<grid, 128, 0, ctx().stream>>>(static_cast<const float2*>(W), static_cast<float2*>(canon), a);
+  OK_LAUNCHED("unpack_pauli_kernel");
+  return OK_SUCCESS;
+}
+
+}  // namespace okd

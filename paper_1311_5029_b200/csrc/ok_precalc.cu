@@ -639,6 +639,57 @@ __global__ void __launch_bounds__(32 * 3) pauli_terms_kernel(const double2* __re
 // same K with the sign of S flipped, P -> P^dag.  One thread per (site, term) writes its own site only (coalesced, sector
 // aligned), one rolled loop over the spin row keeps the code small: the templated assembly path spends most of its time waiting
 // for instructions (profiles/r02_precalc.md).  fp64 throughout, rounded once.
+// the colour matrix of a two-link term at site x: fam 3 P_ii, fam 4 P_ij, fam 5 P_i-j (see above)
+__device__ __forceinline__ cm3 two_link_P(const double2* __restrict__ links, const Site& x, int fam, int i, int j, const PrecalcArgs& a) {
+  cm3 P;
+  if (fam == 3) {
+    P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), i, a));
+  } else if (fam == 4) {
+    P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), j, a));
+    axpy(P, 1.0, 0.0, mul(ldU(links, x, j, a), ldU(links, shift(x, j, 1, a.g), i, a)));
+  } else {
+    const Site xmj = shift(x, j, -1, a.g);
+    P = mul_nd(ldU(links, x, i, a), ldU(links, shift(xmj, i, 1, a.g), j, a));
+    axpy(P, 1.0, 0.0, mul_dn(ldU(links, xmj, j, a), ldU(links, xmj, i, a)));
+  }
+  return P;
+}
+
+// OK_W_PAULI (ok_pauli.cu has the list of the 37 stored matrices): thread = (site, matrix); everything but the two-link
+// products is a scaled copy of a scratch field or a link
+template <typename real>
+__global__ void __launch_bounds__(32 * 4) pauli_store_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                                             typename WUnit<real>::cx* __restrict__ W, PrecalcArgs a) {
+  using cx = typename WUnit<real>::cx;
+  const int lane = threadIdx.x, m = blockIdx.y * 4 + threadIdx.y;
+  if (m >= OK_W_PAULI_MATS) return;
+  const int blk = blockIdx.x, n = (blk + a.blk0) * kBlock + lane;
+  cx* dst = W + ((size_t)blk * (OK_W_PAULI_MATS * 9) + 9 * m) * kBlock + lane;
+  cm3 C = zero3();
+  if (n < a.g.V) {
+    const Site x = site_of(n, a.g);
+    if (m < 3) axpy(C, 0.0, a.d0, ldF(FS, m, x, a));
+    else if (m < 6) axpy(C, a.s0, 0.0, ldF(FS, m, x, a));
+    else if (m == 6) C = ldU(links, x, 3, a);
+    else if (m < 10) C = ldF(FS, 6 + 15 + (m - 7), x, a);
+    else if (m < 28) {
+      const int i = (m - 10) / 6, r = (m - 10) % 6;
+      C = r == 0 ? ldU(links, x, i, a) : ldF(FS, 6 + 5 * i + (r - 1), x, a);
+    } else if (m < 31) C = two_link_P(links, x, 3, m - 28, 0, a);
+    else {
+      const int q = (m - 31) >> 1;
+      C = two_link_P(links, x, ((m - 31) & 1) ? 5 : 4, q == 2 ? 1 : 0, q == 0 ? 1 : 2, a);
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < 9; ++e) {
+    cx v;
+    v.x = (real)C.e[e].x;
+    v.y = (real)C.e[e].y;
+    dst[(size_t)e * kBlock] = v;
+  }
+}
+
 template <typename real>
 __global__ void __launch_bounds__(32 * 3) kron_terms_kernel(const double2* __restrict__ links, typename WUnit<real>::type* __restrict__ W,
                                                             PrecalcArgs a) {
@@ -669,17 +720,7 @@ __global__ void __launch_bounds__(32 * 3) kron_terms_kernel(const double2* __res
   Site x = site_of(n, a.g);
   if (neg)   // the positive blocks live at x + offset(term)
     for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
-  cm3 P;
-  if (fam == 3) {
-    P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), i, a));
-  } else if (fam == 4) {
-    P = mul(ldU(links, x, i, a), ldU(links, shift(x, i, 1, a.g), j, a));
-    axpy(P, 1.0, 0.0, mul(ldU(links, x, j, a), ldU(links, shift(x, j, 1, a.g), i, a)));
-  } else {
-    const Site xmj = shift(x, j, -1, a.g);
-    P = mul_nd(ldU(links, x, i, a), ldU(links, shift(xmj, i, 1, a.g), j, a));
-    axpy(P, 1.0, 0.0, mul_dn(ldU(links, xmj, j, a), ldU(links, xmj, i, a)));
-  }
+  cm3 P = two_link_P(links, x, fam, i, j, a);
   if (neg) P = adj(P);
   // spin structure: D = kD 1 ; S = s1 sigma_1 + s2 sigma_2 + s3 sigma_3 (real coefficients)
   const double kD = fam == 3 ? a.dii : 0.0;
@@ -883,6 +924,13 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
   }
   const int nb = win_nblk < 0 ? a.g.nblk : win_nblk;
   a.blk0 = win_nblk < 0 ? 0 : win_blk0;
+  if (p->storage == OK_W_PAULI) {
+    const dim3 pgrid(nb, (OK_W_PAULI_MATS + 3) / 4), pblock(32, 4);
+    if (p->precision == OK_FP64) pauli_store_kernel<double><<<pgrid, pblock, 0, st>>>(lk, FS, static_cast<double2*>(Wp), a);
+    else pauli_store_kernel<float><<<pgrid, pblock, 0, st>>>(lk, FS, static_cast<float2*>(Wp), a);
+    OK_LAUNCHED("pauli_store_kernel");
+    return OK_SUCCESS;
+  }
   if (p->storage == OK_W_DENSE) {
     OK_PAULI_LAUNCH(nb, Wp);
     OK_KRON_LAUNCH(nb, Wp);

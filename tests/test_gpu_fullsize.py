@@ -153,7 +153,7 @@ def test_fullsize_12rhs_apply_and_solve(big):
     assert np.all(est <= bound), (est, bound)
 
 
-@pytest.mark.parametrize("fmt", [B.OK_W_DS, B.OK_W_CONJ])
+@pytest.mark.parametrize("fmt", [B.OK_W_DS, B.OK_W_CONJ, B.OK_W_PAULI])
 def test_fullsize_reduced_formats_apply_and_mixed_solve(big, fmt):
     """The reduced W storage formats and the mixed-precision inversion (item 3) at the
     bench size: sampled-site parity of the fp32 apply, then ok_bicgstab_mixed(W64, W32) to 1e-10 with the residual
