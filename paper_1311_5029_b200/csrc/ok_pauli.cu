@@ -30,14 +30,15 @@ constexpr int kPauliMats = OK_W_PAULI_MATS;   // 37
 constexpr int kMaxUses = 80;
 enum Coef { C_ONE = 0, C_MINUS, C_D1, C_A1, C_MA1, C_DII, C_SII, C_MSII, C_SIJ, C_MSIJ, C_COUNT };
 
+// (plain ints: the kernel reads the table from constant memory every iteration, byte fields cost a PRMT each)
 struct Placement {
-  int8_t kind;    // 0: D (diagonal spin blocks), 1: S (off-diagonal)
-  int8_t sigma;   // 0 = 1, 1..3 = sigma_x, sigma_y, sigma_z
-  int8_t coef;    // Coef
-  int8_t flags;   // D: bit 0 = upper-left block present, bit 1 = lower-right ; S: bit 2 = the lower-left block carries a minus
+  int kind;    // 0: D (diagonal spin blocks), 1: S (off-diagonal), -1: none
+  int sigma;   // 0 = 1, 1..3 = sigma_x, sigma_y, sigma_z
+  int coef;    // Coef
+  int flags;   // D: bit 0 = upper-left block present, bit 1 = lower-right ; S: bit 2 = the lower-left block carries a minus
 };
 struct Use {
-  int8_t m, term, adj, np;
+  int m, term, adj, np;
   Placement pl[2];
 };
 struct UseTable {
@@ -51,14 +52,14 @@ __constant__ int8_t c_poff2[kTerms][4];
 static bool g_pauli_ready = false;
 static UseTable h_uses;
 
-Placement Dp(int sigma, int coef, int ul = 1, int lr = 1) { return Placement{0, (int8_t)sigma, (int8_t)coef, (int8_t)(ul | (lr << 1))}; }
-Placement Sp(int sigma, int coef, int llneg = 0) { return Placement{1, (int8_t)sigma, (int8_t)coef, (int8_t)(llneg << 2)}; }
+Placement Dp(int sigma, int coef, int ul = 1, int lr = 1) { return Placement{0, sigma, coef, ul | (lr << 1)}; }
+Placement Sp(int sigma, int coef, int llneg = 0) { return Placement{1, sigma, coef, llneg << 2}; }
 
 void add_use(UseTable& t, int m, int term, int adj, Placement a, const Placement* b = nullptr) {
   Use& u = t.u[t.n++];
-  u.m = (int8_t)m; u.term = (int8_t)term; u.adj = (int8_t)adj; u.np = b ? 2 : 1;
+  u.m = m; u.term = term; u.adj = adj; u.np = b ? 2 : 1;
   u.pl[0] = a;
-  u.pl[1] = b ? *b : Placement{0, 0, 0, 0};
+  u.pl[1] = b ? *b : Placement{-1, 0, 0, 0};
 }
 
 // The 68 uses, term by term, from Eqs. (2.6)-(2.12) and the conjugation relations (2.3), (2.10):
@@ -130,6 +131,11 @@ struct PauliArgs {
   double coef[C_COUNT];
   double mass;
 };
+__constant__ float c_coef32[C_COUNT];
+__constant__ double c_coef64[C_COUNT];
+template <typename real> __device__ __forceinline__ real coef_of(int id);
+template <> __device__ __forceinline__ float coef_of<float>(int id) { return c_coef32[id]; }
+template <> __device__ __forceinline__ double coef_of<double>(int id) { return c_coef64[id]; }
 
 __device__ __forceinline__ int wrapp(int x, int L) {
   x += (x < 0) ? L : 0;
@@ -297,20 +303,18 @@ apply_pauli_kernel(const typename PV<real>::cx* __restrict__ W, const typename P
       }
 #pragma unroll
       for (int pi = 0; pi < 2; ++pi) {
-        if (pi >= u.np) break;
         const Placement pl = u.pl[pi];
-        real c = (real)a.coef[pl.coef];
-        int th;   // output spin half
-        if (pl.kind == 0) {
-          if (!((pl.flags >> h) & 1)) continue;   // this diagonal block is absent
-          th = h;
-        } else {
-          th = 1 - h;
-          if (th == 1 && (pl.flags & 4)) c = -c;   // lower-left block = -S (W^0)
-        }
+        real c = coef_of<real>(pl.coef);
+        // D: output half = input half, if that diagonal block is present; S: the other half, the lower-left block of W^0 negated
+        const bool isD = pl.kind == 0;
+        const bool on = isD ? ((pl.flags >> h) & 1) != 0 : pl.kind == 1;
+        const int th = isD ? h : 1 - h;
+        if (!isD && th == 1 && (pl.flags & 4)) c = -c;
         // out[al] += c sigma[al][be] tv[be]; sigma and th are warp-uniform runtime values: branch, no dynamic register indexing
-        if (th == 0) place<0>(acc, tv, pl.sigma, c);
-        else place<6>(acc, tv, pl.sigma, c);
+        if (on) {
+          if (th == 0) place<0>(acc, tv, pl.sigma, c);
+          else place<6>(acc, tv, pl.sigma, c);
+        }
       }
     }
     u = un;
@@ -460,6 +464,17 @@ int launch_pauli(const ok_params* p, const void* W, const void* psi, void* out, 
   using cx = typename PV<real>::cx;
   using vec = typename PV<real>::vec;
   const PauliArgs a = make_args(p);
+  static double last[C_COUNT + 1];   // the constants of the action of the last launch (one device, one thread per process: ok.h)
+  static bool have = false;
+  bool same = have;
+  for (int k = 0; k < C_COUNT && same; ++k) same = last[k] == a.coef[k];
+  if (!same) {
+    float c32[C_COUNT];
+    for (int k = 0; k < C_COUNT; ++k) { c32[k] = (float)a.coef[k]; last[k] = a.coef[k]; }
+    OK_CUDA(cudaMemcpyToSymbolAsync(c_coef32, c32, sizeof(c32), 0, cudaMemcpyHostToDevice, ctx().stream));
+    OK_CUDA(cudaMemcpyToSymbolAsync(c_coef64, a.coef, sizeof(a.coef), 0, cudaMemcpyHostToDevice, ctx().stream));
+    have = true;
+  }
   if (partials)
     apply_pauli_kernel<real, true><<<a.g.nblk, 32 * kPauliWarps, 0, ctx().stream>>>(static_cast<const cx*>(W), static_cast<const vec*>(psi),
                                                                                    static_cast<vec*>(out), a, static_cast<const vec*>(dot_a), partials);
