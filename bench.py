@@ -143,6 +143,7 @@ class ClockSampler:
 # all-core leg only runs Oracle.apply_W on disjoint site ranges in forked worker processes (the sum over the 27 terms of a
 # site never crosses a range) -- no change to the oracle's arithmetic.
 _CPU = {}      # worker globals, inherited by fork
+_ORACLE_SETUP = {}
 
 
 def _cpu_worker(a, b, reps):
@@ -159,16 +160,19 @@ def oracle_sample(dims, eps, lseed, sseed, kappa, budget_s=10.0, nsample=4096, U
     from oracle.ok_oracle import Oracle   # test infrastructure; allowed here for the CPU baseline only
     if U is None:
         U = make_links(dims, eps, lseed)
-    u0 = I.tadpole_u0(I.mean_plaquette(dims, U))
-    o = Oracle(U, I.make_params(dims, kappa, u0))
-    # the apply's cost is data-independent: Gaussian columns stand in for the point sources of the 12-RHS config
-    cols = [I.gaussian_spinor(dims, (sseed if sseed is not None else 6) + j) for j in range(nrhs)]
+    key = (tuple(dims), id(U), kappa, nrhs, nsample, workers)
+    if key not in _ORACLE_SETUP:     # the oracle object, the source columns and the sample's stored W are set up once per run
+        u0 = I.tadpole_u0(I.mean_plaquette(dims, U))
+        o = Oracle(U, I.make_params(dims, kappa, u0))
+        # the apply's cost is data-independent: Gaussian columns stand in for the point sources of the 12-RHS config
+        cols = [I.gaussian_spinor(dims, (sseed if sseed is not None else 6) + j) for j in range(nrhs)]
+        ns = min(nsample * workers, o.V)
+        idx = (np.arange(ns) * (o.V // ns)).astype(np.int64)      # evenly spread sites
+        t0 = time.perf_counter()
+        W = o.precalc_W(idx)
+        _ORACLE_SETUP[key] = (o, cols, ns, idx, W, time.perf_counter() - t0)
+    o, cols, nsample, idx, W, t_pre = _ORACLE_SETUP[key]
     V = o.V
-    nsample = min(nsample * workers, V)
-    idx = (np.arange(nsample) * (V // nsample)).astype(np.int64)      # evenly spread sites
-    t0 = time.perf_counter()
-    W = o.precalc_W(idx)
-    t_pre = time.perf_counter() - t0
     reps = 0
     if workers == 1:
         c0, w0 = time.process_time(), time.perf_counter()
