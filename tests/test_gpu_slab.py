@@ -124,6 +124,24 @@ def test_slab_apply_periodic_time_and_error_paths():
         B.ok_slab_dirac_apply(Wfull, vecs[0], outs[0])
     bad = B.make_slab_params(B.make_params(dict(pd, dims=(3, 3, 3, 8)), B.OK_FP64), 4)       # 27 sites per slice
     assert B.ok_slab_vec_bytes(bad) == 0
+    # the link window must fit the lattice once (Tloc + 4 <= T), t0 must be a slice of it, the workspace must be there
+    Wt = B.alloc_W(sl.slab, G.DEV)
+    lk = G.to_dev(S.link_window(U, dims, 0, 4), torch.complex128)
+    for T_global, t0 in ((7, 0), (8, -1), (8, 8)):
+        with pytest.raises(B.OkError) as e:
+            B.ok_slab_precalc_W(lk, sl.slab, T_global, t0, Wt)
+        assert e.value.status == -1
+    B.ok_set_workspace(None, 0)
+    with pytest.raises(B.OkError) as e:
+        B.ok_slab_precalc_W(lk, sl.slab, 8, 0, Wt)
+    assert e.value.status == -5
+    # slabs of different precision cannot be solved together
+    p32 = B.make_params(pd, B.OK_FP32)
+    sl32 = Slabs(U, pd, B.OK_FP32, 2)
+    v64, v32 = sl.scatter(psi), sl32.scatter(psi)
+    st, _, _ = B.ok_slab_bicgstab([sl.W[0], sl32.W[1]], [v64[0], v32[1]], [torch.zeros_like(v64[0]), torch.zeros_like(v32[1])], 1e-8, 10,
+                                  raise_on_fail=False)
+    assert st == -1
     B.ok_set_workspace(None)
 
 

@@ -62,3 +62,25 @@ def test_layout_reconstructs_the_oracle_W(oracle_W, fmt):
         v = rec[src, u]
         back[:, t, r, c] = sign * (np.conj(v) if conj else v)
     assert np.array_equal(back, W)
+
+
+def test_slab_and_pauli_sizes_are_pure_host_arithmetic():
+    """ok_slab_* sizes (t-slab decomposition, include/ok.h) and the OK_W_PAULI footprint need no device."""
+    from paper_1311_5029_b200 import inputs as I
+    dims = (20, 20, 20, 64)
+    pd = I.make_params(dims, 0.10, 0.95)
+    for prec, rb in ((B.OK_FP32, 4), (B.OK_FP64, 8)):
+        p = B.make_params(pd, prec)
+        sp = B.make_slab_params(p, 16)
+        assert sp.reserved_ == B.OK_SLAB and list(sp.dims) == [20, 20, 20, 16]
+        slice_bytes = 20 * 20 * 20 * 12 * 2 * rb
+        assert B.ok_slab_slice_bytes(sp) == slice_bytes                      # 768 000 B at 20^3 fp32: one halo message
+        assert B.ok_slab_vec_bytes(sp) == 18 * slice_bytes
+        assert B.ok_W_bytes(sp) == 1024 + 20 * 20 * 20 * 16 * 27 * 144 * 2 * rb
+        assert B.ok_slab_work_bytes(sp, 4, 2) > 4 * 6 * 18 * slice_bytes
+        # not a slab (reserved_ = 0), or a time slice that is not a whole number of 32-site blocks: refused
+        assert B.ok_slab_vec_bytes(p) == 0
+        assert B.ok_slab_vec_bytes(B.make_slab_params(B.make_params(I.make_params((3, 3, 3, 8), 0.1, 0.95), prec), 4)) == 0
+        q = B.make_params(pd, prec, storage=B.OK_W_PAULI)
+        assert B.ok_W_bytes(q) == 1024 + 20 * 20 * 20 * 64 * 37 * 9 * 2 * rb   # 2 664 B per site in fp32 (PAPER.md:72: "50 color blocks")
+    assert B.ok_W_unit_index(B.OK_W_PAULI, 0, 0, 0)[0] == -2          # no element-wise layout query for this format (ok.h)
