@@ -18,8 +18,9 @@
 // Apply: out(x) = mass psi(x) + sum over 68 "uses" of a stored matrix: (matrix m at the neighbour site of stencil term t, or its
 // adjoint for an opposite-direction term, Eqs. 2.3/2.10) times the four colour vectors of psi(x + offset_t), placed into the
 // output by one or two Pauli placements  coef * sigma_k  in the diagonal (D) or off-diagonal (S) spin blocks.  The uses are a
-// constant table built on the host from the equations (build_uses below); the kernel is one rolled loop over it.
-// 21 kflop per 2 856 B per site: this format is bound by the fp32 pipes, not by HBM.
+// constexpr table written straight from the equations (make_uses below); the apply kernels are specialised on every entry
+// at compile time (no table reads, no runtime flags, constant offsets), ok_unpack_W walks the same table at run time.
+// 19.6 kflop per 2 856 B per site: this format is bound by the fp32 pipes, not by HBM.
 #include "ok_internal.cuh"
 
 namespace okd {
@@ -28,6 +29,10 @@ namespace {
 
 constexpr int kPauliMats = OK_W_PAULI_MATS;   // 37
 constexpr int kMaxUses = 80;
+#ifndef OK_PAULI_PARTS
+#define OK_PAULI_PARTS 2
+#endif
+constexpr int kPauliParts = OK_PAULI_PARTS;   // launches per apply (see apply_pauli_part_kernel)
 enum Coef { C_ONE = 0, C_MINUS, C_D1, C_A1, C_MA1, C_DII, C_SII, C_MSII, C_SIJ, C_MSIJ, C_COUNT };
 
 // (plain ints: the kernel reads the table from constant memory every iteration, byte fields cost a PRMT each)
@@ -43,33 +48,34 @@ struct Use {
 };
 struct UseTable {
   int n;
-  int first[5];   // warp w of a CTA handles uses first[w] .. first[w+1]-1 (whole terms, so the neighbour spinor is loaded once per term)
+  int first[kPauliParts + 1];   // part q (one launch) handles uses first[q] .. first[q+1]-1: whole terms, so the neighbour spinor is loaded once per term
   Use u[kMaxUses];
 };
 
 __constant__ UseTable c_uses;
 __constant__ int8_t c_poff2[kTerms][4];
 static bool g_pauli_ready = false;
-static UseTable h_uses;
 
-Placement Dp(int sigma, int coef, int ul = 1, int lr = 1) { return Placement{0, sigma, coef, ul | (lr << 1)}; }
-Placement Sp(int sigma, int coef, int llneg = 0) { return Placement{1, sigma, coef, llneg << 2}; }
+constexpr Placement Dp(int sigma, int coef, int ul = 1, int lr = 1) { return Placement{0, sigma, coef, ul | (lr << 1)}; }
+constexpr Placement Sp(int sigma, int coef, int llneg = 0) { return Placement{1, sigma, coef, llneg << 2}; }
+constexpr Placement kNoPlacement{-1, 0, 0, 0};
 
-void add_use(UseTable& t, int m, int term, int adj, Placement a, const Placement* b = nullptr) {
+constexpr void add_use(UseTable& t, int m, int term, int adj, Placement a, Placement b = kNoPlacement) {
   Use& u = t.u[t.n++];
-  u.m = m; u.term = term; u.adj = adj; u.np = b ? 2 : 1;
+  u.m = m; u.term = term; u.adj = adj; u.np = b.kind >= 0 ? 2 : 1;
   u.pl[0] = a;
-  u.pl[1] = b ? *b : Placement{-1, 0, 0, 0};
+  u.pl[1] = b;
 }
 
 // The 68 uses, term by term, from Eqs. (2.6)-(2.12) and the conjugation relations (2.3), (2.10):
 // the opposite-direction matrix is [[D^dag, -S^dag], [-S^dag, D^dag]] of the blocks at the neighbour site.
-void build_uses(UseTable& t) {
+// constexpr: the apply kernel is specialised on every entry at compile time; ok_unpack_W reads the same table at run time.
+constexpr UseTable make_uses() {
+  UseTable t{};
   t.n = 0;
-  int start_of_term[kTerms + 1];
-  auto begin = [&](int term) { start_of_term[term] = t.n; };
+  int start_of_term[kTerms + 1] = {};
   // term 0: W^0 = [[D0, S0], [-S0, D0]] + mass
-  begin(0);
+  start_of_term[0] = t.n;
   for (int m = 0; m < 3; ++m) add_use(t, m, 0, 0, Dp(m + 1, C_ONE));
   for (int m = 0; m < 3; ++m) add_use(t, 3 + m, 0, 0, Sp(m + 1, C_ONE, 1));
   // terms 1..6: one-link hops +-i
@@ -77,9 +83,8 @@ void build_uses(UseTable& t) {
     const int b = 10 + 6 * i, k = (i + 1) % 3, l = (i + 2) % 3;
     for (int neg = 0; neg < 2; ++neg) {
       const int term = 1 + 2 * i + neg;
-      begin(term);
-      const Placement su = Sp(i + 1, neg ? C_MA1 : C_A1);
-      add_use(t, b, term, neg, Dp(0, C_D1), &su);
+      start_of_term[term] = t.n;
+      add_use(t, b, term, neg, Dp(0, C_D1), Sp(i + 1, neg ? C_MA1 : C_A1));
       add_use(t, b + 1, term, neg, Sp(0, neg ? C_MINUS : C_ONE));
       add_use(t, b + 2, term, neg, Sp(k + 1, neg ? C_MINUS : C_ONE));
       add_use(t, b + 3, term, neg, Sp(l + 1, neg ? C_MINUS : C_ONE));
@@ -89,38 +94,48 @@ void build_uses(UseTable& t) {
   }
   // terms 7, 8: temporal hop; D = -U_4 sits in the lower-right block for +t and in the upper-left one for -t
   for (int neg = 0; neg < 2; ++neg) {
-    begin(7 + neg);
+    start_of_term[7 + neg] = t.n;
     add_use(t, 6, 7 + neg, neg, Dp(0, C_MINUS, neg ? 1 : 0, neg ? 0 : 1));
     for (int m = 0; m < 3; ++m) add_use(t, 7 + m, 7 + neg, neg, Sp(m + 1, neg ? C_MINUS : C_ONE));
   }
   // terms 9..14: +-2i
   for (int i = 0; i < 3; ++i)
     for (int neg = 0; neg < 2; ++neg) {
-      begin(9 + 2 * i + neg);
-      const Placement s = Sp(i + 1, neg ? C_MSII : C_SII);
-      add_use(t, 28 + i, 9 + 2 * i + neg, neg, Dp(0, C_DII), &s);
+      start_of_term[9 + 2 * i + neg] = t.n;
+      add_use(t, 28 + i, 9 + 2 * i + neg, neg, Dp(0, C_DII), Sp(i + 1, neg ? C_MSII : C_SII));
     }
   // terms 15..26: pairs (x,y), (x,z), (y,z): +i+j, -i-j, +i-j, -i+j
   for (int q = 0; q < 3; ++q) {
     const int i = q == 2 ? 1 : 0, j = q == 0 ? 1 : 2;
     for (int w = 0; w < 4; ++w) {
-      const int term = 15 + 4 * q + w, neg = w & 1, minus = w >= 2;
-      begin(term);
+      const int term = 15 + 4 * q + w, neg = w & 1, minus = w >= 2 ? 1 : 0;
+      start_of_term[term] = t.n;
       const int ci = neg ? C_MSIJ : C_SIJ, cj = (neg != minus) ? C_MSIJ : C_SIJ;
-      const Placement sj = Sp(j + 1, cj);
-      add_use(t, 31 + 2 * q + (minus ? 1 : 0), term, neg, Sp(i + 1, ci), &sj);
+      add_use(t, 31 + 2 * q + minus, term, neg, Sp(i + 1, ci), Sp(j + 1, cj));
     }
   }
   start_of_term[kTerms] = t.n;
-  // four warps, whole terms each, as even as the term boundaries allow
+  // the parts: whole terms each, as even as the term boundaries allow
   t.first[0] = 0;
-  t.first[4] = t.n;
+  t.first[kPauliParts] = t.n;
   int term = 0;
-  for (int w = 1; w < 4; ++w) {
-    while (term < kTerms && start_of_term[term] < (t.n * w + 2) / 4) ++term;
+  for (int w = 1; w < kPauliParts; ++w) {
+    while (term < kTerms && start_of_term[term] < (t.n * w + kPauliParts / 2) / kPauliParts) ++term;
     t.first[w] = start_of_term[term];
   }
+  return t;
 }
+constexpr UseTable kUses = make_uses();
+static_assert(kUses.n == 68, "68 matrix uses per site");
+// stencil offsets, term order of ok.h (compile-time copy of kOffsets; pauli_init checks the two agree)
+constexpr int kOffC[kTerms][4] = {
+    {0, 0, 0, 0},
+    {1, 0, 0, 0},  {-1, 0, 0, 0}, {0, 1, 0, 0},  {0, -1, 0, 0}, {0, 0, 1, 0},  {0, 0, -1, 0},
+    {0, 0, 0, 1},  {0, 0, 0, -1},
+    {2, 0, 0, 0},  {-2, 0, 0, 0}, {0, 2, 0, 0},  {0, -2, 0, 0}, {0, 0, 2, 0},  {0, 0, -2, 0},
+    {1, 1, 0, 0},  {-1, -1, 0, 0}, {1, -1, 0, 0}, {-1, 1, 0, 0},
+    {1, 0, 1, 0},  {-1, 0, -1, 0}, {1, 0, -1, 0}, {-1, 0, 1, 0},
+    {0, 1, 1, 0},  {0, -1, -1, 0}, {0, 1, -1, 0}, {0, -1, 1, 0}};
 
 template <typename real> struct PV;
 template <> struct PV<float> { using cx = float2; using vec = float4; static constexpr int NC = 6; };
@@ -151,31 +166,36 @@ __device__ __forceinline__ cx pauli_factor(cx v, int sigma, int al, real c) {
   return cx{c * v.x, c * v.y};
 }
 
-constexpr int kPauliWarps = 4;
+// ---- the apply, specialised at compile time on every entry of kUses (no table reads, no runtime flags, constant offsets)
+template <typename real>
+struct PState {
+  using cx = typename PV<real>::cx;
+  using vec = typename PV<real>::vec;
+  cx acc[12];
+  cx phi[12];
+  const cx* W;
+  const vec* psi;
+  const cx* Wn;     // matrices of the current use's site (own site, or the neighbour for an opposite-direction term)
+  int n, x, y, z, t;
+  int L0, L1, L2, L3;
+};
 
-// acc[BASE + 3 al + ca] += c * sigma[al][be] * tv[be][ca]   (BASE = 0: upper spin half of the output, 6: lower)
-template <int BASE, typename cx, typename real>
-__device__ __forceinline__ void place(cx (&acc)[12], const cx (&tv)[2][3], int sigma, real c) {
-  if (sigma == 0 || sigma == 3) {           // diagonal in spin: +c, +-c
-    const real c1 = sigma == 3 ? -c : c;
+template <int BASE, int SIGMA, typename cx, typename real>
+__device__ __forceinline__ void place_ct(cx (&acc)[12], const cx (&tv)[2][3], real c) {
 #pragma unroll
-    for (int ca = 0; ca < 3; ++ca) {
+  for (int ca = 0; ca < 3; ++ca) {
+    if constexpr (SIGMA == 0 || SIGMA == 3) {
+      const real c1 = SIGMA == 3 ? -c : c;
       acc[BASE + ca].x = fma(c, tv[0][ca].x, acc[BASE + ca].x);
       acc[BASE + ca].y = fma(c, tv[0][ca].y, acc[BASE + ca].y);
       acc[BASE + 3 + ca].x = fma(c1, tv[1][ca].x, acc[BASE + 3 + ca].x);
       acc[BASE + 3 + ca].y = fma(c1, tv[1][ca].y, acc[BASE + 3 + ca].y);
-    }
-  } else if (sigma == 1) {                  // sigma_x: swaps the two spins
-#pragma unroll
-    for (int ca = 0; ca < 3; ++ca) {
+    } else if constexpr (SIGMA == 1) {
       acc[BASE + ca].x = fma(c, tv[1][ca].x, acc[BASE + ca].x);
       acc[BASE + ca].y = fma(c, tv[1][ca].y, acc[BASE + ca].y);
       acc[BASE + 3 + ca].x = fma(c, tv[0][ca].x, acc[BASE + 3 + ca].x);
       acc[BASE + 3 + ca].y = fma(c, tv[0][ca].y, acc[BASE + 3 + ca].y);
-    }
-  } else {                                  // sigma_y: out_0 += -i c t_1 ; out_1 += i c t_0
-#pragma unroll
-    for (int ca = 0; ca < 3; ++ca) {
+    } else {
       acc[BASE + ca].x = fma(c, tv[1][ca].y, acc[BASE + ca].x);
       acc[BASE + ca].y = fma(-c, tv[1][ca].x, acc[BASE + ca].y);
       acc[BASE + 3 + ca].x = fma(-c, tv[0][ca].y, acc[BASE + 3 + ca].x);
@@ -184,169 +204,146 @@ __device__ __forceinline__ void place(cx (&acc)[12], const cx (&tv)[2][3], int s
   }
 }
 
-template <typename real, bool DOT>
-__global__ void __launch_bounds__(32 * kPauliWarps)
-apply_pauli_kernel(const typename PV<real>::cx* __restrict__ W, const typename PV<real>::vec* __restrict__ psi,
-                   typename PV<real>::vec* __restrict__ out, PauliArgs a, const typename PV<real>::vec* __restrict__ dot_a,
-                   double* __restrict__ partials) {
+template <typename real, int U, int PI, int H>
+__device__ __forceinline__ void placement_ct(PState<real>& st, const typename PV<real>::cx (&tv)[2][3]) {
+  constexpr Placement pl = kUses.u[U].pl[PI];
+  if constexpr (pl.kind == 0) {                 // D: output half = input half, if that diagonal block is present
+    if constexpr (((pl.flags >> H) & 1) != 0) place_ct<6 * H, pl.sigma>(st.acc, tv, coef_of<real>(pl.coef));
+  } else if constexpr (pl.kind == 1) {          // S: the other half; the lower-left block of W^0 is negated
+    constexpr int TH = 1 - H;
+    const real c = coef_of<real>(pl.coef);
+    place_ct<6 * TH, pl.sigma>(st.acc, tv, (TH == 1 && (pl.flags & 4)) ? -c : c);
+  }
+}
+
+// one use; FIRST: first use of this warp's range (a new term starts there by construction)
+template <typename real, int U, bool FIRST, bool MASS>
+__device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
   using cx = typename PV<real>::cx;
   using vec = typename PV<real>::vec;
   constexpr int NC = PV<real>::NC;
-  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
-  const int blk = blockIdx.x;
+  constexpr Use u = kUses.u[U];
+  constexpr bool newterm = FIRST || kUses.u[U > 0 ? U - 1 : 0].term != u.term;
+  if constexpr (newterm) {
+    constexpr int T = u.term;
+    const int xx = wrapp(st.x + kOffC[T][0], st.L0), yy = wrapp(st.y + kOffC[T][1], st.L1);
+    const int zz = wrapp(st.z + kOffC[T][2], st.L2), tt = wrapp(st.t + kOffC[T][3], st.L3);
+    const int nn = T == 0 ? st.n : xx + st.L0 * (yy + st.L1 * (zz + st.L2 * tt));
+    const vec* sp = st.psi + (size_t)(nn >> 5) * NC * kBlock + (nn & 31);
+    if constexpr (sizeof(real) == 4) {
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        const float4 v = __ldg(sp + c * kBlock);
+        st.phi[2 * c] = cx{v.x, v.y};
+        st.phi[2 * c + 1] = cx{v.z, v.w};
+      }
+    } else {
+#pragma unroll
+      for (int c = 0; c < 12; ++c) st.phi[c] = __ldg(sp + c * kBlock);
+    }
+    const int nm = u.adj ? nn : st.n;
+    st.Wn = st.W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31);
+    if constexpr (MASS && T == 0) {
+#pragma unroll
+      for (int r = 0; r < 12; ++r) { st.acc[r].x += mass * st.phi[r].x; st.acc[r].y += mass * st.phi[r].y; }
+    }
+  }
+  cx C[9];
+#pragma unroll
+  for (int e = 0; e < 9; ++e) C[e] = __ldg(st.Wn + (size_t)(9 * u.m + e) * kBlock);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    cx tv[2][3];
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int ca = 0; ca < 3; ++ca) {
+        real re = 0, im = 0;
+#pragma unroll
+        for (int cb = 0; cb < 3; ++cb) {
+          const cx v = st.phi[3 * (2 * h + s) + cb];
+          if constexpr (u.adj != 0) {
+            const cx w = C[3 * cb + ca];
+            re = fma(w.x, v.x, re); re = fma(w.y, v.y, re);
+            im = fma(w.x, v.y, im); im = fma(-w.y, v.x, im);
+          } else {
+            const cx w = C[3 * ca + cb];
+            re = fma(w.x, v.x, re); re = fma(-w.y, v.y, re);
+            im = fma(w.x, v.y, im); im = fma(w.y, v.x, im);
+          }
+        }
+        tv[s][ca] = cx{re, im};
+      }
+    if (h == 0) { placement_ct<real, U, 0, 0>(st, tv); placement_ct<real, U, 1, 0>(st, tv); }
+    else { placement_ct<real, U, 0, 1>(st, tv); placement_ct<real, U, 1, 1>(st, tv); }
+  }
+}
+
+template <typename real, int U, int UEND, bool FIRST, bool MASS>
+__device__ __forceinline__ void run_uses(PState<real>& st, real mass) {
+  if constexpr (U < UEND) {
+    use_ct<real, U, FIRST, MASS>(st, mass);
+    run_uses<real, U + 1, UEND, false, MASS>(st, mass);
+  }
+}
+
+// kPauliParts launches per apply, each with its share of the uses: the straight-line code of all 68 specialised uses (about
+// 13 k instructions) does not fit the instruction cache -- as ONE kernel it runs at 1.0 ms, slower than the table-driven loop
+// it replaced (0.72 ms) -- while halves do: 0.40 ms with 2 parts (3: 0.47, 4: 0.49, 6: 0.59, 8: 0.62 ms; 20^3x64 fp32).  Part 0
+// writes out (with the mass term), the later parts add to it, the last one also does the fused BiCGStab reductions; launches
+// on one stream are ordered, so the sum has a fixed order.  lane <-> site, one warp per 32-site block, four blocks per CTA.
+template <typename real, int PART, bool DOT>
+__global__ void __launch_bounds__(128)
+apply_pauli_part_kernel(const typename PV<real>::cx* __restrict__ W, const typename PV<real>::vec* __restrict__ psi,
+                        typename PV<real>::vec* __restrict__ out, PauliArgs a, const typename PV<real>::vec* __restrict__ dot_a,
+                        double* __restrict__ partials) {
+  using cx = typename PV<real>::cx;
+  using vec = typename PV<real>::vec;
+  constexpr int NC = PV<real>::NC;
+  const int lane = threadIdx.x & 31;
+  const int blk = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (blk >= a.g.nblk) return;
   int n = blk * kBlock + lane;
   const bool live = n < a.g.V;
   if (!live) n = 0;
-  const int x = n % a.g.L[0];
-  int q = n / a.g.L[0];
-  const int y = q % a.g.L[1];
-  q /= a.g.L[1];
-  const int z = q % a.g.L[2];
-  const int t = q / a.g.L[2];
-
-  cx acc[12];
-#pragma unroll
-  for (int r = 0; r < 12; ++r) acc[r] = cx{0, 0};
-  cx phi[12];
-  // neighbour site of a stencil term: it holds the spinor and, for an opposite-direction term, the matrices
-  auto site_of_term = [&](int term) {
-    const int xx = wrapp(x + c_poff2[term][0], a.g.L[0]);
-    const int yy = wrapp(y + c_poff2[term][1], a.g.L[1]);
-    const int zz = wrapp(z + c_poff2[term][2], a.g.L[2]);
-    const int tt = wrapp(t + c_poff2[term][3], a.g.L[3]);
-    return xx + a.g.L[0] * (yy + a.g.L[1] * (zz + a.g.L[2] * tt));
-  };
-  auto matrix_of = [&](const Use& u, int nn) {   // a positive term and W^0 use the matrices of THIS site
-    const int nm = u.adj ? nn : n;
-    return W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31) + (size_t)(9 * u.m) * kBlock;
-  };
-  // The loop is rolled (one generic body for the 68 uses) and software-pipelined by hand: the nine loads of the NEXT use are
-  // issued before the arithmetic of the current one (every stored matrix is used by its own site and by one neighbour, so
-  // default-policy loads).
-  const int last = c_uses.first[wp + 1];
-  int ui = c_uses.first[wp];
-  Use u = c_uses.u[ui < last ? ui : 0];
-  int nn = site_of_term(u.term);
-  cx C[9];
-  {
-    const cx* cp = matrix_of(u, nn);
-#pragma unroll
-    for (int e = 0; e < 9; ++e) C[e] = __ldg(cp + (size_t)e * kBlock);
-  }
-  int cur = -1;
-#pragma unroll 1
-  for (; ui < last; ++ui) {
-    Use un = u;
-    int nn_next = nn;
-    cx Cn[9];
-    if (ui + 1 < last) {
-      un = c_uses.u[ui + 1];
-      if (un.term != u.term) nn_next = site_of_term(un.term);
-      const cx* cp = matrix_of(un, nn_next);
-#pragma unroll
-      for (int e = 0; e < 9; ++e) Cn[e] = __ldg(cp + (size_t)e * kBlock);
-    } else {
-#pragma unroll
-      for (int e = 0; e < 9; ++e) Cn[e] = C[e];
-    }
-    if (u.term != cur) {   // new stencil term: load its neighbour spinor
-      cur = u.term;
-      const vec* sp = psi + (size_t)(nn >> 5) * NC * kBlock + (nn & 31);
-      if constexpr (sizeof(real) == 4) {
-#pragma unroll
-        for (int c = 0; c < 6; ++c) {
-          const float4 v = __ldg(sp + c * kBlock);
-          phi[2 * c] = cx{v.x, v.y};
-          phi[2 * c + 1] = cx{v.z, v.w};
-        }
-      } else {
-#pragma unroll
-        for (int c = 0; c < 12; ++c) phi[c] = __ldg(sp + c * kBlock);
-      }
-      if (cur == 0 && wp == 0) {   // the mass term of W^0 (Eq. 2.6)
-        const real ms = (real)a.mass;
-#pragma unroll
-        for (int r = 0; r < 12; ++r) { acc[r].x += ms * phi[r].x; acc[r].y += ms * phi[r].y; }
-      }
-    }
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {   // input spin half: upper (spins 0, 1) or lower (2, 3)
-      cx tv[2][3];
-      if (u.adj) {                  // C^dag phi (warp-uniform branch: no per-element selects)
-#pragma unroll
-        for (int s = 0; s < 2; ++s)
-#pragma unroll
-          for (int ca = 0; ca < 3; ++ca) {
-            real re = 0, im = 0;
-#pragma unroll
-            for (int cb = 0; cb < 3; ++cb) {
-              const cx w = C[3 * cb + ca], v = phi[3 * (2 * h + s) + cb];
-              re = fma(w.x, v.x, re); re = fma(w.y, v.y, re);
-              im = fma(w.x, v.y, im); im = fma(-w.y, v.x, im);
-            }
-            tv[s][ca] = cx{re, im};
-          }
-      } else {
-#pragma unroll
-        for (int s = 0; s < 2; ++s)
-#pragma unroll
-          for (int ca = 0; ca < 3; ++ca) {
-            real re = 0, im = 0;
-#pragma unroll
-            for (int cb = 0; cb < 3; ++cb) {
-              const cx w = C[3 * ca + cb], v = phi[3 * (2 * h + s) + cb];
-              re = fma(w.x, v.x, re); re = fma(-w.y, v.y, re);
-              im = fma(w.x, v.y, im); im = fma(w.y, v.x, im);
-            }
-            tv[s][ca] = cx{re, im};
-          }
-      }
-#pragma unroll
-      for (int pi = 0; pi < 2; ++pi) {
-        const Placement pl = u.pl[pi];
-        real c = coef_of<real>(pl.coef);
-        // D: output half = input half, if that diagonal block is present; S: the other half, the lower-left block of W^0 negated
-        const bool isD = pl.kind == 0;
-        const bool on = isD ? ((pl.flags >> h) & 1) != 0 : pl.kind == 1;
-        const int th = isD ? h : 1 - h;
-        if (!isD && th == 1 && (pl.flags & 4)) c = -c;
-        // out[al] += c sigma[al][be] tv[be]; sigma and th are warp-uniform runtime values: branch, no dynamic register indexing
-        if (on) {
-          if (th == 0) place<0>(acc, tv, pl.sigma, c);
-          else place<6>(acc, tv, pl.sigma, c);
-        }
-      }
-    }
-    u = un;
-    nn = nn_next;
-#pragma unroll
-    for (int e = 0; e < 9; ++e) C[e] = Cn[e];
-  }
-
-  // fixed-order sum of the four warps' partial results, then the store (and the fused BiCGStab reductions)
-  __shared__ cx red[kPauliWarps][12][kBlock];
-#pragma unroll
-  for (int r = 0; r < 12; ++r) red[wp][r][lane] = acc[r];
-  __syncthreads();
-  if (wp != 0) return;
-  cx o[12];
-#pragma unroll
-  for (int r = 0; r < 12; ++r) {
-    cx s = red[0][r][lane];
-#pragma unroll
-    for (int w = 1; w < kPauliWarps; ++w) { s.x += red[w][r][lane].x; s.y += red[w][r][lane].y; }
-    if (!live) s = cx{0, 0};
-    o[r] = s;
-  }
+  PState<real> st;
+  st.n = n;
+  st.L0 = a.g.L[0]; st.L1 = a.g.L[1]; st.L2 = a.g.L[2]; st.L3 = a.g.L[3];
+  st.x = n % st.L0;
+  int q = n / st.L0;
+  st.y = q % st.L1;
+  q /= st.L1;
+  st.z = q % st.L2;
+  st.t = q / st.L2;
+  st.W = W; st.psi = psi; st.Wn = W;
   vec* ob = out + (size_t)blk * NC * kBlock + lane;
-  if constexpr (sizeof(real) == 4) {
+  if constexpr (PART == 0) {
 #pragma unroll
-    for (int c = 0; c < 6; ++c) ob[c * kBlock] = make_float4(o[2 * c].x, o[2 * c].y, o[2 * c + 1].x, o[2 * c + 1].y);
+    for (int r = 0; r < 12; ++r) st.acc[r] = cx{0, 0};
+  } else if constexpr (sizeof(real) == 4) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+      const float4 v = ob[c * kBlock];
+      st.acc[2 * c] = cx{v.x, v.y};
+      st.acc[2 * c + 1] = cx{v.z, v.w};
+    }
   } else {
 #pragma unroll
-    for (int c = 0; c < 12; ++c) ob[c * kBlock] = o[c];
+    for (int c = 0; c < 12; ++c) st.acc[c] = ob[c * kBlock];
   }
-  if constexpr (DOT) {
+  run_uses<real, kUses.first[PART], kUses.first[PART + 1], true, PART == 0>(st, (real)a.mass);
+  if (!live) {
+#pragma unroll
+    for (int r = 0; r < 12; ++r) st.acc[r] = cx{0, 0};
+  }
+  if constexpr (sizeof(real) == 4) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) ob[c * kBlock] = make_float4(st.acc[2 * c].x, st.acc[2 * c].y, st.acc[2 * c + 1].x, st.acc[2 * c + 1].y);
+  } else {
+#pragma unroll
+    for (int c = 0; c < 12; ++c) ob[c * kBlock] = st.acc[c];
+  }
+  if constexpr (DOT && PART == kPauliParts - 1) {
     const vec* ab = dot_a + (size_t)blk * NC * kBlock + lane;
     double d0 = 0.0, d1 = 0.0, d2 = 0.0;
 #pragma unroll
@@ -360,7 +357,7 @@ apply_pauli_kernel(const typename PV<real>::cx* __restrict__ W, const typename P
         const double2 v = ab[r * kBlock];
         ar = v.x; ai = v.y;
       }
-      const double vr = (double)o[r].x, vi = (double)o[r].y;
+      const double vr = (double)st.acc[r].x, vi = (double)st.acc[r].y;
       d0 += ar * vr + ai * vi;
       d1 += ar * vi - ai * vr;
       d2 += vr * vr + vi * vi;
@@ -438,7 +435,10 @@ __global__ void __launch_bounds__(128) unpack_pauli_kernel(const typename PV<rea
 
 int pauli_init() {
   if (g_pauli_ready) return OK_SUCCESS;
-  build_uses(h_uses);
+  for (int t = 0; t < kTerms; ++t)
+    for (int d = 0; d < 4; ++d)
+      if (kOffC[t][d] != kOffsets[t][d]) return OK_EINVAL;   // the compile-time copy of the stencil offsets must match ok.h's
+  static const UseTable h_uses = kUses;
   OK_CUDA(cudaMemcpyToSymbol(c_uses, &h_uses, sizeof(UseTable)));
   OK_CUDA(cudaMemcpyToSymbol(c_poff2, kOffsets, sizeof(kOffsets)));
   g_pauli_ready = true;
@@ -459,6 +459,18 @@ PauliArgs make_args(const ok_params* p) {
   return a;
 }
 
+template <typename real, int PART>
+int launch_parts(unsigned grid, cudaStream_t st, const typename PV<real>::cx* W, const typename PV<real>::vec* psi, typename PV<real>::vec* out,
+                 const PauliArgs& a, const typename PV<real>::vec* dot_a, double* partials) {
+  if constexpr (PART < kPauliParts) {
+    if (PART == kPauliParts - 1 && partials) apply_pauli_part_kernel<real, PART, true><<<grid, 128, 0, st>>>(W, psi, out, a, dot_a, partials);
+    else apply_pauli_part_kernel<real, PART, false><<<grid, 128, 0, st>>>(W, psi, out, a, nullptr, nullptr);
+    OK_LAUNCHED("apply_pauli_part_kernel");
+    return launch_parts<real, PART + 1>(grid, st, W, psi, out, a, dot_a, partials);
+  }
+  return OK_SUCCESS;
+}
+
 template <typename real>
 int launch_pauli(const ok_params* p, const void* W, const void* psi, void* out, double* partials, const void* dot_a) {
   using cx = typename PV<real>::cx;
@@ -475,14 +487,13 @@ int launch_pauli(const ok_params* p, const void* W, const void* psi, void* out, 
     OK_CUDA(cudaMemcpyToSymbolAsync(c_coef64, a.coef, sizeof(a.coef), 0, cudaMemcpyHostToDevice, ctx().stream));
     have = true;
   }
-  if (partials)
-    apply_pauli_kernel<real, true><<<a.g.nblk, 32 * kPauliWarps, 0, ctx().stream>>>(static_cast<const cx*>(W), static_cast<const vec*>(psi),
-                                                                                   static_cast<vec*>(out), a, static_cast<const vec*>(dot_a), partials);
-  else
-    apply_pauli_kernel<real, false><<<a.g.nblk, 32 * kPauliWarps, 0, ctx().stream>>>(static_cast<const cx*>(W), static_cast<const vec*>(psi),
-                                                                                    static_cast<vec*>(out), a, nullptr, nullptr);
-  OK_LAUNCHED("apply_pauli_kernel");
-  return OK_SUCCESS;
+  const cx* Wc = static_cast<const cx*>(W);
+  const vec* ps = static_cast<const vec*>(psi);
+  vec* o = static_cast<vec*>(out);
+  const vec* da = static_cast<const vec*>(dot_a);
+  const unsigned grid = (unsigned)((a.g.nblk + 3) / 4);
+  cudaStream_t st = ctx().stream;
+  return launch_parts<real, 0>(grid, st, Wc, ps, o, a, da, partials);
 }
 
 }  // namespace
