@@ -715,7 +715,8 @@ def run_ours(args, wl):
             P.release()
             line["configs"] = {}
             for name, sub in [("configs[3] 12 RHS", "20x20x20x64-fp32-rhs12"), ("configs[2] lattice in fp64", "20x20x20x64-fp64"),
-                              ("configs[4] 32^3x64 Haar", "32x32x32x64-fp32")]:
+                              ("configs[4] 32^3x64 Haar", "32x32x32x64-fp32"),
+                              ("configs[2] in the paper's 50-colour-block compression (OK_W_PAULI)", "20x20x20x64-fp32-pauli")]:
                 try:
                     line["configs"][name] = sub_record(sub, dev, stream, local, peaks)
                 except Exception as e:      # a sub-record must not take the contract line down with it
