@@ -36,8 +36,7 @@ struct PrecalcArgs {
   int storage;                 // OK_W_DENSE / OK_W_BLOCK / OK_W_DS (ok_sparse.cuh)
   int pair;                    // 1: the thread of a positive-direction term also writes the opposite term of the neighbour site
   int posonly;                 // 1: grid over W^0 and the 13 positive-direction terms only (pair, or OK_W_CONJ)
-  int blk0;                    // first 32-site block of this launch (12-RHS: the dense W of a chunk goes to a bounce buffer;
-                               // t-slab: the first interior block of the extended link window)
+  int blk0;                    // first 32-site block of this launch (t-slab: the first interior block of the extended link window)
   int tfold;                   // time slice whose U_4 carries bc[3] (L[3] - 1 on a whole lattice; t-slab: where global T - 1 sits, or -1)
   double mass;                 // u0 / (2 kappa)
   double d0, s0;               // D^0, S^0 prefactors (Eq. 2.6)
@@ -525,6 +524,128 @@ __global__ void __launch_bounds__(32 * 3, CLS == 1 ? OK_CLS1_MINB : 4) assemble_
 // straight from the transposed scratch -- 3 contiguous-line loads per matrix -- and writes the four spin rows (alpha, ca) of
 // W.  No matrix is held in registers across rows (the templated path spilled 2.5-3 KB per thread on the seven matrices of a
 // one-link hop), every thread writes its own site only.  fp64 throughout, rounded once.
+// what a thread of W^0, W^+-_i or W^+-_4 needs besides the colour row: family, directions, signs, and where its colour matrices live
+struct PauliTerm {
+  int fam, i, k, l;           // fam 0: W^0, 1: W^+-_4, 2: W^+-_i ; hop direction i, cyclic (i, k, l)
+  bool neg, ulA, lrA;
+  double usg, llsgn, mass;
+  const double2* F;           // scratch fields at the site of the positive blocks: matrix m, element e at F[(9 m + e) Vpad]
+  const double2* Ul;          // the hop's link there
+};
+__device__ __forceinline__ PauliTerm pauli_term_of(int term, int n, const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                                   const PrecalcArgs& a) {
+  PauliTerm c;
+  c.fam = term == 0 ? 0 : (term >= 7 ? 1 : 2);
+  c.i = c.fam == 2 ? (term - 1) >> 1 : 3;           // hop direction
+  c.neg = c.fam == 0 ? false : (c.fam == 1 ? term == 8 : ((term - 1) & 1) != 0);
+  Site x = site_of(n, a.g);
+  if (c.neg)
+    for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
+  const int ns = index_of(x, a.g);
+  c.F = reinterpret_cast<const double2*>(FS) + ns;
+  c.usg = (c.fam != 0 && a.bc[c.i] < 0 && x.c[c.i] == (c.i == 3 ? a.tfold : a.g.L[c.i] - 1)) ? -1.0 : 1.0;
+  c.Ul = links + (size_t)(9 * (c.fam == 0 ? 0 : c.i)) * a.Vpad + ns;
+  c.k = c.fam == 2 ? (c.i + 1) % 3 : 1;
+  c.l = c.fam == 2 ? (c.i + 2) % 3 : 2;
+  c.ulA = c.fam == 1 ? c.neg : true;
+  c.lrA = c.fam == 1 ? !c.neg : true;
+  c.llsgn = c.fam == 0 ? -1.0 : 1.0;
+  c.mass = c.fam == 0 ? a.mass : 0.0;
+  return c;
+}
+// Colour row ca of the term as the 24 complex numbers its four spin rows (alpha, ca) are made of: with the Pauli components
+// C_0..C_3 of a 6x6 block (header comment), combo 0: C0 + C3 (al = be = 0), 1: C0 - C3 (al = be = 1), 2: C1 - i C2 (al, be = 0, 1),
+// 3: C1 + i C2 (1, 0); Dv[combo][cb] for the diagonal blocks (the mass term of W^0 included), Sv[combo][cb] for the off-diagonal ones.
+__device__ __forceinline__ void pauli_term_tables(const PauliTerm& t, int ca, const PrecalcArgs& a, double2 (&Dv)[4][3], double2 (&Sv)[4][3]) {
+  const int fam = t.fam, i = t.i, k = t.k;
+  const bool neg = t.neg;
+  const double usg = t.usg;
+  const double2* F = t.F;
+  const double2* Ul = t.Ul;
+  auto at = [&](const double2* base, int kmat, int e) { return __ldg(base + (size_t)(9 * kmat + e) * a.Vpad); };
+#pragma unroll
+  for (int cb = 0; cb < 3; ++cb) {
+    const int e = neg ? 3 * cb + ca : 3 * ca + cb;       // the adjoint reads the transposed element
+    const double2 z = make_double2(0.0, 0.0);
+    double2 a0 = z, a1 = z, a2 = z, a3 = z, b0 = z, b1 = z, b2 = z, b3 = z;
+    if (fam == 0) {          // D^0 = i d0 sum sigma_m B_m ; S^0 = s0 sum sigma_m E_m     (Eq. 2.6)
+      const double2 f0 = at(F, 0, e), f1 = at(F, 1, e), f2 = at(F, 2, e);
+      a1 = make_double2(-a.d0 * f0.y, a.d0 * f0.x); a2 = make_double2(-a.d0 * f1.y, a.d0 * f1.x); a3 = make_double2(-a.d0 * f2.y, a.d0 * f2.x);
+      const double2 g0 = at(F, 3, e), g1 = at(F, 4, e), g2 = at(F, 5, e);
+      b1 = make_double2(a.s0 * g0.x, a.s0 * g0.y); b2 = make_double2(a.s0 * g1.x, a.s0 * g1.y); b3 = make_double2(a.s0 * g2.x, a.s0 * g2.y);
+    } else if (fam == 1) {   // D^+_4 = -U_4 ; S^+_4 = sum sigma_m T_m                        (Eq. 2.7)
+      const double2 u = __ldg(Ul + (size_t)e * a.Vpad);
+      a0 = make_double2(-usg * u.x, -usg * u.y);
+      b1 = at(F, 6 + 15, e); b2 = at(F, 6 + 16, e); b3 = at(F, 6 + 17, e);
+    } else {                 // Eq. (2.8): hop_blocks_kernel's q = 0..4 of direction i, and U_i itself
+      const double2 u = __ldg(Ul + (size_t)e * a.Vpad);
+      const int hb = 6 + 5 * i;
+      const double2 vi_b = make_double2(a.a1 * usg * u.x, a.a1 * usg * u.y);                     // S.C_i = a1 U
+      const double2 vk_b = at(F, hb + 1, e), vl_b = at(F, hb + 2, e), vk_a = at(F, hb + 3, e), vl_a = at(F, hb + 4, e);
+      a0 = make_double2(a.d1 * usg * u.x, a.d1 * usg * u.y);                                     // D.C_0 = d1 U
+      b0 = at(F, hb, e);
+      // direction d carries the i-, k- or l-component
+      a1 = i == 0 ? z : (k == 0 ? vk_a : vl_a); b1 = i == 0 ? vi_b : (k == 0 ? vk_b : vl_b);
+      a2 = i == 1 ? z : (k == 1 ? vk_a : vl_a); b2 = i == 1 ? vi_b : (k == 1 ? vk_b : vl_b);
+      a3 = i == 2 ? z : (k == 2 ? vk_a : vl_a); b3 = i == 2 ? vi_b : (k == 2 ? vk_b : vl_b);
+    }
+    if (neg) {               // A -> A^dag, B -> -B^dag (the element was read transposed)
+      a0.y = -a0.y; a1.y = -a1.y; a2.y = -a2.y; a3.y = -a3.y;
+      b0.x = -b0.x; b1.x = -b1.x; b2.x = -b2.x; b3.x = -b3.x;
+    }
+    const double m = ca == cb ? t.mass : 0.0;
+    Dv[0][cb] = make_double2(a0.x + a3.x + m, a0.y + a3.y);
+    Dv[1][cb] = make_double2(a0.x - a3.x + m, a0.y - a3.y);
+    Dv[2][cb] = make_double2(a1.x + a2.y, a1.y - a2.x);
+    Dv[3][cb] = make_double2(a1.x - a2.y, a1.y + a2.x);
+    Sv[0][cb] = make_double2(b0.x + b3.x, b0.y + b3.y);
+    Sv[1][cb] = make_double2(b0.x - b3.x, b0.y - b3.y);
+    Sv[2][cb] = make_double2(b1.x + b2.y, b1.y - b2.x);
+    Sv[3][cb] = make_double2(b1.x - b2.y, b1.y + b2.x);
+  }
+}
+// the four spin rows (alpha, ca), alpha = 0..3: emit(alpha, row[12]) with row[3 beta + cb]
+template <class Emit>
+__device__ __forceinline__ void pauli_term_rows(const PauliTerm& t, int ca, const PrecalcArgs& a, Emit&& emit) {
+  double2 Dv[4][3], Sv[4][3];
+  pauli_term_tables(t, ca, a, Dv, Sv);
+#pragma unroll
+  for (int alpha = 0; alpha < 4; ++alpha) {
+    const int bi = alpha >> 1, al = alpha & 1;
+    double2 row[12];
+#pragma unroll
+    for (int beta = 0; beta < 4; ++beta) {
+      const int bj = beta >> 1, be = beta & 1;
+      const int combo = al == be ? al : (al == 0 ? 2 : 3);
+#pragma unroll
+      for (int cb = 0; cb < 3; ++cb) {
+        double2 v;
+        if (bi == bj) {
+          v = (bi == 0 ? t.ulA : t.lrA) ? Dv[combo][cb] : make_double2(0.0, 0.0);
+        } else {
+          v = Sv[combo][cb];
+          if (bi == 1) { v.x *= t.llsgn; v.y *= t.llsgn; }
+        }
+        row[3 * beta + cb] = v;
+      }
+    }
+    emit(alpha, row);
+  }
+}
+
+// one row of 12 complex numbers -> the dense layout (rounded once to the storage precision)
+template <typename real>
+__device__ __forceinline__ void store_dense_row(typename WUnit<real>::type* __restrict__ dst, const double2 (&row)[12]) {
+  if constexpr (sizeof(real) == 4) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c)
+      dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
+  } else {
+#pragma unroll
+    for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
+  }
+}
+
 template <typename real>
 __global__ void __launch_bounds__(32 * 3) pauli_terms_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
                                                              typename WUnit<real>::type* __restrict__ W, PrecalcArgs a) {
@@ -540,93 +661,10 @@ __global__ void __launch_bounds__(32 * 3) pauli_terms_kernel(const double2* __re
     for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
     return;
   }
-  const int fam = term == 0 ? 0 : (term >= 7 ? 1 : 2);
-  const int i = fam == 2 ? (term - 1) >> 1 : 3;           // hop direction
-  const bool neg = fam == 0 ? false : (fam == 1 ? term == 8 : ((term - 1) & 1) != 0);
-  Site x = site_of(n, a.g);
-  if (neg)
-    for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
-  const int ns = index_of(x, a.g);
-  const double2* F = reinterpret_cast<const double2*>(FS) + ns;                                   // matrix k, element e: F[(9k+e) Vpad]
-  const double usg = (fam != 0 && a.bc[i] < 0 && x.c[i] == (i == 3 ? a.tfold : a.g.L[i] - 1)) ? -1.0 : 1.0;
-  const double2* Ul = links + (size_t)(9 * (fam == 0 ? 0 : i)) * a.Vpad + ns;                       // the hop's link
-  const int k = fam == 2 ? (i + 1) % 3 : 1, l = fam == 2 ? (i + 2) % 3 : 2;
-  const bool ulA = fam == 1 ? neg : true, lrA = fam == 1 ? !neg : true;
-  const double llsgn = fam == 0 ? -1.0 : 1.0, mass = fam == 0 ? a.mass : 0.0;
-  auto at = [&](const double2* base, int kmat, int e) { return __ldg(base + (size_t)(9 * kmat + e) * a.Vpad); };
+  const PauliTerm t = pauli_term_of(term, n, links, FS, a);
 #pragma unroll 1
-  for (int ca = 0; ca < 3; ++ca) {
-    // Pauli components of this colour row: A (diagonal blocks) and B (off-diagonal blocks), index 0 = 1, 1..3 = sigma_x,y,z
-    double2 A[4][3], Bm[4][3];
-#pragma unroll
-    for (int cb = 0; cb < 3; ++cb) {
-      const int e = neg ? 3 * cb + ca : 3 * ca + cb;       // the adjoint reads the transposed element
-      const double2 z = make_double2(0.0, 0.0);
-      double2 a0 = z, a1 = z, a2 = z, a3 = z, b0 = z, b1 = z, b2 = z, b3 = z;
-      if (fam == 0) {          // D^0 = i d0 sum sigma_m B_m ; S^0 = s0 sum sigma_m E_m     (Eq. 2.6)
-        const double2 f0 = at(F, 0, e), f1 = at(F, 1, e), f2 = at(F, 2, e);
-        a1 = make_double2(-a.d0 * f0.y, a.d0 * f0.x); a2 = make_double2(-a.d0 * f1.y, a.d0 * f1.x); a3 = make_double2(-a.d0 * f2.y, a.d0 * f2.x);
-        const double2 g0 = at(F, 3, e), g1 = at(F, 4, e), g2 = at(F, 5, e);
-        b1 = make_double2(a.s0 * g0.x, a.s0 * g0.y); b2 = make_double2(a.s0 * g1.x, a.s0 * g1.y); b3 = make_double2(a.s0 * g2.x, a.s0 * g2.y);
-      } else if (fam == 1) {   // D^+_4 = -U_4 ; S^+_4 = sum sigma_m T_m                        (Eq. 2.7)
-        const double2 u = __ldg(Ul + (size_t)e * a.Vpad);
-        a0 = make_double2(-usg * u.x, -usg * u.y);
-        b1 = at(F, 6 + 15, e); b2 = at(F, 6 + 16, e); b3 = at(F, 6 + 17, e);
-      } else {                 // Eq. (2.8): hop_blocks_kernel's q = 0..4 of direction i, and U_i itself
-        const double2 u = __ldg(Ul + (size_t)e * a.Vpad);
-        const int hb = 6 + 5 * i;
-        const double2 vi_b = make_double2(a.a1 * usg * u.x, a.a1 * usg * u.y);                     // S.C_i = a1 U
-        const double2 vk_b = at(F, hb + 1, e), vl_b = at(F, hb + 2, e), vk_a = at(F, hb + 3, e), vl_a = at(F, hb + 4, e);
-        a0 = make_double2(a.d1 * usg * u.x, a.d1 * usg * u.y);                                     // D.C_0 = d1 U
-        b0 = at(F, hb, e);
-        // direction d carries the i-, k- or l-component
-        a1 = i == 0 ? z : (k == 0 ? vk_a : vl_a); b1 = i == 0 ? vi_b : (k == 0 ? vk_b : vl_b);
-        a2 = i == 1 ? z : (k == 1 ? vk_a : vl_a); b2 = i == 1 ? vi_b : (k == 1 ? vk_b : vl_b);
-        a3 = i == 2 ? z : (k == 2 ? vk_a : vl_a); b3 = i == 2 ? vi_b : (k == 2 ? vk_b : vl_b);
-      }
-      if (neg) {               // A -> A^dag, B -> -B^dag (the element was read transposed)
-        a0.y = -a0.y; a1.y = -a1.y; a2.y = -a2.y; a3.y = -a3.y;
-        b0.x = -b0.x; b1.x = -b1.x; b2.x = -b2.x; b3.x = -b3.x;
-      }
-      A[0][cb] = a0; A[1][cb] = a1; A[2][cb] = a2; A[3][cb] = a3;
-      Bm[0][cb] = b0; Bm[1][cb] = b1; Bm[2][cb] = b2; Bm[3][cb] = b3;
-    }
-#pragma unroll
-    for (int alpha = 0; alpha < 4; ++alpha) {
-      const int bi = alpha >> 1, al = alpha & 1;
-      double2 row[12];
-#pragma unroll
-      for (int beta = 0; beta < 4; ++beta) {
-        const int bj = beta >> 1, be = beta & 1;
-        const bool diag = bi == bj;
-        const bool useA = diag && (bi == 0 ? ulA : lrA);
-#pragma unroll
-        for (int cb = 0; cb < 3; ++cb) {
-          const double2 c0 = diag ? A[0][cb] : Bm[0][cb], c1 = diag ? A[1][cb] : Bm[1][cb], c2 = diag ? A[2][cb] : Bm[2][cb],
-                        c3 = diag ? A[3][cb] : Bm[3][cb];
-          double2 v;
-          if (al == be) v = al == 0 ? make_double2(c0.x + c3.x, c0.y + c3.y) : make_double2(c0.x - c3.x, c0.y - c3.y);
-          else v = al == 0 ? make_double2(c1.x + c2.y, c1.y - c2.x) : make_double2(c1.x - c2.y, c1.y + c2.x);
-          if (diag) {
-            if (!useA) v = make_double2(0.0, 0.0);
-            if (alpha == beta && ca == cb) v.x += mass;
-          } else if (bi == 1) {
-            v.x *= llsgn; v.y *= llsgn;
-          }
-          row[3 * beta + cb] = v;
-        }
-      }
-      unit_t* dst = Wt + (size_t)(3 * alpha + ca) * NC * kBlock;
-      if constexpr (sizeof(real) == 4) {
-#pragma unroll
-        for (int c = 0; c < 6; ++c)
-          dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
-      } else {
-#pragma unroll
-        for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
-      }
-    }
-  }
+  for (int ca = 0; ca < 3; ++ca)
+    pauli_term_rows(t, ca, a, [&](int alpha, const double2 (&row)[12]) { store_dense_row<real>(Wt + (size_t)(3 * alpha + ca) * NC * kBlock, row); });
 }
 
 // ------------------------------------------------------------------------- step a2, the 18 two-link terms (dense layout)
@@ -690,6 +728,54 @@ __global__ void __launch_bounds__(32 * 4) pauli_store_kernel(const double2* __re
   }
 }
 
+// term 9..26 -> family, directions, sign and the spin coefficients of K (term order of ok.h)
+struct KronTerm {
+  int fam, i, j;
+  bool neg;
+  double kD, sk[3];   // D = kD 1 ; S = s1 sigma_1 + s2 sigma_2 + s3 sigma_3 (real coefficients)
+};
+__device__ __forceinline__ KronTerm kron_term_of(int term, const PrecalcArgs& a) {
+  KronTerm t;
+  t.j = 0;
+  if (term < 15) {
+    t.fam = 3; t.i = (term - 9) >> 1; t.neg = ((term - 9) & 1) != 0;
+  } else {
+    const int q = (term - 15) >> 2, w = (term - 15) & 3;
+    t.i = q == 2 ? 1 : 0;
+    t.j = q == 0 ? 1 : 2;
+    t.fam = w < 2 ? 4 : 5;
+    t.neg = (w & 1) != 0;
+  }
+  t.kD = t.fam == 3 ? a.dii : 0.0;
+  t.sk[0] = t.sk[1] = t.sk[2] = 0.0;
+  const double sgn = t.neg ? -1.0 : 1.0;
+  if (t.fam == 3) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) t.sk[d] = d == t.i ? sgn * a.sii : 0.0;
+  } else {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) t.sk[d] = d == t.i ? sgn * a.sij : (d == t.j ? sgn * (t.fam == 4 ? a.sij : -a.sij) : 0.0);
+  }
+  return t;
+}
+// spin row alpha of K = [[D, S], [S, D]], S2[al][be] = [[s3, s1 - i s2], [s1 + i s2, -s3]]: K[beta], beta = 2 bj + be
+__device__ __forceinline__ void kron_K_row(const KronTerm& t, int alpha, double2 (&K)[4]) {
+  const int bi = alpha >> 1, al = alpha & 1;
+#pragma unroll
+  for (int beta = 0; beta < 4; ++beta) {
+    const int bj = beta >> 1, be = beta & 1;
+    double2 v;
+    if (bi == bj) {
+      v = make_double2(al == be ? t.kD : 0.0, 0.0);
+    } else if (al == be) {
+      v = make_double2(al == 0 ? t.sk[2] : -t.sk[2], 0.0);
+    } else {
+      v = make_double2(t.sk[0], al == 0 ? -t.sk[1] : t.sk[1]);
+    }
+    K[beta] = v;
+  }
+}
+
 template <typename real>
 __global__ void __launch_bounds__(32 * 3) kron_terms_kernel(const double2* __restrict__ links, typename WUnit<real>::type* __restrict__ W,
                                                             PrecalcArgs a) {
@@ -705,52 +791,16 @@ __global__ void __launch_bounds__(32 * 3) kron_terms_kernel(const double2* __res
     for (int u = 0; u < 12 * NC; ++u) Wt[(size_t)u * kBlock] = z;
     return;
   }
-  // term -> family, directions, sign (term order of ok.h)
-  int fam, i, j = 0;
-  bool neg;
-  if (term < 15) {
-    fam = 3; i = (term - 9) >> 1; neg = ((term - 9) & 1) != 0;
-  } else {
-    const int q = (term - 15) >> 2, w = (term - 15) & 3;
-    i = q == 2 ? 1 : 0;
-    j = q == 0 ? 1 : 2;
-    fam = w < 2 ? 4 : 5;
-    neg = (w & 1) != 0;
-  }
+  const KronTerm t = kron_term_of(term, a);
   Site x = site_of(n, a.g);
-  if (neg)   // the positive blocks live at x + offset(term)
+  if (t.neg)   // the positive blocks live at x + offset(term)
     for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
-  cm3 P = two_link_P(links, x, fam, i, j, a);
-  if (neg) P = adj(P);
-  // spin structure: D = kD 1 ; S = s1 sigma_1 + s2 sigma_2 + s3 sigma_3 (real coefficients)
-  const double kD = fam == 3 ? a.dii : 0.0;
-  double sk[3] = {0.0, 0.0, 0.0};
-  const double sgn = neg ? -1.0 : 1.0;
-  if (fam == 3) {
-    sk[i] = sgn * a.sii;
-  } else {
-    sk[i] = sgn * a.sij;
-    sk[j] = sgn * (fam == 4 ? a.sij : -a.sij);
-  }
-  // S2[al][be]: [[s3, s1 - i s2], [s1 + i s2, -s3]]
+  cm3 P = two_link_P(links, x, t.fam, t.i, t.j, a);
+  if (t.neg) P = adj(P);
 #pragma unroll 1
   for (int alpha = 0; alpha < 4; ++alpha) {
-    const int bi = alpha >> 1, al = alpha & 1;
-    // this spin row's four coefficients K[alpha][beta], beta = 2 bj + be
     double2 K[4];
-#pragma unroll
-    for (int beta = 0; beta < 4; ++beta) {
-      const int bj = beta >> 1, be = beta & 1;
-      double2 v;
-      if (bi == bj) {
-        v = make_double2(al == be ? kD : 0.0, 0.0);
-      } else if (al == be) {
-        v = make_double2(al == 0 ? sk[2] : -sk[2], 0.0);
-      } else {
-        v = make_double2(sk[0], al == 0 ? -sk[1] : sk[1]);
-      }
-      K[beta] = v;
-    }
+    kron_K_row(t, alpha, K);
 #pragma unroll
     for (int ca = 0; ca < 3; ++ca) {
       double2 row[12];
@@ -758,80 +808,201 @@ __global__ void __launch_bounds__(32 * 3) kron_terms_kernel(const double2* __res
       for (int beta = 0; beta < 4; ++beta)
 #pragma unroll
         for (int cb = 0; cb < 3; ++cb) row[3 * beta + cb] = cmul(K[beta], P.e[3 * ca + cb]);
-      unit_t* dst = Wt + (size_t)(3 * alpha + ca) * NC * kBlock;
-      if constexpr (sizeof(real) == 4) {
-#pragma unroll
-        for (int c = 0; c < 6; ++c)
-          dst[(size_t)c * kBlock] = make_float4((float)row[2 * c].x, (float)row[2 * c].y, (float)row[2 * c + 1].x, (float)row[2 * c + 1].y);
-      } else {
-#pragma unroll
-        for (int c = 0; c < 12; ++c) dst[(size_t)c * kBlock] = row[c];
-      }
+      store_dense_row<real>(Wt + (size_t)(3 * alpha + ca) * NC * kBlock, row);
     }
   }
 }
 
 // ------------------------------------------------------------------------- 12-RHS tile writer
-// The 12-RHS W tile of a site (ok_internal.cuh) interleaves the four terms of a K stage inside 16-byte core-matrix rows,
-// so a (site, term) thread would write 8-byte pieces 31 KB apart.  Instead the dense fp32 W of a chunk of blocks is
-// assembled into a bounce buffer (workspace) and this kernel turns (block, stage) = 32 sites x 4 terms into the split-fp16
-// tile image in shared memory and writes every site's 4608-byte stage chunk with coalesced 16-byte stores
-// (CTA = 16 sites x one stage, 74 KB of smem, 3 CTAs per SM).
-constexpr int kTileSiteStride = kMrhsStageHalves * 2 + 16;   // bytes per site in smem (+16: spreads the sites over banks)
-constexpr int kTileSites = 16;                                // sites per CTA (half a block): 3 CTAs per SM overlap their phases
-constexpr int kTileSmem = kTileSites * kTileSiteStride;       // 73 984
-constexpr int kBounceBlockBytes = kBlock * kTerms * 144 * 8;  // dense fp32 W of one 32-site block
-constexpr int kBounceBlocksMax = 2048;                        // 2 GB chunks at most
-
-constexpr int kTileThreads = 256;
-
-__global__ void __launch_bounds__(kTileThreads) mrhs_tile_kernel(const float4* __restrict__ dense, __half* __restrict__ tiles, int blk0, int V) {
-  extern __shared__ __align__(16) uint8_t sm[];
-  const int blk = blockIdx.x >> 1, half = blockIdx.x & 1, stage = blockIdx.y, tid = threadIdx.x;
-  const int nterm = stage < 6 ? 4 : 3;
-  if (stage == 6) {   // the pad k = 36..39 of the last stage stays zero
-    for (int i = tid; i < kTileSmem / 16; i += kTileThreads) reinterpret_cast<uint4*>(sm)[i] = make_uint4(0u, 0u, 0u, 0u);
-    __syncthreads();
-  }
-  // 16 threads per dense row [term][row][unit] (one half of its 32 sites): thread <-> site; the two columns of a unit are adjacent k, so every
-  // (part, piece) is one 4-byte store into the site's tile image
-  const int lane = tid & (kTileSites - 1), grp = tid / kTileSites;
-  uint8_t* mine = sm + lane * kTileSiteStride;
-  for (int c = grp; c < nterm * 72; c += kTileThreads / kTileSites) {
-    const int u = c % 6, row = (c / 6) % 12, tl = c / 72;
-    const int term = 4 * stage + tl;
-    const float4 v = __ldcs(dense + (((size_t)blk * kTerms + term) * 12 + row) * 6 * kBlock + u * kBlock + half * kTileSites + lane);
-    int k;   // K position of column 2u inside the stage (ok_internal.cuh: mrhs_k); column 2u + 1 is k + 1
-    if (stage < 6) k = 16 * (u >> 1) + 4 * tl + 2 * (u & 1);
-    else { const int sq = 3 * tl + (u >> 1); k = 16 * (sq >> 2) + 4 * (sq & 3) + 2 * (u & 1); }
-    const int kofs = (k >> 3) * 384 + (k & 7);
-    const float vals[2][2] = {{v.x, v.z}, {v.y, v.w}};   // [part][column 2u, 2u + 1]
+// The 12-RHS W tile of a site (ok_internal.cuh) interleaves the four terms of a K stage inside 16-byte core-matrix rows, so a
+// (site, term) thread would write 8-byte pieces 31 KB apart.  mrhs_tiles_kernel computes the entries where they are needed
+// instead: one CTA = one 32-site block x one HALF stage (two stencil terms = the even or the odd 768-byte k chunks of the
+// stage: 3 x 768 B per site), one thread per (site, term, colour row ca).  A thread forms its four spin rows (alpha, ca) --
+// terms 0..8 by pauli_term_rows, terms 9..26 as K (x) (row ca of P) -- rounds them once to fp32 exactly as the dense layout
+// does, splits every number into its two fp16 pieces and puts them into the site's tile image in shared memory (74 KB, two
+// CTAs per SM); the CTA then writes the images with coalesced 16-byte stores.  The last stage (three terms, 5 k chunks, its
+// K order differs) is done by two CTAs of 16 sites x 3 terms.  No dense intermediate, no workspace beyond the scratch fields.
+struct LinkRef {
+  const double2* p;   // element e at p[e Vpad]
+  double sg;          // boundary sign
+  bool dag;
+};
+__device__ __forceinline__ LinkRef link_ref(const double2* __restrict__ links, const Site& s, int mu, bool dag, const PrecalcArgs& a) {
+  LinkRef L;
+  L.p = links + (size_t)(9 * mu) * a.Vpad + index_of(s, a.g);
+  L.sg = (a.bc[mu] < 0 && s.c[mu] == (mu == 3 ? a.tfold : a.g.L[mu] - 1)) ? -1.0 : 1.0;
+  L.dag = dag;
+  return L;
+}
+__device__ __forceinline__ double2 link_el(const LinkRef& L, int r, int c, int Vpad) {   // element (r, c) of U or U^dag
+  const double2 v = __ldg(L.p + (size_t)(L.dag ? 3 * c + r : 3 * r + c) * Vpad);
+  return make_double2(L.sg * v.x, L.dag ? -L.sg * v.y : L.sg * v.y);
+}
+// out[t] += (X Y)[ca][t]  (tr = false)   or   (X Y)[t][ca]  (tr = true: the caller conjugates, row ca of (X Y)^dag)
+__device__ __forceinline__ void acc_prod_line(double2 (&out)[3], const LinkRef& X, const LinkRef& Y, bool tr, int ca, int Vpad) {
+  double2 v[3];
 #pragma unroll
-    for (int part = 0; part < 2; ++part) {
-      __half h0, l0, h1, l1;
-      mrhs_split(vals[part][0], &h0, &l0);
-      mrhs_split(vals[part][1], &h1, &l1);
-      const int w = mrhs_W_row(row, part);
-      *reinterpret_cast<__half2*>(mine + 2 * (kofs + (w >> 3) * 64 + (w & 7) * 8)) = __halves2half2(h0, h1);
-      *reinterpret_cast<__half2*>(mine + 2 * (kofs + ((w + 24) >> 3) * 64 + ((w + 24) & 7) * 8)) = __halves2half2(l0, l1);
+  for (int m = 0; m < 3; ++m) v[m] = tr ? link_el(Y, m, ca, Vpad) : link_el(X, ca, m, Vpad);
+#pragma unroll
+  for (int t = 0; t < 3; ++t)
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      const double2 b = tr ? link_el(X, t, m, Vpad) : link_el(Y, m, t, Vpad);
+      const double2 q = cmul(v[m], b);
+      out[t].x += q.x;
+      out[t].y += q.y;
     }
+}
+// row ca of the colour matrix of a two-link term (two_link_P at x, or its adjoint for an opposite-direction term)
+__device__ __forceinline__ void two_link_P_row(const double2* __restrict__ links, const Site& x, const KronTerm& t, int ca, const PrecalcArgs& a,
+                                               double2 (&P)[3]) {
+  const int i = t.i, j = t.j;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) P[c] = make_double2(0.0, 0.0);
+  if (t.fam == 3) {
+    acc_prod_line(P, link_ref(links, x, i, false, a), link_ref(links, shift(x, i, 1, a.g), i, false, a), t.neg, ca, a.Vpad);
+  } else if (t.fam == 4) {
+    acc_prod_line(P, link_ref(links, x, i, false, a), link_ref(links, shift(x, i, 1, a.g), j, false, a), t.neg, ca, a.Vpad);
+    acc_prod_line(P, link_ref(links, x, j, false, a), link_ref(links, shift(x, j, 1, a.g), i, false, a), t.neg, ca, a.Vpad);
+  } else {
+    const Site xmj = shift(x, j, -1, a.g);
+    acc_prod_line(P, link_ref(links, x, i, false, a), link_ref(links, shift(xmj, i, 1, a.g), j, true, a), t.neg, ca, a.Vpad);
+    acc_prod_line(P, link_ref(links, xmj, j, true, a), link_ref(links, xmj, i, false, a), t.neg, ca, a.Vpad);
   }
-  __syncthreads();
-  const int units = (stage < 6 ? kMrhsStageHalves * 2 : kMrhsStageHalves * 2 - 768) / 16;   // the all-pad k chunk 5 of stage 6 is not stored
-  for (int i = tid; i < kTileSites * units; i += kTileThreads) {
-    const int s = i / units, q = i - s * units;
-    const long long n = (long long)(blk0 + blk) * kBlock + half * kTileSites + s;
-    if (n < V)
-      reinterpret_cast<uint4*>(tiles + n * kMrhsWSiteHalves + stage * kMrhsStageHalves)[q] = reinterpret_cast<const uint4*>(sm + s * kTileSiteStride)[q];
+  if (t.neg) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) P[c].y = -P[c].y;
   }
 }
 
-static int mrhs_bounce_blocks(const Geom& g) { return g.nblk < kBounceBlocksMax ? g.nblk : kBounceBlocksMax; }
+// the 24 complex numbers of pauli_term_tables as fp16 pieces: [0 = D, 1 = S][combo][cb] -> (Re, Im) as __half2
+struct HalfTab {
+  uint32_t hi[2][4][3], lo[2][4][3];
+};
+// one complex number, rounded once to fp32 (as the dense layout stores it), then split as mrhs_split does
+__device__ __forceinline__ void split_cx(const double2& v, uint32_t& hi, uint32_t& lo) {
+  const float fx = (float)v.x, fy = (float)v.y;
+  const __half2 h = __floats2half2_rn(fx, fy);
+  const float2 b = __half22float2(h);
+  const __half2 l = __floats2half2_rn((fx - b.x) * kMrhsLoScale, (fy - b.y) * kMrhsLoScale);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
+}
+
+constexpr int kTilesThreads = 192;                               // 32 sites x 2 terms x 3 colour rows
+constexpr int kTilesHalfBytes = 3 * 768;                         // a half stage of one site: its 3 k chunks
+constexpr int kTilesLastBytes = 5 * 768;                         // stage 6 of one site (the all-pad k chunk 5 is not stored)
+constexpr int kTilesSmem = kBlock * (kTilesHalfBytes + 16);      // 74 240 (>= 16 x (3840 + 16)); + 16: odd multiple of 16 B between sites
+
+// LAST = false: grid (blocks, 12 half stages), CTA = 32 sites x 2 terms.  LAST = true: grid (blocks, 2), CTA = 16 sites x the 3 terms of stage 6.
+template <bool LAST>
+__global__ void __launch_bounds__(kTilesThreads, 2) mrhs_tiles_kernel(const double2* __restrict__ links, const cm3* __restrict__ FS,
+                                                                       __half* __restrict__ tiles, PrecalcArgs a) {
+  extern __shared__ __align__(16) uint8_t sm[];
+  const int tid = threadIdx.x, blk = blockIdx.x, h = blockIdx.y;
+  constexpr int nsite = LAST ? 16 : 32, nterm = LAST ? 3 : 2;
+  constexpr int stride = (LAST ? kTilesLastBytes : kTilesHalfBytes) + 16;
+  const int stage = LAST ? 6 : h >> 1;
+  const int s = tid & (nsite - 1), item = tid / nsite;          // item = 3 tl + ca
+  const int site0 = blk * kBlock + (LAST ? h * 16 : 0);
+  if (LAST) {   // the pad k = 36..39 of the last stage stays zero
+    for (int q = tid; q < nsite * stride / 16; q += kTilesThreads) reinterpret_cast<uint4*>(sm)[q] = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+  }
+  const int n = site0 + s;
+  if (item < 3 * nterm && n < a.g.V) {
+    const int tl = item / 3, ca = item - 3 * tl;
+    const int term = LAST ? 24 + tl : 4 * stage + 2 * (h & 1) + tl;
+    HalfTab T;
+    uint32_t mUL = 0xffffffffu, mLR = 0xffffffffu, sLL = 0u;   // zero / sign masks of the UL, LR, LL blocks
+    if (term < 9) {
+      const PauliTerm t = pauli_term_of(term, n, links, FS, a);
+      double2 Dv[4][3], Sv[4][3];
+      pauli_term_tables(t, ca, a, Dv, Sv);
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int cb = 0; cb < 3; ++cb) {
+          split_cx(Dv[c][cb], T.hi[0][c][cb], T.lo[0][c][cb]);
+          split_cx(Sv[c][cb], T.hi[1][c][cb], T.lo[1][c][cb]);
+        }
+      mUL = t.ulA ? 0xffffffffu : 0u;
+      mLR = t.lrA ? 0xffffffffu : 0u;
+      sLL = t.llsgn < 0.0 ? 0x80008000u : 0u;
+    } else {   // W = K (x) P: D = kD 1 (x) P, S = (s1 sigma_1 + s2 sigma_2 + s3 sigma_3) (x) P
+      const KronTerm t = kron_term_of(term, a);
+      Site x = site_of(n, a.g);
+      if (t.neg)
+        for (int mu = 0; mu < 4; ++mu) x = shift(x, mu, c_poff[term][mu], a.g);
+      double2 P[3];
+      two_link_P_row(links, x, t, ca, a, P);
+#pragma unroll
+      for (int cb = 0; cb < 3; ++cb) {
+        split_cx(make_double2(t.kD * P[cb].x, t.kD * P[cb].y), T.hi[0][0][cb], T.lo[0][0][cb]);
+        T.hi[0][1][cb] = T.hi[0][0][cb]; T.lo[0][1][cb] = T.lo[0][0][cb];
+        T.hi[0][2][cb] = T.hi[0][3][cb] = T.lo[0][2][cb] = T.lo[0][3][cb] = 0u;
+        split_cx(make_double2(t.sk[2] * P[cb].x, t.sk[2] * P[cb].y), T.hi[1][0][cb], T.lo[1][0][cb]);
+        T.hi[1][1][cb] = T.hi[1][0][cb] ^ 0x80008000u; T.lo[1][1][cb] = T.lo[1][0][cb] ^ 0x80008000u;
+        split_cx(cmul(make_double2(t.sk[0], -t.sk[1]), P[cb]), T.hi[1][2][cb], T.lo[1][2][cb]);
+        split_cx(cmul(make_double2(t.sk[0], t.sk[1]), P[cb]), T.hi[1][3][cb], T.lo[1][3][cb]);
+      }
+    }
+    // The image of a site in 8-byte slots: [k chunk][row group w48/8 : 6][w48 % 8][k % 8 / 4]; a slot holds columns 4g .. 4g + 3 of
+    // one term.  Sites 8 apart share their banks: the odd ones among them swap the two slots of every 16 bytes.
+    uint2* mine = reinterpret_cast<uint2*>(sm + s * stride);
+    const int swz = (s >> 3) & 1;
+    int gslot[3];
+#pragma unroll
+    for (int g = 0; g < 3; ++g) {
+      if (LAST) { const int sq = 3 * tl + g; gslot[g] = (2 * (sq >> 2) + ((sq & 3) >> 1)) * 96 + ((sq & 1) ^ swz); }
+      else gslot[g] = g * 96 + (tl ^ swz);
+    }
+#pragma unroll
+    for (int alpha = 0; alpha < 4; ++alpha) {
+      const int r = 3 * alpha + ca, bi = alpha >> 1, al = alpha & 1;
+      uint2* rowp = mine + (r >> 2) * 16 + (r & 3) * 4;   // B rows w = 8 (r / 4) + 2 (r % 4) + part (hi) and w + 24 (lo)
+#pragma unroll
+      for (int g = 0; g < 3; ++g) {
+        uint2* dst = rowp + gslot[g];
+#pragma unroll
+        for (int hl = 0; hl < 2; ++hl)
+#pragma unroll
+          for (int part = 0; part < 2; ++part) {
+            uint32_t w[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {   // columns 4 g + 2 e and the next
+              const int c0 = 4 * g + 2 * e, c1 = c0 + 1;
+              const int be0 = c0 / 3, cb0 = c0 % 3, be1 = c1 / 3, cb1 = c1 % 3;
+              const int bj = be0 >> 1;      // = be1 >> 1: a column pair never straddles the spin blocks
+              const int ds = bi == bj ? 0 : 1;
+              const int k0 = al == (be0 & 1) ? al : (al == 0 ? 2 : 3), k1 = al == (be1 & 1) ? al : (al == 0 ? 2 : 3);
+              const uint32_t v0 = hl ? T.lo[ds][k0][cb0] : T.hi[ds][k0][cb0], v1 = hl ? T.lo[ds][k1][cb1] : T.hi[ds][k1][cb1];
+              uint32_t v = __byte_perm(v0, v1, part ? 0x7632 : 0x5410);
+              if (ds == 0) v &= bi == 0 ? mUL : mLR;
+              else if (bi == 1) v ^= sLL;
+              w[e] = v;
+            }
+            dst[hl * 48 + part * 2] = make_uint2(w[0], w[1]);
+          }
+      }
+    }
+  }
+  __syncthreads();
+  constexpr int units = (stride - 16) / 16;   // 16-byte units per site: 144 (3 pieces of 48) or 240 (contiguous)
+  for (int q = tid; q < nsite * units; q += kTilesThreads) {
+    const int ss = q / units, u = q - ss * units;
+    const long long nn = (long long)site0 + ss;
+    if (nn >= a.g.V) continue;
+    uint4 v = *reinterpret_cast<const uint4*>(sm + ss * stride + u * 16);
+    if ((ss >> 3) & 1) { uint32_t t0 = v.x; v.x = v.z; v.z = t0; t0 = v.y; v.y = v.w; v.w = t0; }
+    const int ofs = LAST ? u : (2 * (u / 48) + (h & 1)) * 48 + u % 48;   // 16-byte unit inside the stage
+    reinterpret_cast<uint4*>(tiles + nn * kMrhsWSiteHalves + stage * kMrhsStageHalves)[ofs] = v;
+  }
+}
 
 size_t precalc_work_bytes(const ok_params* p) {
   Geom g = make_geom(p);
-  const size_t fs = (size_t)(6 + kHopMats + 4) * g.nblk * kBlock * sizeof(cm3);
-  return p->nrhs == 12 ? fs + 256 + (size_t)mrhs_bounce_blocks(g) * kBounceBlockBytes : fs;
+  return (size_t)(6 + kHopMats + 4) * g.nblk * kBlock * sizeof(cm3);
 }
 
 int launch_precalc(const ok_params* p, const void* links, void* Wp, void* work) {
@@ -903,23 +1074,17 @@ int launch_precalc_window(const ok_params* p, const void* links, void* Wp, void*
     OK_LAUNCHED("kron_terms_kernel");                                                                                       \
   } while (0)
   a.blk0 = 0;
-  if (a.mrhs) {   // dense fp32 W of a chunk of blocks -> bounce buffer -> split-fp16 tiles (mrhs_tile_kernel)
+  if (a.mrhs) {   // the split-fp16 tiles straight from the scratch fields and links
     static bool attr_set = false;
     if (!attr_set) {
-      OK_CUDA(cudaFuncSetAttribute(mrhs_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTileSmem));
+      OK_CUDA(cudaFuncSetAttribute(mrhs_tiles_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTilesSmem));
+      OK_CUDA(cudaFuncSetAttribute(mrhs_tiles_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kTilesSmem));
       attr_set = true;
     }
-    const size_t fs = ((size_t)(6 + kHopMats + 4) * a.g.nblk * kBlock * sizeof(cm3) + 255) / 256 * 256;
-    void* bounce = static_cast<char*>(work) + fs;
-    const int cap = mrhs_bounce_blocks(a.g);
-    for (int b0 = 0; b0 < a.g.nblk; b0 += cap) {
-      const int nb = a.g.nblk - b0 < cap ? a.g.nblk - b0 : cap;
-      a.blk0 = b0;
-      OK_PAULI_LAUNCH(nb, bounce);
-      OK_KRON_LAUNCH(nb, bounce);
-      mrhs_tile_kernel<<<dim3(2 * nb, kMrhsStages), kTileThreads, kTileSmem, st>>>(static_cast<const float4*>(bounce), static_cast<__half*>(Wp), b0, a.g.V);
-      OK_LAUNCHED("mrhs_tile_kernel");
-    }
+    mrhs_tiles_kernel<false><<<dim3(a.g.nblk, 12), kTilesThreads, kTilesSmem, st>>>(lk, FS, static_cast<__half*>(Wp), a);
+    OK_LAUNCHED("mrhs_tiles_kernel");
+    mrhs_tiles_kernel<true><<<dim3(a.g.nblk, 2), kTilesThreads, kTilesSmem, st>>>(lk, FS, static_cast<__half*>(Wp), a);
+    OK_LAUNCHED("mrhs_tiles_kernel");
     return OK_SUCCESS;
   }
   const int nb = win_nblk < 0 ? a.g.nblk : win_nblk;
