@@ -905,9 +905,11 @@ __global__ void __launch_bounds__(kTilesThreads, 2) mrhs_tiles_kernel(const doub
   const int stage = LAST ? 6 : h >> 1;
   const int s = tid & (nsite - 1), item = tid / nsite;          // item = 3 tl + ca
   const int site0 = blk * kBlock + (LAST ? h * 16 : 0);
-  if (LAST) {   // the pad k = 36..39 of the last stage stays zero
-    for (int q = tid; q < nsite * stride / 16; q += kTilesThreads) reinterpret_cast<uint4*>(sm)[q] = make_uint4(0u, 0u, 0u, 0u);
-    __syncthreads();
+  if (LAST) {   // the pad k = 36..39 of the last stage (the second slot of every row of k chunk 4) is zero; no thread below writes it
+    for (int q = tid; q < nsite * 48; q += kTilesThreads) {
+      const int zs = q / 48, row = q - 48 * zs;
+      reinterpret_cast<uint2*>(sm + zs * stride)[4 * 96 + 2 * row + (1 ^ ((zs >> 3) & 1))] = make_uint2(0u, 0u);
+    }
   }
   const int n = site0 + s;
   if (item < 3 * nterm && n < a.g.V) {
@@ -988,15 +990,23 @@ __global__ void __launch_bounds__(kTilesThreads, 2) mrhs_tiles_kernel(const doub
     }
   }
   __syncthreads();
-  constexpr int units = (stride - 16) / 16;   // 16-byte units per site: 144 (3 pieces of 48) or 240 (contiguous)
-  for (int q = tid; q < nsite * units; q += kTilesThreads) {
-    const int ss = q / units, u = q - ss * units;
-    const long long nn = (long long)site0 + ss;
-    if (nn >= a.g.V) continue;
-    uint4 v = *reinterpret_cast<const uint4*>(sm + ss * stride + u * 16);
-    if ((ss >> 3) & 1) { uint32_t t0 = v.x; v.x = v.z; v.z = t0; t0 = v.y; v.y = v.w; v.w = t0; }
-    const int ofs = LAST ? u : (2 * (u / 48) + (h & 1)) * 48 + u % 48;   // 16-byte unit inside the stage
-    reinterpret_cast<uint4*>(tiles + nn * kMrhsWSiteHalves + stage * kMrhsStageHalves)[ofs] = v;
+  // images -> tiles in 768-byte pieces (48 x 16 B): thread = (16-byte unit u of a piece, site ss = pp, pp + 4, ...); half stage: the
+  // 3 pieces are the even or the odd k chunks of the stage, last stage: 5 contiguous pieces
+  constexpr int npiece = LAST ? 5 : 3;
+  const int u = tid % 48, pp = tid / 48;
+  const uint8_t* src = sm + pp * stride + u * 16;
+  uint8_t* dstg = reinterpret_cast<uint8_t*>(tiles) + ((size_t)(site0 + pp) * kMrhsWSiteHalves + (size_t)stage * kMrhsStageHalves) * 2 +
+                  (LAST ? 0 : (h & 1) * 768) + u * 16;
+#pragma unroll 2
+  for (int ss = pp; ss < nsite; ss += 4, src += 4 * stride, dstg += (size_t)4 * kMrhsWSiteBytes) {
+    if (site0 + ss >= a.g.V) break;
+    const bool swp = (ss >> 3) & 1;
+#pragma unroll
+    for (int g = 0; g < npiece; ++g) {
+      uint4 v = *reinterpret_cast<const uint4*>(src + g * 768);
+      if (swp) { uint32_t t0 = v.x; v.x = v.z; v.z = t0; t0 = v.y; v.y = v.w; v.w = t0; }
+      *reinterpret_cast<uint4*>(dstg + g * (LAST ? 768 : 1536)) = v;
+    }
   }
 }
 
