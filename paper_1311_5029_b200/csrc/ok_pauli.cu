@@ -29,6 +29,9 @@ namespace {
 
 constexpr int kPauliMats = OK_W_PAULI_MATS;   // 37
 constexpr int kMaxUses = 80;
+#ifndef OK_PAULI_MINB
+#define OK_PAULI_MINB 4
+#endif
 #ifndef OK_PAULI_PARTS
 #define OK_PAULI_PARTS 2
 #endif
@@ -173,9 +176,9 @@ struct PState {
   using vec = typename PV<real>::vec;
   cx acc[12];
   cx phi[12];
+  uint32_t ring;    // fp32 only: shared-memory address of this lane's column of the warp's matrix ring (see use_ct)
   const cx* W;
   const vec* psi;
-  const cx* Wn;     // matrices of the current use's site (own site, or the neighbour for an opposite-direction term)
   int n, x, y, z, t;
   int L0, L1, L2, L3;
 };
@@ -184,7 +187,19 @@ template <int BASE, int SIGMA, typename cx, typename real>
 __device__ __forceinline__ void place_ct(cx (&acc)[12], const cx (&tv)[2][3], real c) {
 #pragma unroll
   for (int ca = 0; ca < 3; ++ca) {
-    if constexpr (SIGMA == 0 || SIGMA == 3) {
+    if constexpr (sizeof(real) == 4) {   // packed: (Re, Im) of one output component per FFMA2
+      if constexpr (SIGMA == 0 || SIGMA == 3) {
+        const float c1 = SIGMA == 3 ? -c : c;
+        acc[BASE + ca] = __ffma2_rn(make_float2(c, c), tv[0][ca], acc[BASE + ca]);
+        acc[BASE + 3 + ca] = __ffma2_rn(make_float2(c1, c1), tv[1][ca], acc[BASE + 3 + ca]);
+      } else if constexpr (SIGMA == 1) {
+        acc[BASE + ca] = __ffma2_rn(make_float2(c, c), tv[1][ca], acc[BASE + ca]);
+        acc[BASE + 3 + ca] = __ffma2_rn(make_float2(c, c), tv[0][ca], acc[BASE + 3 + ca]);
+      } else {                            // sigma_y: -i v below the diagonal, +i v above: (v.y, -v.x) and (-v.y, v.x)
+        acc[BASE + ca] = __ffma2_rn(make_float2(c, -c), make_float2(tv[1][ca].y, tv[1][ca].x), acc[BASE + ca]);
+        acc[BASE + 3 + ca] = __ffma2_rn(make_float2(-c, c), make_float2(tv[0][ca].y, tv[0][ca].x), acc[BASE + 3 + ca]);
+      }
+    } else if constexpr (SIGMA == 0 || SIGMA == 3) {
       const real c1 = SIGMA == 3 ? -c : c;
       acc[BASE + ca].x = fma(c, tv[0][ca].x, acc[BASE + ca].x);
       acc[BASE + ca].y = fma(c, tv[0][ca].y, acc[BASE + ca].y);
@@ -216,19 +231,70 @@ __device__ __forceinline__ void placement_ct(PState<real>& st, const typename PV
   }
 }
 
-// one use; FIRST: first use of this warp's range (a new term starts there by construction)
-template <typename real, int U, bool FIRST, bool MASS>
+// site index of x + offset(term T)
+template <typename real, int T>
+__device__ __forceinline__ int neighbour_ct(const PState<real>& st) {
+  if constexpr (T == 0) return st.n;
+  const int xx = wrapp(st.x + kOffC[T][0], st.L0), yy = wrapp(st.y + kOffC[T][1], st.L1);
+  const int zz = wrapp(st.z + kOffC[T][2], st.L2), tt = wrapp(st.t + kOffC[T][3], st.L3);
+  return xx + st.L0 * (yy + st.L1 * (zz + st.L2 * tt));
+}
+// where use U's stored matrix lives (own site, or the neighbour's for an opposite-direction term): element e at [e kBlock]
+template <typename real, int U>
+__device__ __forceinline__ const typename PV<real>::cx* matrix_ptr_ct(const PState<real>& st) {
+  constexpr Use u = kUses.u[U];
+  const int nm = u.adj ? neighbour_ct<real, u.term>(st) : st.n;
+  return st.W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31) + (size_t)(9 * u.m) * kBlock;
+}
+// fp32: the matrices reach the FMAs through a per-warp ring in shared memory filled by asynchronous 8-byte copies
+// (cp.async, SASS LDGSTS): with packed FMAs a use is ~150 issue slots, too short to hide an L2 / HBM round trip behind the
+// four warps of a scheduler, and registers cannot hold several uses in flight.  Every lane copies and later reads only its own
+// site's elements, so no barrier is needed: cp.async.wait_group orders a lane's reads after its own copies.
+constexpr int kRingDepth = 4;                         // uses in flight per warp
+constexpr int kRingSlotBytes = 9 * kBlock * 8;        // one 3x3 complex fp32 matrix for 32 sites
+template <int U>
+__device__ __forceinline__ void ring_issue_ct(const PState<float>& st, int slot) {
+  const float2* p = matrix_ptr_ct<float, U>(st);
+#pragma unroll
+  for (int e = 0; e < 9; ++e)
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st.ring + slot * kRingSlotBytes + e * (kBlock * 8)), "l"(p + (size_t)e * kBlock)
+                 : "memory");
+}
+
+template <int U, int UEND, int D>
+__device__ __forceinline__ void ring_prologue_ct(const PState<float>& st) {   // the first kRingDepth uses of the range: D = slot
+  if constexpr (D < kRingDepth) {
+    if constexpr (U < UEND) ring_issue_ct<U>(st, D);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    ring_prologue_ct<U + 1, UEND, D + 1>(st);
+  }
+}
+
+// one use; FIRST: first use of this warp's range (a new term starts there by construction); UEND: end of the range
+template <typename real, int U, int UBEG, int UEND, bool MASS>
 __device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
+  constexpr bool FIRST = U == UBEG;
   using cx = typename PV<real>::cx;
   using vec = typename PV<real>::vec;
   constexpr int NC = PV<real>::NC;
   constexpr Use u = kUses.u[U];
   constexpr bool newterm = FIRST || kUses.u[U > 0 ? U - 1 : 0].term != u.term;
+  cx C[9];
+  if constexpr (sizeof(real) == 4) {
+    if constexpr (FIRST) ring_prologue_ct<U, UEND, 0>(st);
+    asm volatile("cp.async.wait_group %0;" ::"n"(kRingDepth - 1) : "memory");
+    constexpr int slot = (U - UBEG) % kRingDepth;
+#pragma unroll
+    for (int e = 0; e < 9; ++e)
+      asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(C[e].x), "=f"(C[e].y) : "r"(st.ring + slot * kRingSlotBytes + e * (kBlock * 8)) : "memory");
+  } else {
+    const cx* p = matrix_ptr_ct<real, U>(st);
+#pragma unroll
+    for (int e = 0; e < 9; ++e) C[e] = __ldg(p + (size_t)e * kBlock);
+  }
   if constexpr (newterm) {
     constexpr int T = u.term;
-    const int xx = wrapp(st.x + kOffC[T][0], st.L0), yy = wrapp(st.y + kOffC[T][1], st.L1);
-    const int zz = wrapp(st.z + kOffC[T][2], st.L2), tt = wrapp(st.t + kOffC[T][3], st.L3);
-    const int nn = T == 0 ? st.n : xx + st.L0 * (yy + st.L1 * (zz + st.L2 * tt));
+    const int nn = neighbour_ct<real, T>(st);
     const vec* sp = st.psi + (size_t)(nn >> 5) * NC * kBlock + (nn & 31);
     if constexpr (sizeof(real) == 4) {
 #pragma unroll
@@ -241,16 +307,40 @@ __device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
 #pragma unroll
       for (int c = 0; c < 12; ++c) st.phi[c] = __ldg(sp + c * kBlock);
     }
-    const int nm = u.adj ? nn : st.n;
-    st.Wn = st.W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31);
     if constexpr (MASS && T == 0) {
 #pragma unroll
       for (int r = 0; r < 12; ++r) { st.acc[r].x += mass * st.phi[r].x; st.acc[r].y += mass * st.phi[r].y; }
     }
   }
-  cx C[9];
+  if constexpr (sizeof(real) == 4) {
+    // fp32: packed FMAs (fma.rn.f32x2, SASS FFMA2: two fp32 FMAs per issue slot on sm_100; one operand may be a broadcast scalar,
+    // the other may be read with its halves swapped).  With w = C[ca][cb] (or C[cb][ca] for the adjoint) and v = (v.x, v.y):
+    //   A += w.x (v.x, v.y) ,  B += w.y (v.y, v.x)   and   w v = A + (-B.x, B.y) ,  conj(w) v = A + (B.x, -B.y)
 #pragma unroll
-  for (int e = 0; e < 9; ++e) C[e] = __ldg(st.Wn + (size_t)(9 * u.m + e) * kBlock);
+    for (int h = 0; h < 2; ++h) {
+      cx tv[2][3];
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int ca = 0; ca < 3; ++ca) {
+          float2 A = make_float2(0.f, 0.f), B = make_float2(0.f, 0.f);
+#pragma unroll
+          for (int cb = 0; cb < 3; ++cb) {
+            const cx w = u.adj != 0 ? C[3 * cb + ca] : C[3 * ca + cb];
+            const cx v = st.phi[3 * (2 * h + s) + cb];
+            A = __ffma2_rn(make_float2(w.x, w.x), v, A);
+            B = __ffma2_rn(make_float2(w.y, w.y), make_float2(v.y, v.x), B);
+          }
+          tv[s][ca] = __ffma2_rn(B, u.adj != 0 ? make_float2(1.f, -1.f) : make_float2(-1.f, 1.f), A);
+        }
+      if (h == 0) { placement_ct<real, U, 0, 0>(st, tv); placement_ct<real, U, 1, 0>(st, tv); }
+      else { placement_ct<real, U, 0, 1>(st, tv); placement_ct<real, U, 1, 1>(st, tv); }
+    }
+    // this use's slot is free (its values are in registers and consumed): refill it kRingDepth uses ahead
+    if constexpr (U + kRingDepth < UEND) ring_issue_ct<U + kRingDepth>(st, (U - UBEG) % kRingDepth);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    return;
+  }
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     cx tv[2][3];
@@ -279,11 +369,11 @@ __device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
   }
 }
 
-template <typename real, int U, int UEND, bool FIRST, bool MASS>
+template <typename real, int U, int UBEG, int UEND, bool MASS>
 __device__ __forceinline__ void run_uses(PState<real>& st, real mass) {
   if constexpr (U < UEND) {
-    use_ct<real, U, FIRST, MASS>(st, mass);
-    run_uses<real, U + 1, UEND, false, MASS>(st, mass);
+    use_ct<real, U, UBEG, UEND, MASS>(st, mass);
+    run_uses<real, U + 1, UBEG, UEND, MASS>(st, mass);
   }
 }
 
@@ -293,7 +383,7 @@ __device__ __forceinline__ void run_uses(PState<real>& st, real mass) {
 // writes out (with the mass term), the later parts add to it, the last one also does the fused BiCGStab reductions; launches
 // on one stream are ordered, so the sum has a fixed order.  lane <-> site, one warp per 32-site block, four blocks per CTA.
 template <typename real, int PART, bool DOT>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, sizeof(real) == 4 ? OK_PAULI_MINB : 1)
 apply_pauli_part_kernel(const typename PV<real>::cx* __restrict__ W, const typename PV<real>::vec* __restrict__ psi,
                         typename PV<real>::vec* __restrict__ out, PauliArgs a, const typename PV<real>::vec* __restrict__ dot_a,
                         double* __restrict__ partials) {
@@ -315,7 +405,11 @@ apply_pauli_part_kernel(const typename PV<real>::cx* __restrict__ W, const typen
   q /= st.L1;
   st.z = q % st.L2;
   st.t = q / st.L2;
-  st.W = W; st.psi = psi; st.Wn = W;
+  st.W = W; st.psi = psi;
+  if constexpr (sizeof(real) == 4) {
+    extern __shared__ __align__(16) uint8_t pauli_ring[];
+    st.ring = (uint32_t)__cvta_generic_to_shared(pauli_ring) + (threadIdx.x >> 5) * (kRingDepth * kRingSlotBytes) + lane * 8;
+  }
   vec* ob = out + (size_t)blk * NC * kBlock + lane;
   if constexpr (PART == 0) {
 #pragma unroll
@@ -331,7 +425,7 @@ apply_pauli_part_kernel(const typename PV<real>::cx* __restrict__ W, const typen
 #pragma unroll
     for (int c = 0; c < 12; ++c) st.acc[c] = ob[c * kBlock];
   }
-  run_uses<real, kUses.first[PART], kUses.first[PART + 1], true, PART == 0>(st, (real)a.mass);
+  run_uses<real, kUses.first[PART], kUses.first[PART], kUses.first[PART + 1], PART == 0>(st, (real)a.mass);
   if (!live) {
 #pragma unroll
     for (int r = 0; r < 12; ++r) st.acc[r] = cx{0, 0};
@@ -463,8 +557,9 @@ template <typename real, int PART>
 int launch_parts(unsigned grid, cudaStream_t st, const typename PV<real>::cx* W, const typename PV<real>::vec* psi, typename PV<real>::vec* out,
                  const PauliArgs& a, const typename PV<real>::vec* dot_a, double* partials) {
   if constexpr (PART < kPauliParts) {
-    if (PART == kPauliParts - 1 && partials) apply_pauli_part_kernel<real, PART, true><<<grid, 128, 0, st>>>(W, psi, out, a, dot_a, partials);
-    else apply_pauli_part_kernel<real, PART, false><<<grid, 128, 0, st>>>(W, psi, out, a, nullptr, nullptr);
+    constexpr size_t smem = sizeof(real) == 4 ? 4 * kRingDepth * kRingSlotBytes : 0;   // 4 warps x ring (36 864 B: below the 48 KB default)
+    if (PART == kPauliParts - 1 && partials) apply_pauli_part_kernel<real, PART, true><<<grid, 128, smem, st>>>(W, psi, out, a, dot_a, partials);
+    else apply_pauli_part_kernel<real, PART, false><<<grid, 128, smem, st>>>(W, psi, out, a, nullptr, nullptr);
     OK_LAUNCHED("apply_pauli_part_kernel");
     return launch_parts<real, PART + 1>(grid, st, W, psi, out, a, dot_a, partials);
   }
