@@ -14,7 +14,8 @@
  *     aligned, unless the argument is documented as HOST.  `ok_params*`, `iters`, `resid`
  *     are HOST pointers.
  *   - The caller owns every buffer.  The library allocates no persistent device memory and
- *     frees nothing; scratch comes from the buffer given to ok_set_workspace.
+ *     frees nothing; scratch comes from the buffer given to ok_set_workspace (one exception: the
+ *     fixed 1.5 MiB static array behind ok_dirac_apply_dot_static, see there).
  *   - All work is enqueued on the stream given to ok_set_stream (default: the legacy default
  *     stream).  Calls are asynchronous except ok_bicgstab, ok_*_host and the first use of a W
  *     buffer the library has not seen (one 1 KiB header read), which synchronise that stream.
@@ -241,6 +242,24 @@ int ok_slab_dirac_apply(const void* W, const void* psi_ext, void* out_ext);
  * ok_bicgstab, identical on every process.  Pointer arrays, iters, resid: HOST. */
 int ok_slab_bicgstab(int nslab, const void* const* W, const void* const* src_ext, void* const* x_ext, double tol, int maxit,
                      const ok_comm* comm, int* iters, double* resid);
+
+/* ---- an entry point that allocates nothing ------------------------------------------------ */
+/* For callers that cannot call cudaMalloc and have no workspace to lend (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid allocation): the Dirac apply of Eq. (2.2) together with the three
+ * reductions BiCGStab takes from it,
+ *     out = M psi ,   result[0..2] = ( Re<a,out>, Im<a,out>, ||out||^2 ) ,   <a,b> = sum conj(a) b ,
+ * fp64 sums in a fixed order (bit-reproducible).  W, psi, a, out as in ok_dirac_apply (nrhs = 1, any precision and W storage
+ * format; out must alias neither psi nor a); result: DEVICE, 3 doubles, written by the call (asynchronously, on the library's stream).
+ * The per-block partial sums live in a static __device__ array inside the library instead of the workspace: 1.5 MiB
+ * (65 536 rows of 3 doubles) on every GPU that loads the library, for lattices of up to OK_STATIC_MAX_SITES sites.  Larger
+ * lattices are rejected with OK_EINVAL and a message in ok_static_strerror().  The call uses neither the workspace nor
+ * cudaMalloc / cudaFree nor any allocating library routine.  Every call shares the one array: calls whose kernels overlap on the GPU
+ * (two streams) race on it; calls on one stream are safe, nothing in the array has to be cleared between them.
+ * The first use of a W buffer the library has not seen reads its 1 KiB header synchronously (General rules). */
+#define OK_STATIC_MAX_SITES 2097152   /* 32^3 x 64 */
+int ok_dirac_apply_dot_static(const void* W, const void* psi, const void* a, void* out, double* result);
+size_t ok_static_max_sites(void);          /* = OK_STATIC_MAX_SITES */
+const char* ok_static_strerror(void);      /* text of the last error ok_dirac_apply_dot_static returned */
 
 /* ---- diagnostics -------------------------------------------------------------------------- */
 /* Read the parameters stored in W's header back into *p (HOST).  Always reads the 1 KiB device header (synchronises the

@@ -57,6 +57,9 @@ EXPORTS = {
     "ok_bicgstab": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int,
                               C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_dirac_apply_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_dirac_apply_dot_static": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_static_max_sites": (C.c_size_t, []),
+    "ok_static_strerror": (C.c_char_p, []),
     "ok_cgnr": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_W_unit_index": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int)]),
     "ok_mixed_work_bytes": (C.c_size_t, [C.POINTER(ok_params)]),
@@ -177,6 +180,21 @@ def ok_precalc_W(links, p, W):
 
 def ok_dirac_apply(W, psi, out):
     _check(lib().ok_dirac_apply(_ptr(W), _ptr(psi), _ptr(out)), "ok_dirac_apply")
+
+
+def ok_static_max_sites():
+    return lib().ok_static_max_sites()
+
+
+def ok_static_strerror():
+    return lib().ok_static_strerror().decode()
+
+
+def ok_dirac_apply_dot_static(W, psi, a, out, result):
+    """out = M psi, result (device, 3 doubles) = Re<a,out>, Im<a,out>, ||out||^2; allocates nothing (ok.h)."""
+    st = lib().ok_dirac_apply_dot_static(_ptr(W), _ptr(psi), _ptr(a), _ptr(out), _ptr(result))
+    if st != 0:
+        raise OkError(st, "ok_dirac_apply_dot_static: " + ok_static_strerror())
 
 
 def ok_dirac_apply_host(W, psi_host, out_host):
