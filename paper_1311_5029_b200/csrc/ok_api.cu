@@ -256,21 +256,26 @@ int ok_dirac_apply(const void* W, const void* psi, void* out) {
 // c + 1 have landed (the stencil reaches one slice in t) while later chunks are still crossing PCIe, and its
 // result starts back to the host while the next chunk is computed.  Three streams: copies in, the caller's stream for
 // pack / apply / unpack, copies out.  Copy order n-1, 0, 1, ..., n-2 so that chunk 0 (which needs the last chunk through the
-// periodic closure) can start after three chunks.  The paper's GPU code pays these copies in sequence on every call
-// (96.6 % of its overhead); here they hide behind the W stream.
+// periodic closure) can start after three chunks.  The applies (with their unpack) alternate between two more library-owned
+// streams, so that the ramp-down of one chunk's launch overlaps the next chunk's ramp-up (16 short launches otherwise lose
+// a tail each).  The paper's GPU code pays these copies in sequence on every call (96.6 % of its
+// overhead); here they hide behind the W stream.
 static int apply_host_pipelined(const ok_params& p, const void* W, const char* psi_host, char* out_host, char* canon_in, char* packed_in,
                                 char* packed_out, char* canon_out) {
   constexpr int kMaxChunks = 16;
-  static cudaStream_t s_in = nullptr, s_out = nullptr;
-  static cudaEvent_t ev_start = nullptr, ev_end = nullptr, ev_in[kMaxChunks], ev_done[kMaxChunks];
+  static cudaStream_t s_in = nullptr, s_out = nullptr, s_ap[2] = {nullptr, nullptr};
+  static cudaEvent_t ev_start = nullptr, ev_end = nullptr, ev_in[kMaxChunks], ev_done[kMaxChunks], ev_packed[kMaxChunks];
   if (!s_in) {
     OK_CUDA(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
     OK_CUDA(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    OK_CUDA(cudaStreamCreateWithFlags(&s_ap[0], cudaStreamNonBlocking));
+    OK_CUDA(cudaStreamCreateWithFlags(&s_ap[1], cudaStreamNonBlocking));
     OK_CUDA(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
     OK_CUDA(cudaEventCreateWithFlags(&ev_end, cudaEventDisableTiming));
     for (int c = 0; c < kMaxChunks; ++c) {
       OK_CUDA(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming));
       OK_CUDA(cudaEventCreateWithFlags(&ev_done[c], cudaEventDisableTiming));
+      OK_CUDA(cudaEventCreateWithFlags(&ev_packed[c], cudaEventDisableTiming));
     }
   }
   cudaStream_t st = ctx().stream;
@@ -294,20 +299,29 @@ static int apply_host_pipelined(const ok_params& p, const void* W, const char* p
     q.dims[3] = t0[c + 1] - t0[c];
     return q;
   };
+  int last_packed = -1;   // the packs run in issue order on st, so the latest one's event covers all of them
   auto pack = [&](int c) -> int {
     OK_CUDA(cudaStreamWaitEvent(st, ev_in[c], 0));
     const ok_params q = chunk_params(c);
     const size_t off = (size_t)t0[c] * sb;
-    return launch_pack_spinor(&q, canon_in + off, packed_in + off, false);
+    int r = launch_pack_spinor(&q, canon_in + off, packed_in + off, false);
+    if (r) return r;
+    OK_CUDA(cudaEventRecord(ev_packed[c], st));
+    last_packed = c;
+    return OK_SUCCESS;
   };
-  auto apply = [&](int c) -> int {
+  auto apply = [&](int c) -> int {   // issued right after the last pack it needs
     const ok_params q = chunk_params(c);
     const size_t off = (size_t)t0[c] * sb;
     const int blk0 = (int)(t0[c] * slice_sites / kBlock), nblk = (int)((t0[c + 1] - t0[c]) * slice_sites / kBlock);
+    cudaStream_t sa = s_ap[c & 1];
+    OK_CUDA(cudaStreamWaitEvent(sa, ev_packed[last_packed], 0));
+    ctx().stream = sa;
     int r = launch_apply_range(&p, W_payload(W), packed_in, packed_out, blk0, nblk);
+    if (!r) r = launch_pack_spinor(&q, canon_out + off, packed_out + off, true);
+    ctx().stream = st;
     if (r) return r;
-    if ((r = launch_pack_spinor(&q, canon_out + off, packed_out + off, true))) return r;
-    OK_CUDA(cudaEventRecord(ev_done[c], st));
+    OK_CUDA(cudaEventRecord(ev_done[c], sa));
     OK_CUDA(cudaStreamWaitEvent(s_out, ev_done[c], 0));
     OK_CUDA(cudaMemcpyAsync(out_host + off, canon_out + off, (size_t)(t0[c + 1] - t0[c]) * sb, cudaMemcpyDeviceToHost, s_out));
     return OK_SUCCESS;
