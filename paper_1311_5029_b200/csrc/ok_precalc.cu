@@ -61,6 +61,20 @@ __device__ __forceinline__ cm3 zero3() {
   for (int i = 0; i < 9; ++i) r.e[i] = make_double2(0.0, 0.0);
   return r;
 }
+// s += a b, s += a conj(b), s += conj(a) b: four DFMA each (written out so that no product is rounded on its own and added later:
+// the clover and hop-block kernels are bound by the fp64 pipe)
+__device__ __forceinline__ void cmac(double2& s, double2 a, double2 b) {
+  s.x = fma(a.x, b.x, s.x); s.x = fma(-a.y, b.y, s.x);
+  s.y = fma(a.x, b.y, s.y); s.y = fma(a.y, b.x, s.y);
+}
+__device__ __forceinline__ void cmacc(double2& s, double2 a, double2 b) {   // a * conj(b)
+  s.x = fma(a.x, b.x, s.x); s.x = fma(a.y, b.y, s.x);
+  s.y = fma(a.y, b.x, s.y); s.y = fma(-a.x, b.y, s.y);
+}
+__device__ __forceinline__ void cconjmac(double2& s, double2 a, double2 b) {   // conj(a) * b
+  s.x = fma(a.x, b.x, s.x); s.x = fma(a.y, b.y, s.x);
+  s.y = fma(a.x, b.y, s.y); s.y = fma(-a.y, b.x, s.y);
+}
 __device__ cm3 mul(const cm3& A, const cm3& B) {   // A B
   cm3 r;
 #pragma unroll
@@ -69,7 +83,7 @@ __device__ cm3 mul(const cm3& A, const cm3& B) {   // A B
     for (int j = 0; j < 3; ++j) {
       double2 s = cmul(A.e[3 * i], B.e[j]);
 #pragma unroll
-      for (int k = 1; k < 3; ++k) { double2 q = cmul(A.e[3 * i + k], B.e[3 * k + j]); s.x += q.x; s.y += q.y; }
+      for (int k = 1; k < 3; ++k) cmac(s, A.e[3 * i + k], B.e[3 * k + j]);
       r.e[3 * i + j] = s;
     }
   return r;
@@ -82,7 +96,7 @@ __device__ cm3 mul_nd(const cm3& A, const cm3& B) {   // A B^dag
     for (int j = 0; j < 3; ++j) {
       double2 s = cmulc(A.e[3 * i], B.e[3 * j]);
 #pragma unroll
-      for (int k = 1; k < 3; ++k) { double2 q = cmulc(A.e[3 * i + k], B.e[3 * j + k]); s.x += q.x; s.y += q.y; }
+      for (int k = 1; k < 3; ++k) cmacc(s, A.e[3 * i + k], B.e[3 * j + k]);
       r.e[3 * i + j] = s;
     }
   return r;
@@ -95,7 +109,7 @@ __device__ cm3 mul_dn(const cm3& A, const cm3& B) {   // A^dag B
     for (int j = 0; j < 3; ++j) {
       double2 s = cconjmul(A.e[i], B.e[j]);
 #pragma unroll
-      for (int k = 1; k < 3; ++k) { double2 q = cconjmul(A.e[3 * k + i], B.e[3 * k + j]); s.x += q.x; s.y += q.y; }
+      for (int k = 1; k < 3; ++k) cconjmac(s, A.e[3 * k + i], B.e[3 * k + j]);
       r.e[3 * i + j] = s;
     }
   return r;
@@ -112,8 +126,8 @@ __device__ __forceinline__ cm3 adj(const cm3& A) {
 __device__ __forceinline__ void axpy(cm3& r, double cr, double ci, const cm3& A) {
 #pragma unroll
   for (int i = 0; i < 9; ++i) {
-    r.e[i].x += cr * A.e[i].x - ci * A.e[i].y;
-    r.e[i].y += cr * A.e[i].y + ci * A.e[i].x;
+    r.e[i].x = fma(cr, A.e[i].x, r.e[i].x); r.e[i].x = fma(-ci, A.e[i].y, r.e[i].x);
+    r.e[i].y = fma(cr, A.e[i].y, r.e[i].y); r.e[i].y = fma(ci, A.e[i].x, r.e[i].y);
   }
 }
 
@@ -848,9 +862,7 @@ __device__ __forceinline__ void acc_prod_line(double2 (&out)[3], const LinkRef& 
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
       const double2 b = tr ? link_el(X, t, m, Vpad) : link_el(Y, m, t, Vpad);
-      const double2 q = cmul(v[m], b);
-      out[t].x += q.x;
-      out[t].y += q.y;
+      cmac(out[t], v[m], b);
     }
 }
 // row ca of the colour matrix of a two-link term (two_link_P at x, or its adjoint for an opposite-direction term)
