@@ -236,10 +236,23 @@ int ok_slab_precalc_W(const void* links_ext, const ok_params* slab, int T_global
 /* Eq. (2.2) on one slab: out(x) for the slab's sites; psi_ext must hold the two halo slices.  out_ext's halos are not written. */
 int ok_slab_dirac_apply(const void* W, const void* psi_ext, void* out_ext);
 
+/* The same apply with the halo exchange fused into it (only the two outermost time slices of a node's
+ * sub-lattice involve its neighbours): the halo slices of psi_ext are NOT read; wherever Eq. (2.2) reaches across the lower /
+ * upper t-face the kernel loads psi(x -+ t) straight from lo_slice / hi_slice -- the lower neighbour's LAST own time slice and
+ * the upper neighbour's FIRST own time slice, internal layout, ok_slab_slice_bytes each.  Any address this GPU can load from
+ * will do: another slab's field in the same process (its ext base + Tloc slices, resp. + 1 slice), or a buffer in a
+ * neighbour GPU's memory opened through CUDA peer access / IPC, in which case the neighbour's slice crosses NVLink once, as
+ * the 512-byte lines the warps ask for, with no copy kernel, staging buffer or collective in front of the apply.  The caller
+ * orders the call after the neighbours have finished writing those slices (same stream, an event, or a barrier between the
+ * processes) and keeps them unchanged until the apply has completed.  Bit-identical to ok_slab_dirac_apply on filled halos. */
+int ok_slab_dirac_apply_peer(const void* W, const void* psi_ext, const void* lo_slice, const void* hi_slice, void* out_ext);
+
 /* BiCGStab (as ok_bicgstab) over the nslab slabs this process holds, in t order (W[s], src_ext[s], x_ext[s] of slab s);
  * with comm, over nslab * comm->nranks slabs in all.  Every reduction is summed per slab and then over the slabs in global
  * order, so the iteration is bit-reproducible and independent of how the slabs are dealt to processes.  *iters, *resid as
- * ok_bicgstab, identical on every process.  Pointer arrays, iters, resid: HOST. */
+ * ok_bicgstab, identical on every process.  Pointer arrays, iters, resid: HOST.
+ * Between slabs of one process the applies read each other's boundary slices in place (as ok_slab_dirac_apply_peer does); only
+ * the two outer faces of a process go through comm->exchange into halo slices. */
 int ok_slab_bicgstab(int nslab, const void* const* W, const void* const* src_ext, void* const* x_ext, double tol, int maxit,
                      const ok_comm* comm, int* iters, double* resid);
 

@@ -70,6 +70,7 @@ EXPORTS = {
     "ok_slab_work_bytes": (C.c_size_t, [C.POINTER(ok_params), C.c_int, C.c_int]),
     "ok_slab_precalc_W": (C.c_int, [C.c_void_p, C.POINTER(ok_params), C.c_int, C.c_int, C.c_void_p]),
     "ok_slab_dirac_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_slab_dirac_apply_peer": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "ok_slab_bicgstab": (C.c_int, [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.c_int,
                                    C.POINTER(ok_comm), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_W_params": (C.c_int, [C.c_void_p, C.POINTER(ok_params)]),
@@ -266,6 +267,11 @@ def ok_slab_precalc_W(links_ext, slab, T_global, t0, W):
 
 def ok_slab_dirac_apply(W, psi_ext, out_ext):
     _check(lib().ok_slab_dirac_apply(_ptr(W), _ptr(psi_ext), _ptr(out_ext)), "ok_slab_dirac_apply")
+
+
+def ok_slab_dirac_apply_peer(W, psi_ext, lo_slice, hi_slice, out_ext):
+    """lo_slice / hi_slice: device addresses (tensor views or ints) of the neighbours' boundary slices (ok.h)."""
+    _check(lib().ok_slab_dirac_apply_peer(_ptr(W), _ptr(psi_ext), _ptr(lo_slice), _ptr(hi_slice), _ptr(out_ext)), "ok_slab_dirac_apply_peer")
 
 
 def ok_slab_bicgstab(W, src_ext, x_ext, tol, maxit, comm=None, raise_on_fail=True):

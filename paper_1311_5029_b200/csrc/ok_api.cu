@@ -465,6 +465,15 @@ int ok_slab_dirac_apply(const void* W, const void* psi, void* out) {
   return launch_apply_slab(&p, W_payload(W), psi, out, nullptr, nullptr);
 }
 
+int ok_slab_dirac_apply_peer(const void* W, const void* psi, const void* lo_slice, const void* hi_slice, void* out) {
+  if (!aligned16(psi) || !aligned16(out) || !aligned16(lo_slice) || !aligned16(hi_slice) || psi == out) return OK_EINVAL;
+  ok_params p;
+  int st = lookup_W(W, &p);
+  if (st) return st;
+  if (!valid_slab(&p)) return OK_EINVAL;
+  return launch_apply_slab(&p, W_payload(W), psi, out, nullptr, nullptr, lo_slice, hi_slice);
+}
+
 int ok_slab_bicgstab(int nslab, const void* const* W, const void* const* src, void* const* x, double tol, int maxit, const ok_comm* comm,
                      int* iters, double* resid) {
   if (nslab < 1 || nslab > 64 || !W || !src || !x || !iters || !resid || !(tol > 0.0) || maxit < 1) return OK_EINVAL;

@@ -45,11 +45,16 @@ __device__ __forceinline__ int wrap(int x, int L) {
   return x;
 }
 
-template <typename real, int RPT, bool DOT>
+// PEER (t-slab only, ok_slab_dirac_apply_peer): the two halo time slices of the extended field are not read from psi but from
+// lo_peer / hi_peer -- the t-neighbours' own boundary slices, wherever they live (another slab's field on this GPU, or a
+// neighbour GPU's memory mapped through NVLink peer access): the halo exchange is the apply's own loads, no copy, no staging.
+template <typename real, int RPT, bool DOT, bool PEER = false>
 __global__ void __launch_bounds__(32 * (12 / RPT))
 apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typename Vec<real>::type* __restrict__ psi,
                     typename Vec<real>::type* __restrict__ out, Geom g, int vblk0,
-                    const typename Vec<real>::type* __restrict__ dot_a, double* __restrict__ partials) {
+                    const typename Vec<real>::type* __restrict__ dot_a, double* __restrict__ partials,
+                    const typename Vec<real>::type* __restrict__ lo_peer = nullptr,
+                    const typename Vec<real>::type* __restrict__ hi_peer = nullptr) {
   using vec_t = typename Vec<real>::type;
   constexpr int NC = Vec<real>::NC;
   constexpr int NW = 12 / RPT;
@@ -82,6 +87,10 @@ apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typena
     const int tt = wrap(t + c_off[o][3], g.L[3]);
     const int nn = xx + g.L[0] * (yy + g.L[1] * (zz + g.L[2] * tt));
     const vec_t* sp = psi + (size_t)(nn >> 5) * NC * kBlock + (nn & 31);
+    if constexpr (PEER) {   // a time slice is a whole number of blocks (vblk0), so tt is uniform over the warp
+      if (tt == 0) sp = lo_peer + (size_t)(nn >> 5) * NC * kBlock + (nn & 31);
+      else if (tt == g.L[3] - 1) sp = hi_peer + (size_t)((nn >> 5) - (g.L[3] - 1) * vblk0) * NC * kBlock + (nn & 31);
+    }
     vec_t w[RPT][NC];
 #pragma unroll
     for (int r = 0; r < RPT; ++r)
@@ -147,9 +156,21 @@ apply_direct_kernel(const typename Vec<real>::type* __restrict__ W, const typena
 
 template <typename real, int RPT>
 static int launch_direct(const Geom& g, const void* W, const void* psi, void* out, double* partials,
-                         const void* dot_a, int nblk = -1, int vblk0 = 0) {
+                         const void* dot_a, int nblk = -1, int vblk0 = 0, const void* lo_peer = nullptr, const void* hi_peer = nullptr) {
   using vec_t = typename Vec<real>::type;
   dim3 grid(nblk < 0 ? g.nblk : nblk), block(32 * (12 / RPT));
+  if (lo_peer && hi_peer) {
+    if (partials)
+      apply_direct_kernel<real, RPT, true, true><<<grid, block, 0, ctx().stream>>>(
+          static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g, vblk0,
+          static_cast<const vec_t*>(dot_a), partials, static_cast<const vec_t*>(lo_peer), static_cast<const vec_t*>(hi_peer));
+    else
+      apply_direct_kernel<real, RPT, false, true><<<grid, block, 0, ctx().stream>>>(
+          static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g, vblk0, nullptr, nullptr,
+          static_cast<const vec_t*>(lo_peer), static_cast<const vec_t*>(hi_peer));
+    OK_LAUNCHED("apply_direct_kernel (peer halos)");
+    return OK_SUCCESS;
+  }
   if (partials)
     apply_direct_kernel<real, RPT, true><<<grid, block, 0, ctx().stream>>>(
         static_cast<const vec_t*>(W), static_cast<const vec_t*>(psi), static_cast<vec_t*>(out), g, vblk0,
@@ -198,7 +219,10 @@ int launch_apply_range(const ok_params* p, const void* Wp, const void* psi, void
 
 // t-slab apply (ok_slab.cu): p = the slab's own lattice (Lx, Ly, Lz, Tloc) whose W this is; psi, out, dot_a are fields of the
 // extended lattice (Lx, Ly, Lz, Tloc + 2) in the internal layout, i.e. [lower halo slice][Tloc slices][upper halo slice].
-int launch_apply_slab(const ok_params* p, const void* W, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext) {
+// lo_peer / hi_peer (both or neither): the neighbours' boundary slices, read in place of psi_ext's halo slices.
+int launch_apply_slab(const ok_params* p, const void* W, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext,
+                      const void* lo_peer, const void* hi_peer) {
+  if ((lo_peer == nullptr) != (hi_peer == nullptr)) return OK_EINVAL;
   if (p->nrhs != 1 || p->storage != OK_W_DENSE) return OK_EINVAL;
   int st = upload_offsets();
   if (st) return st;
@@ -209,8 +233,9 @@ int launch_apply_slab(const ok_params* p, const void* W, const void* psi_ext, vo
   ge.L[3] = g.L[3] + 2;
   ge.V = g.V + 2 * slice;
   ge.nblk = ge.V / kBlock;
-  if (p->precision == OK_FP64) return launch_direct<double, kRowsPerWarp>(ge, W, psi_ext, out_ext, partials, dot_a_ext, g.nblk, slice / kBlock);
-  return launch_direct<float, kRowsPerWarp>(ge, W, psi_ext, out_ext, partials, dot_a_ext, g.nblk, slice / kBlock);
+  if (p->precision == OK_FP64)
+    return launch_direct<double, kRowsPerWarp>(ge, W, psi_ext, out_ext, partials, dot_a_ext, g.nblk, slice / kBlock, lo_peer, hi_peer);
+  return launch_direct<float, kRowsPerWarp>(ge, W, psi_ext, out_ext, partials, dot_a_ext, g.nblk, slice / kBlock, lo_peer, hi_peer);
 }
 
 }  // namespace okd

@@ -357,8 +357,9 @@ int run_bicgstab(const ok_params* p, const void* W, const void* src, void* x, do
 // t-slab decomposition: the same BiCGStab over a lattice cut along T into slabs.
 // "In the temporal direction, only the nearest neighbors are involved" and "off-node communications are
 // necessary only for the outermost boundary surfaces": W is slab-local, a slab's fields carry one halo
-// time slice below and above (ok.h), and before every apply each slab's halos are refreshed from its t-neighbours --
-// device copies between the slabs of this process, the caller's `exchange` for the two outer faces.  Reductions:
+// time slice below and above (ok.h); an apply reads its t-neighbours' boundary slices in place where they belong to a slab
+// of this process (fused halo loads, apply_direct_kernel<.., PEER>) and from the halo slices filled by the caller's
+// `exchange` at the two outer faces of the process.  Reductions:
 // per-CTA partials (as above) -> one fixed-order total per SLAB -> (all-gather over processes) -> sum over all slabs in
 // global slab order -> scalars.  The result therefore depends on the number of slabs, not on how they are dealt to
 // processes; every process computes identical scalars.
@@ -505,23 +506,31 @@ static int solve_slabs(int nslab, const ok_params* const* ps, const void* const*
     OK_LAUNCHED("k_slab_scalars");
     return OK_SUCCESS;
   };
-  // halo refresh of one field of every slab; sel picks the field
-  auto halos = [&](c2* Slab::*field) -> int {
+  // The t-faces of one field of every slab.  Slabs of this process read each other's boundary slices in place (the apply's
+  // PEER loads, ok_slab_dirac_apply_peer): nothing is copied for them.  Only the two outer faces of the process arrive through
+  // the caller's `exchange`, into the lower halo slice of the first slab and the upper halo slice of the last one; without
+  // comm the process holds the whole T extent and the periodic closure is one more in-place read (the boundary condition
+  // sits in W).  lo[i] / hi[i]: where slab i finds psi(x - t) of its first slice and psi(x + t) of its last one.
+  const char* face_lo[64];
+  const char* face_hi[64];
+  auto faces = [&](c2* Slab::*field) -> int {
     auto lo_halo = [&](Slab& a) { return reinterpret_cast<char*>(a.*field); };
     auto first_slice = [&](Slab& a) { return reinterpret_cast<char*>(a.*field) + a.slice_bytes; };
     auto last_slice = [&](Slab& a) { return reinterpret_cast<char*>(a.*field) + (size_t)a.p->dims[3] * a.slice_bytes; };
     auto hi_halo = [&](Slab& a) { return reinterpret_cast<char*>(a.*field) + (size_t)(a.p->dims[3] + 1) * a.slice_bytes; };
     const size_t nb = sl[0].slice_bytes;
-    for (int i = 0; i + 1 < nslab; ++i) {
-      OK_CUDA(cudaMemcpyAsync(hi_halo(sl[i]), first_slice(sl[i + 1]), nb, cudaMemcpyDeviceToDevice, st));
-      OK_CUDA(cudaMemcpyAsync(lo_halo(sl[i + 1]), last_slice(sl[i]), nb, cudaMemcpyDeviceToDevice, st));
+    for (int i = 0; i < nslab; ++i) {
+      face_lo[i] = i > 0 ? last_slice(sl[i - 1]) : nullptr;
+      face_hi[i] = i + 1 < nslab ? first_slice(sl[i + 1]) : nullptr;
     }
     Slab &a0 = sl[0], &a1 = sl[nslab - 1];
     if (comm && comm->exchange) {
       if (comm->exchange(comm->user, first_slice(a0), last_slice(a1), lo_halo(a0), hi_halo(a1), nb)) return OK_ECOMM;
-    } else {   // this process holds the whole T extent: periodic closure (the boundary condition sits in W)
-      OK_CUDA(cudaMemcpyAsync(lo_halo(a0), last_slice(a1), nb, cudaMemcpyDeviceToDevice, st));
-      OK_CUDA(cudaMemcpyAsync(hi_halo(a1), first_slice(a0), nb, cudaMemcpyDeviceToDevice, st));
+      face_lo[0] = lo_halo(a0);
+      face_hi[nslab - 1] = hi_halo(a1);
+    } else {
+      face_lo[0] = last_slice(a1);
+      face_hi[nslab - 1] = first_slice(a0);
     }
     return OK_SUCCESS;
   };
@@ -543,10 +552,11 @@ static int solve_slabs(int nslab, const ok_params* const* ps, const void* const*
   }
   const double target = tol * tol * bnorm2;
   auto apply_all = [&](c2* Slab::*in, c2* Slab::*out, c2* Slab::*dot) -> int {
-    OK_TRY(halos(in));
+    OK_TRY(faces(in));
     for (int i = 0; i < nslab; ++i) {
       Slab& a = sl[i];
-      OK_TRY(launch_apply_slab(a.p, a.W, a.*in, a.*out, dot ? partials + (size_t)a.pfirst * 3 : nullptr, dot ? a.*dot : nullptr));
+      OK_TRY(launch_apply_slab(a.p, a.W, a.*in, a.*out, dot ? partials + (size_t)a.pfirst * 3 : nullptr, dot ? a.*dot : nullptr,
+                               face_lo[i], face_hi[i]));
     }
     return OK_SUCCESS;
   };

@@ -215,7 +215,8 @@ int launch_precalc(const ok_params* p, const void* links, void* Wpayload, void* 
 int launch_precalc_window(const ok_params* p, const void* links, void* Wpayload, void* work, int tfold, int win_blk0, int win_nblk);
 // t-slab decomposition (ok.h): p = the slab's own lattice
 int launch_apply_range(const ok_params* p, const void* Wpayload, const void* psi, void* out, int blk0, int nblk);
-int launch_apply_slab(const ok_params* p, const void* Wpayload, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext);
+int launch_apply_slab(const ok_params* p, const void* Wpayload, const void* psi_ext, void* out_ext, double* partials, const void* dot_a_ext,
+                      const void* lo_peer = nullptr, const void* hi_peer = nullptr);
 size_t bicgstab_slab_work_bytes(const ok_params* p);
 size_t bicgstab_slab_shared_bytes(int nslab, int nranks);
 int run_bicgstab_slabs(int nslab, const ok_params* const* ps, const void* const* Wpayloads, const void* const* srcs, void* const* xs,

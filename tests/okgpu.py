@@ -97,3 +97,49 @@ def fp32_operator_slack(o, x, b, idx=None, W=None):
     if S.ndim == 3:     # [site][comp][rhs]: one bound per column
         return 2.0 * 2.0 ** -24 * scale * np.linalg.norm(S.reshape(-1, S.shape[2]), axis=0) / np.linalg.norm(b.reshape(-1, b.shape[2]), axis=0)
     return 2.0 * 2.0 ** -24 * scale * float(np.linalg.norm(S)) / float(np.linalg.norm(b))
+
+
+def ipc_slab_worker(rank, nranks, U, pd, prec, psi, q_in, q_out, results, barrier):
+    """One process = one t-slab on cuda:0 (tests/test_gpu_slab.py, the CUDA-IPC test): builds its W and field, hands its field to
+    the two t-neighbours as a CUDA IPC handle (a torch CUDA tensor sent through a multiprocessing queue), maps theirs, and applies
+    with ok_slab_dirac_apply_peer reading the neighbours' boundary slices through the mapping.  Host-side barriers order the
+    phases; no kernel waits on another process's kernel."""
+    from paper_1311_5029_b200 import slab as S
+    try:
+        torch.cuda.set_device(0)
+        dims = tuple(pd["dims"])
+        p = B.make_params(pd, prec)
+        t0, Tl = S.slab_ranges(dims[3], nranks)[rank]
+        slab = B.make_slab_params(p, Tl)
+        plocal = B.make_params(dict(pd, dims=dims[:3] + (Tl,)), prec)
+        work = B.alloc_bytes(B.ok_slab_work_bytes(slab, 1, 1), DEV)
+        B.ok_set_stream(None)
+        B.ok_set_workspace(work, work.numel())
+        W = B.alloc_W(slab, DEV)
+        B.ok_slab_precalc_W(to_dev(S.link_window(U, dims, t0, Tl), torch.complex128), slab, dims[3], t0, W)
+        v = torch.zeros(B.ok_slab_vec_bytes(slab), dtype=torch.uint8, device=DEV)
+        B.ok_pack_spinor(plocal, to_dev(S.spinor_slab(psi, dims, t0, Tl), cdtype(prec)), S.interior(slab, v))
+        lo, first, last, hi = S.halo_views(slab, v)
+        lo.fill_(0xFF)
+        hi.fill_(0xFF)
+        torch.cuda.synchronize()
+        q_in[(rank - 1) % nranks].put(("from_above", v))      # my field, for my lower neighbour's upper face
+        q_in[(rank + 1) % nranks].put(("from_below", v))
+        got = dict(q_in[rank].get(timeout=120) for _ in range(2))
+        barrier.wait(timeout=120)                              # every field is complete and mapped
+        out = torch.zeros_like(v)
+        lo_slice = S.halo_views(slab, got["from_below"])[2]    # the lower neighbour's last own slice, in ITS memory
+        hi_slice = S.halo_views(slab, got["from_above"])[1]
+        B.ok_slab_dirac_apply_peer(W, v, lo_slice, hi_slice, out)
+        canon = torch.empty((Tl * dims[0] * dims[1] * dims[2], 12), dtype=cdtype(prec), device=DEV)
+        B.ok_unpack_spinor(plocal, S.interior(slab, out), canon)
+        torch.cuda.synchronize()
+        results.put((rank, canon.cpu().numpy(), None))
+        barrier.wait(timeout=120)                              # nobody frees a field a neighbour may still be reading
+        del got, lo_slice, hi_slice
+    except Exception as e:  # pragma: no cover
+        results.put((rank, None, repr(e)))
+        try:
+            barrier.abort()
+        except Exception:
+            pass

@@ -3,8 +3,10 @@ held by one process stand in for the ranks ("virtual ranks": separate W, fields 
   * ok_slab_precalc_W from a slab's link window == the whole-lattice W on the slab's sites, bit for bit;
   * ok_slab_dirac_apply with the neighbours' boundary slices in the halos == the whole-lattice apply, bit for bit, and
     within the north_star tolerance of the ORACLE on the full lattice;
+  * ok_slab_dirac_apply_peer (halo exchange fused into the apply: the neighbours' boundary slices loaded in place) the same, with
+    the neighbours in this process and in ANOTHER process whose memory is mapped through CUDA IPC;
   * ok_slab_bicgstab == the oracle's BiCGStab (iterations +-2, true residual <= tol, solution), bit-reproducible, and
-    bit-identical whether the T closure goes through device copies or through the ok_comm callbacks (the multi-process path).
+    bit-identical whether the T closure is read in place or goes through the ok_comm callbacks (the multi-process path).
 """
 import numpy as np
 import pytest
@@ -101,6 +103,71 @@ def test_slab_W_and_apply_equal_the_whole_lattice_bit_for_bit(dims, nslab, prec)
         assert G.per_site_rel_err(got, want) <= 1e-12
     else:
         assert G.rel_l2(got, want) <= 2e-5
+    B.ok_set_workspace(None)
+
+
+@pytest.mark.parametrize("prec", [B.OK_FP64, B.OK_FP32])
+@pytest.mark.parametrize("dims,nslab", CASES)
+def test_slab_apply_with_fused_halo_loads_equals_the_whole_lattice_bit_for_bit(dims, nslab, prec):
+    """ok_slab_dirac_apply_peer: the neighbours' boundary slices are read in place (the address a peer GPU's mapped buffer would
+    have); this slab's own halo slices are poisoned to show that nothing reads them."""
+    U, pd, o = setup(dims)
+    p = B.make_params(pd, prec)
+    W = G.precalc(p, U)
+    psi = I.gaussian_spinor(dims, 2)
+    whole = G.apply(p, W, psi)
+    sl = Slabs(U, pd, prec, nslab)
+    vecs = sl.scatter(psi)
+    for v in vecs:
+        lo, first, last, hi = S.halo_views(sl.slab, v)
+        lo.fill_(0xFF)          # NaN patterns in both precisions
+        hi.fill_(0xFF)
+    outs = [torch.zeros_like(v) for v in vecs]
+    for i, (Ws, v, out) in enumerate(zip(sl.W, vecs, outs)):
+        lo_slice = S.halo_views(sl.slab, vecs[(i - 1) % nslab])[2]      # the lower neighbour's last own slice
+        hi_slice = S.halo_views(sl.slab, vecs[(i + 1) % nslab])[1]      # the upper neighbour's first own slice
+        B.ok_slab_dirac_apply_peer(Ws, v, lo_slice, hi_slice, out)
+    got = sl.gather(outs)
+    assert np.array_equal(got, whole)
+    want = o.apply_W(psi)
+    if prec == B.OK_FP64:
+        assert G.per_site_rel_err(got, want) <= 1e-12
+    else:
+        assert G.rel_l2(got, want) <= 2e-5
+    with pytest.raises(B.OkError):
+        B.ok_slab_dirac_apply_peer(sl.W[0], vecs[0], None, S.halo_views(sl.slab, vecs[0])[1], outs[0])
+    B.ok_set_workspace(None)
+
+
+def test_slab_apply_reads_another_process_memory_through_cuda_ipc():
+    """Two processes on cuda:0, one slab each: every process maps the other's field through CUDA IPC and its apply loads the
+    neighbour's boundary slices straight from that mapping -- the mechanism a multi-GPU run uses over NVLink peer access --
+    and the gathered result equals the whole-lattice apply bit for bit."""
+    import torch.multiprocessing as mp
+    dims, nranks, prec = (4, 4, 4, 8), 2, B.OK_FP64
+    U, pd, o = setup(dims)
+    p = B.make_params(pd, prec)
+    psi = I.gaussian_spinor(dims, 2)
+    whole = G.apply(p, G.precalc(p, U), psi)
+    ctx = mp.get_context("spawn")
+    q_in = [ctx.Queue() for _ in range(nranks)]
+    results, barrier = ctx.Queue(), ctx.Barrier(nranks)
+    procs = [ctx.Process(target=G.ipc_slab_worker, args=(r, nranks, U, pd, prec, psi, q_in, q_in, results, barrier)) for r in range(nranks)]
+    for pr in procs:
+        pr.start()
+    try:
+        parts = {}
+        for _ in range(nranks):
+            rank, arr, err = results.get(timeout=300)
+            assert err is None, err
+            parts[rank] = arr
+    finally:
+        for pr in procs:
+            pr.join(timeout=60)
+            if pr.is_alive():
+                pr.kill()
+    got = np.concatenate([parts[r] for r in range(nranks)]).astype(np.complex128)
+    assert np.array_equal(got, whole)
     B.ok_set_workspace(None)
 
 
