@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(256) transpose_links_kernel(const double2* __r
 // ------------------------------------------------------------------------- step a1: clover F
 // FS[k][n]: k = 0..2 -> B_1,B_2,B_3 = F_23, F_31, F_12 ; k = 3..5 -> E_i = F_4i   (anti-Hermitian,
 // F = (Q - Q^dag)/8, Q = sum of the four leaves starting and ending at x, no trace subtraction).
-__global__ void __launch_bounds__(128) field_strength_kernel(const double2* __restrict__ links, cm3* __restrict__ FS, PrecalcArgs a) {
+__global__ void __launch_bounds__(128, 3) field_strength_kernel(const double2* __restrict__ links, cm3* __restrict__ FS, PrecalcArgs a) {
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   const int k = blockIdx.y;
   if (n >= a.g.V) return;
