@@ -53,8 +53,8 @@
  *   OK_W_BLOCK / OK_W_DS: header, then [block][unit][site_in_block][complex]; the unit order is the list of
  *           stored colour-block rows in csrc/ok_sparse.cuh.  ok_pack_W drops what the format does not keep
  *           (OK_W_DS keeps UL (else LR) as D and UR as S); ok_unpack_W rebuilds the full 12 x 12 matrices.
- *   OK_W_PAULI: header, then [block][9 m + element][site_in_block][complex], m = 0..36 the stored colour matrices of
- *           csrc/ok_pauli.cu (row-major 3 x 3 elements).
+ *   OK_W_PAULI: header, then per block and stored colour matrix m = 0..36 (csrc/ok_pauli.cu) 288 complex numbers: the row-major
+ *           3 x 3 elements in pairs, [pair e/2 : 4][site_in_block][2], then element 8 as [site_in_block] (a lane moves 16 bytes).
  *   nrhs=12 (fp32, OK_W_DENSE only): spinor = 256-byte header, then per-site fp32 records [component/4][2*rhs+part][component%4]
  *           (1152 B, the field), then per-site tensor-core operand records (1152 B: the same numbers scaled per right-hand
  *           side by a power of two and split into two fp16 pieces).  The operand records are what ok_dirac_apply reads; they

@@ -133,6 +133,12 @@ __device__ __forceinline__ void mrhs_split_scaled(float x, float S, __half* hi, 
   *lo = __float2half_rn((y - __half2float(h)) * kMrhsLoScale);
 }
 
+// OK_W_PAULI (ok_pauli.cu): where element e (row-major 3x3) of a stored matrix sits for the site at `lane` of a 32-site block, in
+// complex units from the matrix's base ((block * OK_W_PAULI_MATS + m) * 288).  The elements of a site are kept in PAIRS, so that
+// a lane moves 16 bytes at a time in fp32 (one cp.async / LDS.128 per pair instead of two 8-byte ones): [pair e/2 : 4][site][2],
+// then element 8 as [site].
+__host__ __device__ inline int pauli_elem_index(int e, int lane) { return e < 8 ? (e >> 1) * 64 + lane * 2 + (e & 1) : 256 + lane; }
+
 struct Geom {
   int L[4];
   int V;      // sites

@@ -7,7 +7,7 @@
 // D = (c4/u0) P and S = ((c1+2c2)/2u0) sigma_i P of W_ii; the two sigma components of a pair term) it is stored once, so a
 // site holds 37 colour matrices = 333 complex = 2 664 B in fp32 (dense: 31 104 B; OK_W_CONJ: 5 040 B).
 //
-// Stored matrices, index m (layout [block 32 sites][9 m + element][site][complex]):
+// Stored matrices, index m (layout [block 32 sites][m][element pairs 4][site][2 complex], then [element 8][site]; pauli_elem_index):
 //   0..2  i d0 B_m           3..5  s0 E_m             (Eq. 2.6; D^0, S^0 components sigma_m)
 //   6     U_4                7..9  T_m = (cEE/2u0^4)(U_4 E_m(x+t) - E_m(x) U_4)                              (Eq. 2.7)
 //   10+6i U_i   +1 S.C_0   +2 S.C_k   +3 S.C_l   +4 D.C_k   +5 D.C_l      (Eq. 2.8; i = 0..2, cyclic (i,k,l); hop_blocks_kernel)
@@ -176,7 +176,7 @@ struct PState {
   using vec = typename PV<real>::vec;
   cx acc[12];
   cx phi[12];
-  uint32_t ring;    // fp32 only: shared-memory address of this lane's column of the warp's matrix ring (see use_ct)
+  uint32_t ring16, ring8;   // fp32 only: shared-memory addresses of this lane's 16-byte and 8-byte columns of the warp's matrix ring (see use_ct)
   const cx* W;
   const vec* psi;
   int n, x, y, z, t;
@@ -239,26 +239,34 @@ __device__ __forceinline__ int neighbour_ct(const PState<real>& st) {
   const int zz = wrapp(st.z + kOffC[T][2], st.L2), tt = wrapp(st.t + kOffC[T][3], st.L3);
   return xx + st.L0 * (yy + st.L1 * (zz + st.L2 * tt));
 }
-// where use U's stored matrix lives (own site, or the neighbour's for an opposite-direction term): element e at [e kBlock]
+// where use U's stored matrix lives (own site, or the neighbour's for an opposite-direction term): the matrix's base in its
+// 32-site block and the site's lane there; element e at base[pauli_elem_index(e, lane)] (ok_internal.cuh)
 template <typename real, int U>
-__device__ __forceinline__ const typename PV<real>::cx* matrix_ptr_ct(const PState<real>& st) {
+__device__ __forceinline__ const typename PV<real>::cx* matrix_base_ct(const PState<real>& st, int* lane) {
   constexpr Use u = kUses.u[U];
   const int nm = u.adj ? neighbour_ct<real, u.term>(st) : st.n;
-  return st.W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31) + (size_t)(9 * u.m) * kBlock;
+  *lane = nm & 31;
+  return st.W + ((size_t)(nm >> 5) * kPauliMats + u.m) * (9 * kBlock);
 }
-// fp32: the matrices reach the FMAs through a per-warp ring in shared memory filled by asynchronous 8-byte copies
-// (cp.async, SASS LDGSTS): with packed FMAs a use is ~150 issue slots, too short to hide an L2 / HBM round trip behind the
-// four warps of a scheduler, and registers cannot hold several uses in flight.  Every lane copies and later reads only its own
-// site's elements, so no barrier is needed: cp.async.wait_group orders a lane's reads after its own copies.
-constexpr int kRingDepth = 4;                         // uses in flight per warp
-constexpr int kRingSlotBytes = 9 * kBlock * 8;        // one 3x3 complex fp32 matrix for 32 sites
+// fp32: the matrices reach the FMAs through a per-warp ring in shared memory filled by asynchronous copies (cp.async, SASS
+// LDGSTS; four of 16 bytes -- an element pair -- and one of 8 per matrix and lane): with packed FMAs a use is ~150 issue slots,
+// too short to hide an L2 / HBM round trip behind the four warps of a scheduler, and registers cannot hold several uses in
+// flight.  Every lane copies and later reads only its own site's elements, so no barrier is needed: cp.async.wait_group
+// orders a lane's reads after its own copies.
+#ifndef OK_PAULI_RING
+#define OK_PAULI_RING 4
+#endif
+constexpr int kRingDepth = OK_PAULI_RING;             // uses in flight per warp
+constexpr int kRingSlotBytes = 9 * kBlock * 8;        // one 3x3 complex fp32 matrix for 32 sites: [pair 4][lane][16 B], [lane][8 B]
 template <int U>
 __device__ __forceinline__ void ring_issue_ct(const PState<float>& st, int slot) {
-  const float2* p = matrix_ptr_ct<float, U>(st);
+  int ln;
+  const float2* p = matrix_base_ct<float, U>(st, &ln);
 #pragma unroll
-  for (int e = 0; e < 9; ++e)
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st.ring + slot * kRingSlotBytes + e * (kBlock * 8)), "l"(p + (size_t)e * kBlock)
+  for (int q = 0; q < 4; ++q)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(st.ring16 + slot * kRingSlotBytes + q * (kBlock * 16)), "l"(p + q * 64 + ln * 2)
                  : "memory");
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(st.ring8 + slot * kRingSlotBytes), "l"(p + 256 + ln) : "memory");
 }
 
 template <int U, int UEND, int D>
@@ -285,12 +293,17 @@ __device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
     asm volatile("cp.async.wait_group %0;" ::"n"(kRingDepth - 1) : "memory");
     constexpr int slot = (U - UBEG) % kRingDepth;
 #pragma unroll
-    for (int e = 0; e < 9; ++e)
-      asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(C[e].x), "=f"(C[e].y) : "r"(st.ring + slot * kRingSlotBytes + e * (kBlock * 8)) : "memory");
+    for (int q = 0; q < 4; ++q)
+      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                   : "=f"(C[2 * q].x), "=f"(C[2 * q].y), "=f"(C[2 * q + 1].x), "=f"(C[2 * q + 1].y)
+                   : "r"(st.ring16 + slot * kRingSlotBytes + q * (kBlock * 16))
+                   : "memory");
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(C[8].x), "=f"(C[8].y) : "r"(st.ring8 + slot * kRingSlotBytes) : "memory");
   } else {
-    const cx* p = matrix_ptr_ct<real, U>(st);
+    int ln;
+    const cx* p = matrix_base_ct<real, U>(st, &ln);
 #pragma unroll
-    for (int e = 0; e < 9; ++e) C[e] = __ldg(p + (size_t)e * kBlock);
+    for (int e = 0; e < 9; ++e) C[e] = __ldg(p + pauli_elem_index(e, ln));
   }
   if constexpr (newterm) {
     constexpr int T = u.term;
@@ -339,8 +352,7 @@ __device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
     // this use's slot is free (its values are in registers and consumed): refill it kRingDepth uses ahead
     if constexpr (U + kRingDepth < UEND) ring_issue_ct<U + kRingDepth>(st, (U - UBEG) % kRingDepth);
     asm volatile("cp.async.commit_group;" ::: "memory");
-    return;
-  }
+  } else {
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     cx tv[2][3];
@@ -367,6 +379,7 @@ __device__ __forceinline__ void use_ct(PState<real>& st, real mass) {
     if (h == 0) { placement_ct<real, U, 0, 0>(st, tv); placement_ct<real, U, 1, 0>(st, tv); }
     else { placement_ct<real, U, 0, 1>(st, tv); placement_ct<real, U, 1, 1>(st, tv); }
   }
+  }   // fp64
 }
 
 template <typename real, int U, int UBEG, int UEND, bool MASS>
@@ -408,7 +421,9 @@ apply_pauli_part_kernel(const typename PV<real>::cx* __restrict__ W, const typen
   st.W = W; st.psi = psi;
   if constexpr (sizeof(real) == 4) {
     extern __shared__ __align__(16) uint8_t pauli_ring[];
-    st.ring = (uint32_t)__cvta_generic_to_shared(pauli_ring) + (threadIdx.x >> 5) * (kRingDepth * kRingSlotBytes) + lane * 8;
+    const uint32_t wring = (uint32_t)__cvta_generic_to_shared(pauli_ring) + (threadIdx.x >> 5) * (kRingDepth * kRingSlotBytes);
+    st.ring16 = wring + lane * 16;
+    st.ring8 = wring + 4 * (kBlock * 16) + lane * 8;
   }
   vec* ob = out + (size_t)blk * NC * kBlock + lane;
   if constexpr (PART == 0) {
@@ -495,11 +510,11 @@ __global__ void __launch_bounds__(128) unpack_pauli_kernel(const typename PV<rea
       const int zz = wrapp(z + c_poff2[term][2], a.g.L[2]), tt = wrapp(t + c_poff2[term][3], a.g.L[3]);
       nm = xx + a.g.L[0] * (yy + a.g.L[1] * (zz + a.g.L[2] * tt));
     }
-    const cx* cp = W + (size_t)(nm >> 5) * (kPauliMats * 9) * kBlock + (nm & 31) + (size_t)(9 * u.m) * kBlock;
+    const cx* cp = W + ((size_t)(nm >> 5) * kPauliMats + u.m) * (9 * kBlock);
     cx C[9];
     for (int ca = 0; ca < 3; ++ca)
       for (int cb = 0; cb < 3; ++cb) {
-        cx v = cp[(size_t)(u.adj ? 3 * cb + ca : 3 * ca + cb) * kBlock];
+        cx v = cp[pauli_elem_index(u.adj ? 3 * cb + ca : 3 * ca + cb, nm & 31)];
         if (u.adj) v.y = -v.y;
         C[3 * ca + cb] = v;
       }

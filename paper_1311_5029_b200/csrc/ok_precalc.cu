@@ -716,7 +716,7 @@ __global__ void __launch_bounds__(32 * 4) pauli_store_kernel(const double2* __re
   const int lane = threadIdx.x, m = blockIdx.y * 4 + threadIdx.y;
   if (m >= OK_W_PAULI_MATS) return;
   const int blk = blockIdx.x, n = (blk + a.blk0) * kBlock + lane;
-  cx* dst = W + ((size_t)blk * (OK_W_PAULI_MATS * 9) + 9 * m) * kBlock + lane;
+  cx* dst = W + ((size_t)blk * OK_W_PAULI_MATS + m) * (9 * kBlock);   // + pauli_elem_index(e, lane)
   cm3 C = zero3();
   if (n < a.g.V) {
     const Site x = site_of(n, a.g);
@@ -738,7 +738,7 @@ __global__ void __launch_bounds__(32 * 4) pauli_store_kernel(const double2* __re
     cx v;
     v.x = (real)C.e[e].x;
     v.y = (real)C.e[e].y;
-    dst[(size_t)e * kBlock] = v;
+    dst[pauli_elem_index(e, lane)] = v;
   }
 }
 
