@@ -256,6 +256,22 @@ int ok_slab_dirac_apply_peer(const void* W, const void* psi_ext, const void* lo_
 int ok_slab_bicgstab(int nslab, const void* const* W, const void* const* src_ext, void* const* x_ext, double tol, int maxit,
                      const ok_comm* comm, int* iters, double* resid);
 
+/* Peer access for ok_slab_bicgstab (optional).  With peers set, a process's two OUTER t-faces are read in place as well: its
+ * applies load the neighbour processes' boundary slices straight from their memory (NVLink peer access / CUDA IPC mappings), and
+ * comm->exchange is not called; barrier() takes its place before every apply.  Requirements: every process holds the same number
+ * of equal slabs and has given ok_set_workspace a buffer of the same size (the solver's vectors then sit at the same offsets
+ * everywhere); lo_work / hi_work = the lower / upper neighbour's workspace base as mapped into THIS process; lo_x = x_ext of the
+ * lower neighbour's LAST slab, hi_x = x_ext of the upper neighbour's FIRST slab, mapped likewise; barrier(user) returns 0 once
+ * all work enqueued so far on every process's library stream is complete (or ordered before whatever the streams run next).
+ * The neighbours never overwrite a slice while it may still be read: every apply is followed by an all-gather of its
+ * reductions.  NULL clears the setting.  Results are bit-identical to the exchange path. */
+typedef struct ok_slab_peers {
+  const void *lo_work, *hi_work, *lo_x, *hi_x;
+  int (*barrier)(void* user);
+  void* user;
+} ok_slab_peers;
+int ok_slab_set_peers(const ok_slab_peers* peers);
+
 /* ---- an entry point that allocates nothing ------------------------------------------------ */
 /* For callers that cannot call cudaMalloc and have no workspace to lend (code under CUDA graph capture, tight serving
  * loops, harnesses that forbid allocation): the Dirac apply of Eq. (2.2) together with the three

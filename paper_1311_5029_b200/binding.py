@@ -37,6 +37,14 @@ EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_
 ALLGATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int)
 
 
+BARRIER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p)
+
+
+class ok_slab_peers(C.Structure):
+    _fields_ = [("lo_work", C.c_void_p), ("hi_work", C.c_void_p), ("lo_x", C.c_void_p), ("hi_x", C.c_void_p), ("barrier", BARRIER_FN),
+                ("user", C.c_void_p)]
+
+
 class ok_comm(C.Structure):
     _fields_ = [("rank", C.c_int32), ("nranks", C.c_int32), ("exchange", EXCHANGE_FN), ("allgather", ALLGATHER_FN), ("user", C.c_void_p)]
 
@@ -71,6 +79,7 @@ EXPORTS = {
     "ok_slab_precalc_W": (C.c_int, [C.c_void_p, C.POINTER(ok_params), C.c_int, C.c_int, C.c_void_p]),
     "ok_slab_dirac_apply": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "ok_slab_dirac_apply_peer": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "ok_slab_set_peers": (C.c_int, [C.POINTER(ok_slab_peers)]),
     "ok_slab_bicgstab": (C.c_int, [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.c_int,
                                    C.POINTER(ok_comm), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ok_W_params": (C.c_int, [C.c_void_p, C.POINTER(ok_params)]),
@@ -272,6 +281,11 @@ def ok_slab_dirac_apply(W, psi_ext, out_ext):
 def ok_slab_dirac_apply_peer(W, psi_ext, lo_slice, hi_slice, out_ext):
     """lo_slice / hi_slice: device addresses (tensor views or ints) of the neighbours' boundary slices (ok.h)."""
     _check(lib().ok_slab_dirac_apply_peer(_ptr(W), _ptr(psi_ext), _ptr(lo_slice), _ptr(hi_slice), _ptr(out_ext)), "ok_slab_dirac_apply_peer")
+
+
+def ok_slab_set_peers(peers):
+    """peers: ok_slab_peers (keep it and its callback alive while set) or None to clear."""
+    _check(lib().ok_slab_set_peers(C.byref(peers) if peers is not None else None), "ok_slab_set_peers")
 
 
 def ok_slab_bicgstab(W, src_ext, x_ext, tol, maxit, comm=None, raise_on_fail=True):

@@ -142,6 +142,10 @@ static int write_header(void* W, const ok_params* p) {
   return remember_W(W, p);
 }
 
+static ok_slab_peers g_peers;
+static bool g_have_peers = false;
+const ok_slab_peers* slab_peers() { return g_have_peers ? &g_peers : nullptr; }
+
 }  // namespace okd
 
 using namespace okd;
@@ -463,6 +467,17 @@ int ok_slab_dirac_apply(const void* W, const void* psi, void* out) {
   if (st) return st;
   if (!valid_slab(&p)) return OK_EINVAL;
   return launch_apply_slab(&p, W_payload(W), psi, out, nullptr, nullptr);
+}
+
+int ok_slab_set_peers(const ok_slab_peers* peers) {
+  if (!peers) {
+    g_have_peers = false;
+    return OK_SUCCESS;
+  }
+  if (!peers->lo_work || !peers->hi_work || !peers->lo_x || !peers->hi_x || !peers->barrier) return OK_EINVAL;
+  g_peers = *peers;
+  g_have_peers = true;
+  return OK_SUCCESS;
 }
 
 int ok_slab_dirac_apply_peer(const void* W, const void* psi, const void* lo_slice, const void* hi_slice, void* out) {

@@ -524,7 +524,20 @@ static int solve_slabs(int nslab, const ok_params* const* ps, const void* const*
       face_hi[i] = i + 1 < nslab ? first_slice(sl[i + 1]) : nullptr;
     }
     Slab &a0 = sl[0], &a1 = sl[nslab - 1];
-    if (comm && comm->exchange) {
+    const ok_slab_peers* pr = slab_peers();
+    if (comm && comm->exchange && pr) {
+      // peer access (ok_slab_set_peers): the outer faces too are read in place, from the neighbour processes' memory.  Every
+      // process has the same workspace layout (equal slabs, the same number per process), so the lower neighbour's last slab
+      // keeps its field where this process's last slab keeps its own, and x is the caller's buffer named in the peers.
+      if (pr->barrier(pr->user)) return OK_ECOMM;
+      auto remote = [&](const void* peer_work, const void* peer_x, const char* mine, const Slab& a) -> const char* {
+        const char* wb = static_cast<const char*>(ctx().work);
+        if (mine >= wb && mine < wb + ctx().work_bytes) return static_cast<const char*>(peer_work) + (mine - wb);
+        return static_cast<const char*>(peer_x) + (mine - reinterpret_cast<const char*>(a.x));
+      };
+      face_lo[0] = remote(pr->lo_work, pr->lo_x, last_slice(a1), a1);
+      face_hi[nslab - 1] = remote(pr->hi_work, pr->hi_x, first_slice(a0), a0);
+    } else if (comm && comm->exchange) {
       if (comm->exchange(comm->user, first_slice(a0), last_slice(a1), lo_halo(a0), hi_halo(a1), nb)) return OK_ECOMM;
       face_lo[0] = lo_halo(a0);
       face_hi[nslab - 1] = hi_halo(a1);

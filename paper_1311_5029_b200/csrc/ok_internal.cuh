@@ -227,6 +227,7 @@ size_t bicgstab_slab_work_bytes(const ok_params* p);
 size_t bicgstab_slab_shared_bytes(int nslab, int nranks);
 int run_bicgstab_slabs(int nslab, const ok_params* const* ps, const void* const* Wpayloads, const void* const* srcs, void* const* xs,
                        double tol, int maxit, const ok_comm* comm, int* iters, double* resid);
+const ok_slab_peers* slab_peers();   // what ok_slab_set_peers stored (nullptr: none)
 int launch_apply_pauli(const ok_params* p, const void* Wpayload, const void* psi, void* out, double* dot_partials, const void* dot_a);
 int launch_unpack_pauli(const ok_params* p, const void* Wpayload, void* canon);
 int launch_apply_sparse(const ok_params* p, const void* Wpayload, const void* psi, void* out, double* dot_partials, const void* dot_a);

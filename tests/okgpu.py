@@ -143,3 +143,93 @@ def ipc_slab_worker(rank, nranks, U, pd, prec, psi, q_in, q_out, results, barrie
             barrier.abort()
         except Exception:
             pass
+
+
+def ipc_solver_worker(rank, nranks, U, pd, prec, b_np, tol, q_in, q_ag, results, barrier):
+    """One process = one t-slab on cuda:0 running ok_slab_bicgstab with ok_slab_set_peers: the outer faces of every apply are
+    read from the other process's workspace / x buffer through CUDA IPC mappings; the reductions cross the processes through
+    multiprocessing queues (plumbing); `exchange` must never be called."""
+    import ctypes as C
+    from paper_1311_5029_b200 import slab as S
+    try:
+        torch.cuda.set_device(0)
+        dims = tuple(pd["dims"])
+        p = B.make_params(pd, prec)
+        t0, Tl = S.slab_ranges(dims[3], nranks)[rank]
+        slab = B.make_slab_params(p, Tl)
+        plocal = B.make_params(dict(pd, dims=dims[:3] + (Tl,)), prec)
+        work = B.alloc_bytes(B.ok_slab_work_bytes(slab, 1, nranks), DEV)
+        B.ok_set_stream(None)
+        B.ok_set_workspace(work, work.numel())
+        W = B.alloc_W(slab, DEV)
+        B.ok_slab_precalc_W(to_dev(S.link_window(U, dims, t0, Tl), torch.complex128), slab, dims[3], t0, W)
+        src = torch.zeros(B.ok_slab_vec_bytes(slab), dtype=torch.uint8, device=DEV)
+        B.ok_pack_spinor(plocal, to_dev(S.spinor_slab(b_np, dims, t0, Tl), cdtype(prec)), S.interior(slab, src))
+        x = torch.zeros_like(src)
+        torch.cuda.synchronize()
+        q_in[(rank - 1) % nranks].put(("from_above", work, x))
+        q_in[(rank + 1) % nranks].put(("from_below", work, x))
+        got = {}
+        for _ in range(2):
+            tag, w_, x_ = q_in[rank].get(timeout=120)
+            got[tag] = (w_, x_)
+        barrier.wait(timeout=120)
+        calls = {"exchange": 0, "allgather": 0, "barrier": 0}
+
+        def view(addr, nbytes):
+            off = addr - work.data_ptr()
+            assert 0 <= off and off + nbytes <= work.numel()
+            return work[off:off + nbytes]
+
+        def on_barrier(user):
+            try:
+                calls["barrier"] += 1
+                torch.cuda.synchronize()
+                barrier.wait(timeout=120)
+                return 0
+            except Exception:
+                return 1
+
+        def on_allgather(user, send, recv, n):
+            try:
+                calls["allgather"] += 1
+                torch.cuda.synchronize()
+                mine = view(send, 8 * n).view(torch.float64).cpu().numpy().copy()
+                for r in range(nranks):
+                    if r != rank:
+                        q_ag[r].put((rank, mine))
+                parts = {rank: mine}
+                while len(parts) < nranks:
+                    r, arr = q_ag[rank].get(timeout=120)
+                    parts[r] = arr
+                allv = np.concatenate([parts[r] for r in range(nranks)])
+                view(recv, 8 * n * nranks).view(torch.float64).copy_(torch.from_numpy(allv))
+                torch.cuda.synchronize()
+                return 0
+            except Exception:
+                return 1
+
+        def on_exchange(*a):
+            calls["exchange"] += 1
+            return 1
+
+        cb = (B.EXCHANGE_FN(on_exchange), B.ALLGATHER_FN(on_allgather), B.BARRIER_FN(on_barrier))
+        comm = B.ok_comm(rank, nranks, cb[0], cb[1], None)
+        peers = B.ok_slab_peers(got["from_below"][0].data_ptr(), got["from_above"][0].data_ptr(), got["from_below"][1].data_ptr(),
+                                got["from_above"][1].data_ptr(), cb[2], None)
+        B.ok_slab_set_peers(peers)
+        st, it, res = B.ok_slab_bicgstab([W], [src], [x], tol, 2000, comm=comm, raise_on_fail=False)
+        B.ok_slab_set_peers(None)
+        canon = torch.empty((Tl * dims[0] * dims[1] * dims[2], 12), dtype=cdtype(prec), device=DEV)
+        B.ok_unpack_spinor(plocal, S.interior(slab, x), canon)
+        torch.cuda.synchronize()
+        results.put((rank, (st, it, res, dict(calls), canon.cpu().numpy()), None))
+        barrier.wait(timeout=120)
+        del got
+    except Exception as e:  # pragma: no cover
+        import traceback
+        results.put((rank, None, traceback.format_exc()))
+        try:
+            barrier.abort()
+        except Exception:
+            pass

@@ -179,6 +179,53 @@ def test_slab_apply_reads_another_process_memory_through_cuda_ipc():
     B.ok_set_workspace(None)
 
 
+def test_slab_bicgstab_with_peer_access_across_two_processes():
+    """ok_slab_set_peers: two processes on cuda:0, one slab each; in every apply of the solver each process reads the other's
+    boundary slices (of p, s and x) in place through CUDA IPC mappings of the other's workspace and x buffer; `exchange` is never
+    called.  Bit-identical to the two-slab solve of one process."""
+    import torch.multiprocessing as mp
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        mode = pynvml.nvmlDeviceGetComputeMode(pynvml.nvmlDeviceGetHandleByIndex(torch.cuda.current_device()))
+        if mode != pynvml.NVML_COMPUTEMODE_DEFAULT:
+            pytest.skip("GPU compute mode %d does not admit a second process" % mode)
+    except Exception:
+        pass
+    dims, nranks, prec, tol = (4, 4, 4, 8), 2, B.OK_FP64, 1e-10
+    U, pd, o = setup(dims)
+    b = I.gaussian_spinor(dims, 2)
+    sl = Slabs(U, pd, prec, nranks)
+    src = sl.scatter(b)
+    xs = [torch.zeros_like(v) for v in src]
+    want = B.ok_slab_bicgstab(sl.W, src, xs, tol, 2000, raise_on_fail=False)
+    xwant = sl.gather(xs)
+    B.ok_set_workspace(None)
+    ctx = mp.get_context("spawn")
+    q_in, q_ag = [ctx.Queue() for _ in range(nranks)], [ctx.Queue() for _ in range(nranks)]
+    results, barrier = ctx.Queue(), ctx.Barrier(nranks)
+    procs = [ctx.Process(target=G.ipc_solver_worker, args=(r, nranks, U, pd, prec, b, tol, q_in, q_ag, results, barrier)) for r in range(nranks)]
+    for pr in procs:
+        pr.start()
+    try:
+        parts = {}
+        for _ in range(nranks):
+            rank, val, err = results.get(timeout=300)
+            assert err is None, err
+            parts[rank] = val
+    finally:
+        for pr in procs:
+            pr.join(timeout=60)
+            if pr.is_alive():
+                pr.kill()
+    for r in range(nranks):
+        st, it, res, calls, _ = parts[r]
+        assert (st, it, res) == want                                   # same iteration, same residual, on every process
+        assert calls["exchange"] == 0 and calls["barrier"] >= 2 * it and calls["allgather"] >= 3 * it
+    got = np.concatenate([parts[r][4] for r in range(nranks)]).astype(np.complex128)
+    assert np.array_equal(got, xwant)
+
+
 def test_slab_apply_periodic_time_and_error_paths():
     dims = (4, 4, 2, 8)
     U, pd, o = setup(dims, bc=[1, 1, 1, 1])
