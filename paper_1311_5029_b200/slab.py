@@ -93,6 +93,10 @@ class TorchComm:
         """recv[r * n : (r + 1) * n] = rank r's send."""
         if self.nranks == 1:
             recv.copy_(send)
+        elif send.is_cuda and self.dist.get_backend(self.group) == "gloo":   # gloo has no all-gather on device tensors: stage on the host
+            host = self.torch.empty(recv.numel(), dtype=recv.dtype)
+            self.dist.all_gather_into_tensor(host, send.cpu(), group=self.group)
+            recv.copy_(host)
         else:
             self.dist.all_gather_into_tensor(recv, send, group=self.group)
 
@@ -120,3 +124,37 @@ class TorchComm:
         except Exception as e:
             self.error = e
             return 1
+
+
+class PeerLinks:
+    """ok_slab_peers over torch (include/ok.h: ok_slab_set_peers): maps the two t-neighbour processes' workspace and x buffers
+    into this process -- CUDA IPC through torch's own tensor sharing, i.e. NVLink peer access when the neighbour sits on another
+    GPU -- and provides the barrier callback.  Every rank passes its workspace tensor and the x_ext tensors of its first and
+    last slab; keep this object (and the tensors) alive while the peers are set, and delete it before the buffers are freed."""
+
+    def __init__(self, dist, work, x_first, x_last, group=None, stream=None):
+        import torch
+        from torch.multiprocessing.reductions import reduce_tensor
+        self.torch, self.dist, self.group, self.stream = torch, dist, group, stream
+        rank, n = dist.get_rank(group), dist.get_world_size(group)
+        mine = tuple(reduce_tensor(t) for t in (work, x_first, x_last))      # picklable (rebuild function, IPC handle) pairs
+        everyone = [None] * n
+        dist.all_gather_object(everyone, mine, group=group)
+        opened = lambda h: h[0](*h[1])
+        lo, hi = everyone[(rank - 1) % n], everyone[(rank + 1) % n]
+        self.lo_work, self.lo_x = opened(lo[0]), opened(lo[2])                # the lower neighbour's LAST slab
+        self.hi_work, self.hi_x = opened(hi[0]), opened(hi[1])                # the upper neighbour's FIRST slab
+        self.error = None
+        self._bar = B.BARRIER_FN(self._barrier)
+        self.struct = B.ok_slab_peers(self.lo_work.data_ptr(), self.hi_work.data_ptr(), self.lo_x.data_ptr(), self.hi_x.data_ptr(),
+                                      self._bar, None)
+
+    def _barrier(self, user):
+        try:   # everything enqueued so far is complete on every rank before anyone goes on
+            (self.stream.synchronize() if self.stream is not None else self.torch.cuda.synchronize())
+            self.dist.barrier(group=self.group)
+            return 0
+        except Exception as e:
+            self.error = e
+            return 1
+

@@ -233,3 +233,50 @@ def ipc_solver_worker(rank, nranks, U, pd, prec, b_np, tol, q_in, q_ag, results,
             barrier.abort()
         except Exception:
             pass
+
+
+def torch_peer_solver_worker(rank, nranks, port, U, pd, prec, b_np, tol, results):
+    """The same solve through the package's own plumbing: torch.distributed (gloo here: both ranks share cuda:0) for the
+    reductions and the barrier, slab.PeerLinks for the mappings, slab.TorchComm for ok_comm."""
+    import os
+    import torch.distributed as dist
+    from paper_1311_5029_b200 import slab as S
+    try:
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(nranks))
+        dist.init_process_group("gloo", rank=rank, world_size=nranks)
+        torch.cuda.set_device(0)
+        dims = tuple(pd["dims"])
+        p = B.make_params(pd, prec)
+        t0, Tl = S.slab_ranges(dims[3], nranks)[rank]
+        slab = B.make_slab_params(p, Tl)
+        plocal = B.make_params(dict(pd, dims=dims[:3] + (Tl,)), prec)
+        work = B.alloc_bytes(B.ok_slab_work_bytes(slab, 1, nranks), DEV)
+        B.ok_set_stream(None)
+        B.ok_set_workspace(work, work.numel())
+        W = B.alloc_W(slab, DEV)
+        B.ok_slab_precalc_W(to_dev(S.link_window(U, dims, t0, Tl), torch.complex128), slab, dims[3], t0, W)
+        src = torch.zeros(B.ok_slab_vec_bytes(slab), dtype=torch.uint8, device=DEV)
+        B.ok_pack_spinor(plocal, to_dev(S.spinor_slab(b_np, dims, t0, Tl), cdtype(prec)), S.interior(slab, src))
+        x = torch.zeros_like(src)
+        torch.cuda.synchronize()
+        comm = S.TorchComm(dist)
+        comm.register(work, x)
+        calls = [0]
+        orig = comm.exchange_tensors
+        comm.exchange_tensors = lambda *a: (calls.__setitem__(0, calls[0] + 1), orig(*a))
+        links = S.PeerLinks(dist, work, x, x)
+        B.ok_slab_set_peers(links.struct)
+        st, it, res = B.ok_slab_bicgstab([W], [src], [x], tol, 2000, comm=comm.struct, raise_on_fail=False)
+        B.ok_slab_set_peers(None)
+        assert comm.error is None and links.error is None, (comm.error, links.error)
+        canon = torch.empty((Tl * dims[0] * dims[1] * dims[2], 12), dtype=cdtype(prec), device=DEV)
+        B.ok_unpack_spinor(plocal, S.interior(slab, x), canon)
+        torch.cuda.synchronize()
+        results.put((rank, (st, it, res, calls[0], canon.cpu().numpy()), None))
+        dist.barrier()
+        del links
+        dist.barrier()
+        dist.destroy_process_group()
+    except Exception:  # pragma: no cover
+        import traceback
+        results.put((rank, None, traceback.format_exc()))

@@ -224,6 +224,31 @@ def test_slab_bicgstab_with_peer_access_across_two_processes():
         assert calls["exchange"] == 0 and calls["barrier"] >= 2 * it and calls["allgather"] >= 3 * it
     got = np.concatenate([parts[r][4] for r in range(nranks)]).astype(np.complex128)
     assert np.array_equal(got, xwant)
+    # the same through the package's own plumbing: torch.distributed + slab.TorchComm + slab.PeerLinks
+    import socket
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    results = ctx.Queue()
+    procs = [ctx.Process(target=G.torch_peer_solver_worker, args=(r, nranks, port, U, pd, prec, b, tol, results)) for r in range(nranks)]
+    for pr in procs:
+        pr.start()
+    try:
+        parts = {}
+        for _ in range(nranks):
+            rank, val, err = results.get(timeout=300)
+            assert err is None, err
+            parts[rank] = val
+    finally:
+        for pr in procs:
+            pr.join(timeout=60)
+            if pr.is_alive():
+                pr.kill()
+    for r in range(nranks):
+        assert parts[r][:3] == want and parts[r][3] == 0               # exchange_tensors never ran
+    got = np.concatenate([parts[r][4] for r in range(nranks)]).astype(np.complex128)
+    assert np.array_equal(got, xwant)
 
 
 def test_slab_apply_periodic_time_and_error_paths():
