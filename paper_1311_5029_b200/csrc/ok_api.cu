@@ -288,6 +288,17 @@ static int apply_host_pipelined(const ok_params& p, const void* W, const char* p
   const size_t sb = slice_sites * 12 * 2 * real_bytes(&p);          // bytes of a time slice, canonical and internal alike
   int t0[kMaxChunks + 1];
   for (int c = 0; c <= n; ++c) t0[c] = (int)((long long)c * T / n);
+  if (n == kMaxChunks && T >= 64) {
+    // small chunks at both ends, large ones in the middle: the first apply starts after three short copies (chunks n-1, 0, 1)
+    // and only a short result is still on its way back when the last apply ends; in between the copies run ahead of the applies
+    static const int w[kMaxChunks] = {1, 1, 2, 4, 6, 6, 6, 6, 6, 6, 6, 6, 4, 2, 1, 1};   // sum 64
+    int acc = 0;
+    for (int c = 0; c < n; ++c) {
+      t0[c] = (int)((long long)acc * T / 64);
+      acc += w[c];
+    }
+    t0[n] = T;
+  }
   OK_CUDA(cudaEventRecord(ev_start, st));
   OK_CUDA(cudaStreamWaitEvent(s_in, ev_start, 0));
   OK_CUDA(cudaStreamWaitEvent(s_out, ev_start, 0));
